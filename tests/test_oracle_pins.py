@@ -1,0 +1,322 @@
+"""Pins of the CPU oracle against things other than itself (SURVEY.md 8(c) "Pins").
+
+Every test here runs on CPU.  The independent references are: the DFT definition typed out with
+numpy on tiny inputs, numpy's library FFT, closed forms, invariants and symmetries of the
+method, a generic least-squares solver, and data simulated by `synth` with the library FFT.
+"""
+import numpy as np
+import pytest
+
+from paper_2202_03144_b200 import synth
+
+RNG = np.random.default_rng(12345)
+
+
+def crandn(*shape):
+    return RNG.standard_normal(shape) + 1j * RNG.standard_normal(shape)
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.ravel(a) - np.ravel(b)) / max(np.linalg.norm(np.ravel(b)), 1e-300))
+
+
+# ------------------------------------------------------------------------------------- FFT pins
+def test_fft_vs_dft_definition_8x8(oracle_mod):
+    x = crandn(8, 8)
+    u = np.arange(8)
+    w = np.exp(-2j * np.pi * np.outer(u, u) / 8)            # the definition, typed here
+    want = w @ x @ w.T
+    assert rel(oracle_mod.dft2_naive(x), want) < 1e-14
+    assert rel(oracle_mod.fft2(x), want) < 1e-14
+    assert rel(oracle_mod.fft2(want, inverse=True), x) < 1e-14
+    assert rel(oracle_mod.dft2_naive(want, inverse=True), x) < 1e-14
+
+
+def test_fft_rows_vs_naive_64(oracle_mod):
+    x = crandn(16, 16)
+    assert rel(oracle_mod.fft2(x), oracle_mod.dft2_naive(x)) < 1e-13
+
+
+@pytest.mark.parametrize("n", [64, 128, 256, 512])
+def test_fft_vs_library(oracle_mod, n):
+    x = crandn(n, n)
+    assert rel(oracle_mod.fft2(x), np.fft.fft2(x)) < 1e-13
+    assert rel(oracle_mod.fft2(x, inverse=True), np.fft.ifft2(x)) < 1e-13
+
+
+def test_fft_asymmetric_input_not_transposed(oracle_mod):
+    """A transposed or sign-flipped transform fails here: single off-axis plane wave."""
+    n = 32
+    y, x = np.mgrid[0:n, 0:n]
+    wave = np.exp(2j * np.pi * (3 * y + 5 * x) / n)         # peak must land at [3, 5], value n^2
+    f = oracle_mod.fft2(wave)
+    want = np.zeros((n, n), complex)
+    want[3, 5] = n * n
+    assert np.abs(f - want).max() < 1e-9
+    d = np.zeros((n, n), complex)
+    d[2, 7] = 1.0                                           # shifted delta -> pure phase ramp
+    assert np.abs(oracle_mod.fft2(d) - np.exp(-2j * np.pi * (2 * y + 7 * x) / n)).max() < 1e-12
+
+
+def test_fft_parseval_roundtrip_linearity(oracle_mod):
+    n = 64
+    a, b = crandn(n, n), crandn(n, n)
+    fa, fb = oracle_mod.fft2(a), oracle_mod.fft2(b)
+    assert abs(np.sum(np.abs(fa) ** 2) / (n * n * np.sum(np.abs(a) ** 2)) - 1) < 1e-14
+    assert rel(oracle_mod.fft2(fa, inverse=True), a) < 1e-14
+    assert rel(oracle_mod.fft2(2.5 * a - 1j * b), 2.5 * fa - 1j * fb) < 1e-14
+
+
+# ------------------------------------------------------------------------- modulus projection
+def test_projection_modulus_phase_idempotent(oracle_mod):
+    n, k = 16, 3
+    phi = crandn(k, n, n)
+    inten = RNG.random((n, n)) * 50
+    out, err = oracle_mod.modulus_project(phi, inten)
+    assert np.allclose(np.sum(np.abs(out) ** 2, 0), inten, rtol=1e-13)          # |Phi'|^2 = I
+    assert np.abs(np.angle(out * np.conj(phi))).max() < 1e-12                   # phases kept
+    ratio = np.abs(out) / np.abs(phi)
+    assert np.allclose(ratio, ratio[0][None], rtol=1e-12)                       # one scale per pixel
+    out2, err2 = oracle_mod.modulus_project(out, inten)
+    assert rel(out2, out) < 1e-14 and err2 < 1e-20                              # idempotent
+    a = np.sqrt(np.sum(np.abs(phi) ** 2, 0))
+    assert abs(err - np.sum((np.sqrt(inten) - a) ** 2)) < 1e-10 * err
+
+
+def test_projection_mask_and_zero_amplitude(oracle_mod):
+    n = 8
+    phi = crandn(2, n, n)
+    phi[:, 1, 2] = 0                                                            # A = 0 pixel (R2)
+    inten = RNG.random((n, n)) * 9 + 1
+    inten[3, 4] = -1.0                                                          # masked (R3)
+    out, err = oracle_mod.modulus_project(phi, inten)
+    assert np.array_equal(out[:, 3, 4], phi[:, 3, 4])
+    assert out[0, 1, 2] == np.sqrt(inten[1, 2]) and out[1, 1, 2] == 0
+    a = np.sqrt(np.sum(np.abs(phi) ** 2, 0))
+    ok = inten >= 0
+    assert abs(err - np.sum((np.sqrt(inten[ok]) - a[ok]) ** 2)) < 1e-12 * err
+    # uint16 sentinel is the same mask
+    cnt = np.full((n, n), 7, np.uint16)
+    cnt[3, 4] = 65535
+    out_u, _ = oracle_mod.modulus_project(phi, cnt)
+    assert np.array_equal(out_u[:, 3, 4], phi[:, 3, 4])
+    assert np.allclose(np.sum(np.abs(out_u) ** 2, 0)[cnt < 65535], 7.0)
+
+
+def test_projection_relaxed_closed_form(oracle_mod):
+    n = 16
+    phi = crandn(1, n, n) * 3
+    inten = RNG.random((n, n)) * 20
+    exact, err = oracle_mod.modulus_project(phi, inten, 0.0)
+    e = err / (n * n)
+    same, _ = oracle_mod.modulus_project(phi, inten, pbound=e * 1.01)           # inside the bound
+    assert np.array_equal(same, phi)
+    pb = e * 0.3
+    out, _ = oracle_mod.modulus_project(phi, inten, pbound=pb)
+    _, err_after = oracle_mod.modulus_project(out, inten, 0.0)
+    assert abs(err_after / (n * n) - pb) < 1e-12 * pb                           # lands on the bound
+    r = np.sqrt(pb / e)
+    assert rel(out, (1 - r) * exact + r * phi) < 1e-14
+
+
+# ------------------------------------------------------------------- whole-cycle invariants
+def f64_scan(n=16, h=40, side=4, step=6, k=1, probe_kind="disk"):
+    s = synth.make_custom(n, h, side, step, k=k, probe_kind=probe_kind)
+    lam = np.concatenate([l for _, l in synth.model_intensity(s.obj_true, s.probe_true, s.pos, 1)])
+    return s, lam                                           # float64 noiseless intensities
+
+
+@pytest.mark.parametrize("alg,k", [("DM", 1), ("EPIE_MB", 1), ("LSQML", 1), ("LSQML", 3), ("DM", 2)])
+def test_ground_truth_is_fixed_point_with_zero_error(oracle_mod, alg, k):
+    s, lam = f64_scan(k=k)
+    o = oracle_mod.Oracle(s.obj_true, s.probe_true, s.pos, lam, dict(batch_size=5))
+    o.iterate(alg, 2)
+    assert max(o.err) < 1e-25
+    assert rel(o.O, s.obj_true) < 1e-13 and rel(o.P, s.probe_true) < 1e-13
+    assert o.eval_error() < 1e-25
+    if alg == "DM":
+        want = np.stack([s.probe_true * s.obj_true[None, y:y + s.n, x:x + s.n] for y, x in s.pos])
+        assert rel(o.psi, want) < 1e-13
+
+
+def test_dm_all_masked_closed_forms(oracle_mod):
+    """With no Fourier constraint Pi_M = id, so psi_new = P O_j, O is unchanged, and the lagged
+    probe update from incoming psi_j = Q O_j is the closed form (d_P Q + eps P)/(d_P + eps)."""
+    s, lam = f64_scan()
+    n = s.n
+    obj = s.obj_true * (1 + 0.1 * crandn(*s.obj_true.shape))
+    q = s.probe_true * (1 + 0.2 * crandn(*s.probe_true.shape))
+    o = oracle_mod.Oracle(obj, s.probe_true, s.pos, -np.ones_like(lam))
+    o.psi = np.stack([q * obj[None, y:y + n, x:x + n] for y, x in s.pos]).astype(complex)
+    p_old, eps = o.P.copy(), o.eps_P
+    o.iterate("DM", 1)
+    want_psi = np.stack([p_old * obj[None, y:y + n, x:x + n] for y, x in s.pos])
+    assert rel(o.psi, want_psi) < 1e-14
+    assert rel(o.O, obj) < 1e-14
+    d_p = sum(np.abs(obj[y:y + n, x:x + n]) ** 2 for y, x in s.pos)
+    assert rel(o.P, (d_p * q + eps * p_old) / (d_p + eps)) < 1e-14
+    assert eps == pytest.approx(1e-2 * len(s.pos) * np.max(np.abs(obj) ** 2))   # R5 constants
+    assert o.eps_O == pytest.approx(1e-2 * np.max(np.abs(p_old) ** 2))
+
+
+def test_epie_single_frame_closed_form_with_library_fft(oracle_mod):
+    """J = 1, alpha = 1, delta -> 0, probe frozen: O_new = psi_F / P on the probe support, with
+    psi_F = ifft2(fft2(P O) sqrt(I) / |fft2(P O)|) evaluated here with numpy's FFT."""
+    s, lam = f64_scan(side=1)
+    obj0 = 1 + 0.05 * crandn(*s.obj_true.shape)
+    o = oracle_mod.Oracle(obj0, s.probe_true, s.pos, lam,
+                          dict(delta_obj=1e-30, probe_start=10 ** 9), keep_revised=True)
+    o.iterate("EPIE_MB", 1)
+    (y, x), n, p = s.pos[0], s.n, s.probe_true[0]
+    f = np.fft.fft2(p * obj0[y:y + n, x:x + n])
+    psi_f = np.fft.ifft2(f * np.sqrt(lam[0]) / np.abs(f))
+    assert rel(o.revised[0, 0], psi_f) < 1e-12
+    sup = np.abs(p) > 0
+    assert rel(o.O[y:y + n, x:x + n][sup], (psi_f / np.where(sup, p, 1))[sup]) < 1e-10
+    assert np.array_equal(o.O[y:y + n, x:x + n][~sup], obj0[y:y + n, x:x + n][~sup])
+    assert o.err[0] == pytest.approx(np.sum((np.sqrt(lam[0]) - np.abs(f)) ** 2) / lam.sum(), rel=1e-12)
+
+
+def test_dm_first_iteration_equals_full_batch_epie(oracle_mod):
+    """From psi0 = P O_j the reflector is the identity, so DM's first iteration and one full-batch
+    ePIE step (alpha 1) give the same revised waves and, with delta_obj = delta_blend, the same
+    object; DM's lagged probe update returns P unchanged.  Two code paths, one answer."""
+    s, lam = f64_scan(n=16, h=48, side=5, step=5)
+    cnt = RNG.poisson(lam * 50).astype(np.float64)
+    p0 = s.probe_true * np.sqrt(50)
+    dm = oracle_mod.Oracle(s.obj0, p0, s.pos, cnt, dict(delta_blend=0.37), keep_revised=True)
+    ep = oracle_mod.Oracle(s.obj0, p0, s.pos, cnt, dict(delta_obj=0.37, probe_start=10 ** 9), keep_revised=True)
+    dm.iterate("DM", 1)
+    ep.iterate("EPIE_MB", 1)
+    assert rel(dm.revised, ep.revised) < 1e-14
+    assert rel(dm.psi, ep.revised) < 1e-14
+    assert rel(dm.O, ep.O) < 1e-13
+    assert rel(dm.P, p0) < 1e-13
+    assert dm.err[0] == pytest.approx(ep.err[0], rel=1e-12)
+    # the overlap formula applied to the revised waves, summed here with plain numpy slices
+    n = s.n
+    num = np.zeros_like(s.obj0)
+    den = np.zeros(s.obj0.shape)
+    for j, (y, x) in enumerate(s.pos):
+        num[y:y + n, x:x + n] += np.conj(p0[0]) * ep.revised[j, 0]
+        den[y:y + n, x:x + n] += np.abs(p0[0]) ** 2
+    eps = 0.37 * np.max(np.abs(p0) ** 2)
+    assert rel(dm.O, (num + eps * s.obj0) / (den + eps)) < 1e-13
+
+
+def test_lsqml_direction_and_step_vs_generic_least_squares(oracle_mod):
+    """LSQML-style moves along the ePIE directions (O_l - O = a dO, P_l - P = b dP_k) and (a, b)
+    solves the Tikhonov-regularised real least-squares problem of reading R9, here handed as an
+    explicit stacked system to numpy.linalg.lstsq (J = 4, N = 8, K = 2)."""
+    s, lam = f64_scan(n=8, h=20, side=2, step=4, k=2)
+    cnt = RNG.poisson(lam * 30).astype(np.float64)
+    p0 = s.probe_true * np.sqrt(30)
+    obj0 = 1 + 0.1 * crandn(*s.obj_true.shape)
+    lam_t = 0.1
+    ep = oracle_mod.Oracle(obj0, p0, s.pos, cnt, keep_revised=True)
+    ls = oracle_mod.Oracle(obj0, p0, s.pos, cnt, dict(lsq_lambda=lam_t))
+    ep.iterate("EPIE_MB", 1)
+    ls.iterate("LSQML", 1)
+    d_o, d_p = ep.O - obj0, ep.P - p0
+    a, b = ls.steps[0]
+    assert rel(ls.O - obj0, a * d_o) < 1e-12 and rel(ls.P - p0, b * d_p) < 1e-12
+    n = s.n
+    u, v, c = [], [], []
+    for j, (y, x) in enumerate(s.pos):
+        oj, doj = obj0[y:y + n, x:x + n], d_o[y:y + n, x:x + n]
+        u.append(p0 * doj[None])
+        v.append(d_p * oj[None])
+        c.append(ep.revised[j] - p0 * oj[None])
+    u, v, c = (np.ravel(np.stack(z)) for z in (u, v, c))
+    ri = lambda z: np.concatenate([z.real, z.imag])
+    a11, a22 = np.vdot(u, u).real, np.vdot(v, v).real
+    m = np.stack([np.concatenate([ri(u), [np.sqrt(lam_t * a11), 0]]),
+                  np.concatenate([ri(v), [0, np.sqrt(lam_t * a22)]])], 1)
+    sol = np.linalg.lstsq(m, np.concatenate([ri(c), [0, 0]]), rcond=None)[0]
+    assert a == pytest.approx(sol[0], rel=1e-10) and b == pytest.approx(sol[1], rel=1e-10)
+    # frozen probe: a = b1 / (A11 (1 + lambda)), b = 0
+    lf = oracle_mod.Oracle(obj0, p0, s.pos, cnt, dict(lsq_lambda=lam_t, probe_start=10 ** 9))
+    lf.iterate("LSQML", 1)
+    assert lf.steps[0][1] == 0
+    assert lf.steps[0][0] == pytest.approx(np.vdot(u, c).real / (a11 * (1 + lam_t)), rel=1e-10)
+    assert rel(lf.P, p0) == 0
+
+
+def test_zero_modes_reduce_to_single_mode(oracle_mod):
+    s, lam = f64_scan(k=1)
+    cnt = RNG.poisson(lam * 20).astype(np.float64)
+    p1 = s.probe_true * np.sqrt(20)
+    p3 = np.concatenate([p1, np.zeros_like(p1), np.zeros_like(p1)])
+    for alg in ("LSQML", "EPIE_MB", "DM"):
+        a = oracle_mod.Oracle(s.obj0, p1, s.pos, cnt, dict(batch_size=6)).iterate(alg, 3)
+        b = oracle_mod.Oracle(s.obj0, p3, s.pos, cnt, dict(batch_size=6)).iterate(alg, 3)
+        assert rel(b.O, a.O) < 1e-13 and rel(b.P[0], a.P[0]) < 1e-13 and np.abs(b.P[1:]).max() == 0
+        assert np.allclose(a.err, b.err, rtol=1e-12)
+
+
+# ------------------------------------------------------------------------------- symmetries
+@pytest.mark.parametrize("alg", ["DM", "EPIE_MB", "LSQML"])
+def test_symmetries(oracle_mod, alg):
+    s, lam = f64_scan(n=16, h=44, side=4, step=6)
+    cnt = RNG.poisson(lam * 40).astype(np.float64)
+    p0 = s.probe_true * np.sqrt(40)
+    obj0 = 1 + 0.05 * crandn(*s.obj_true.shape)
+    par = dict(batch_size=4, pbound=0.05 if alg == "DM" else 0.0)
+    base = oracle_mod.Oracle(obj0, p0, s.pos, cnt, par).iterate(alg, 3)
+    # (1) translating positions and object together changes nothing
+    big = np.ones((60, 60), complex)
+    big[7:51, 9:53] = obj0
+    sh = oracle_mod.Oracle(big, p0, s.pos + np.array([7, 9], np.int32), cnt, par).iterate(alg, 3)
+    assert rel(sh.O[7:51, 9:53], base.O) < 1e-13 and rel(sh.P, base.P) < 1e-13
+    # (2) global phase of a frozen probe comes out conjugated on the object
+    th = np.exp(0.7j)
+    fz = dict(par, probe_start=10 ** 9)
+    b0 = oracle_mod.Oracle(obj0, p0, s.pos, cnt, fz).iterate(alg, 2)
+    b1 = oracle_mod.Oracle(obj0 * np.conj(th), p0 * th, s.pos, cnt, fz).iterate(alg, 2)
+    assert rel(b1.O * th, b0.O) < 1e-13
+    # (3) uint16 and float copies of the same integer counts agree exactly
+    u = oracle_mod.Oracle(obj0, p0, s.pos, cnt.astype(np.uint16), par).iterate(alg, 3)
+    assert np.array_equal(u.O, base.O) and np.array_equal(u.P, base.P)
+    # (4) frame order only changes summation rounding (full batch)
+    perm = RNG.permutation(len(s.pos))
+    fb = dict(par, batch_size=0)
+    c0 = oracle_mod.Oracle(obj0, p0, s.pos, cnt, fb).iterate(alg, 2)
+    c1 = oracle_mod.Oracle(obj0, p0, s.pos[perm], cnt[perm], fb).iterate(alg, 2)
+    assert rel(c1.O, c0.O) < 1e-12 and rel(c1.P, c0.P) < 1e-12
+
+
+def test_strided_batches(oracle_mod):
+    b = oracle_mod.batches(10, 4)
+    assert [list(x) for x in b] == [[0, 3, 6, 9], [1, 4, 7], [2, 5, 8]]                # n_b = 3
+    assert [len(x) for x in oracle_mod.batches(20000, 512)] == [500] * 40            # cfg3
+    assert [list(x) for x in oracle_mod.batches(5, 2, order=[4, 3, 2, 1, 0])] == [[4, 3], [2, 1], [0]]
+    assert len(oracle_mod.batches(7, 0)) == 1
+
+
+# ------------------------------------------------------------------------------ convergence
+def test_cfg0_dm_error_history_against_survey_values(oracle_mod):
+    s = synth.make_config(0)
+    gold = np.loadtxt("tests/golden/survey_x12_cfg0.txt")[:, 1]
+    for ps in (10 ** 9, 0):
+        o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(probe_start=ps)).iterate("DM", 10)
+        e = np.array(o.err)
+        assert np.all(np.diff(e[:8]) < 0), e                 # decreasing while far from the floor
+        assert e[-1] < 0.1 * e[0]
+        assert np.all((e > gold / 2) & (e < gold * 2)), e    # same order as the survey prototype
+
+
+@pytest.mark.parametrize("alg", ["EPIE_MB", "LSQML"])
+def test_minibatch_monotone_on_noiseless_data(oracle_mod, alg):
+    s = synth.make_config(0)
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(batch_size=16)).iterate(alg, 50)
+    e = np.array(o.err)
+    assert np.all(np.diff(e) < 0), e
+    assert e[-1] < 1e-3 * e[0]
+
+
+def test_float_build_tracks_double(oracle_mod):
+    """Precision floor: the same oracle compiled in float stays within the parity tolerances."""
+    s = synth.make_config(0)
+    d = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities).iterate("DM", 10)
+    f = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, precision="f32").iterate("DM", 10)
+    assert rel(f.O, d.O) < 1e-4 and rel(f.psi, d.psi) < 1e-4

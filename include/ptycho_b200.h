@@ -1,0 +1,154 @@
+/* ptycho_b200.h -- C ABI of the B200-native ptychographic projection cycle.
+ *
+ * The calls follow the paper's step-mode API  init / step / fetch object / fetch probe / post
+ * (PAPER.md:96 and Listing 1: epieinit, epiestep, epieresobj, epieresprobe,
+ * epiepost; "analogous calls for DM and LSQML", Fig. 3) and BASELINE.json north_star:
+ * "init(object, probe, positions, intensities), iterate(algorithm, n), fetch object/probe/error".
+ * The state (object, probe, exit waves) stays on the GPU between calls and can be fetched at
+ * any iteration.  The shape of this header is SURVEY.md section 8(b).
+ *
+ * Notation: N frame side, J scan positions, K probe modes, object O
+ * (H x W), probe P_k (N x N), position r_j = (y_j, x_j) = top-left corner of the patch,
+ * O_j = O[y_j : y_j+N, x_j : x_j+N], I_j measured intensity (N x N, >= 0, FFT order: DC at
+ * [0,0]).  F = unnormalised forward 2-D DFT, F^-1 carries 1/N^2 (reading R1).  All complex
+ * arrays are interleaved complex64 (re, im), row-major.
+ *
+ * Pointers: every data pointer may be HOST or DEVICE memory (detected with
+ * cudaPointerGetAttributes) unless stated.  `workspace` must be DEVICE memory.
+ * Threading: one context is used from one host thread at a time.
+ * Errors: every call returns a status; nothing is thrown across the ABI; a call that returns
+ * an error leaves the context unchanged (except PTYCHO_ECUDA, after which the context should
+ * be destroyed).  ptycho_last_error() gives a message for the last failing call.
+ */
+#ifndef PTYCHO_B200_H
+#define PTYCHO_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ptycho_ctx ptycho_ctx; /* opaque; owned by the library */
+
+typedef enum {
+    PTYCHO_OK = 0,
+    PTYCHO_EINVAL = 1,       /* null pointer, N not in {64,128,256,512}, K < 1, J < 1, bad parameter */
+    PTYCHO_EBOUNDS = 2,      /* a position with y<0, x<0, y+N>H or x+N>W (no wrap, no clamp; R10)     */
+    PTYCHO_EUNSUPPORTED = 3, /* K > PTYCHO_MAX_MODES                                                  */
+    PTYCHO_ENOMEM = 4,       /* workspace smaller than ptycho_workspace_bytes()                       */
+    PTYCHO_ECUDA = 5,        /* a CUDA runtime error; message in ptycho_last_error()                  */
+    PTYCHO_ESTATE = 6        /* call not valid in the current state (e.g. exit waves before any DM)   */
+} ptycho_status;
+
+/* The three algorithms the paper's back end offers, in their data-parallel
+ * forms: */
+typedef enum {
+    PTYCHO_EPIE_MB = 0, /* ePIE, minibatch form (reading R8)                             */
+    PTYCHO_DM = 1,      /* difference map, all positions at once (reading R4) */
+    PTYCHO_LSQML = 2    /* LSQML-style minibatch with one joint step per batch (R9)       */
+} ptycho_alg;
+
+typedef enum {
+    PTYCHO_I_F32 = 0, /* float32 counts; a negative value marks a masked pixel (R3)   */
+    PTYCHO_I_U16 = 1  /* uint16 counts; 65535 marks a masked / saturated pixel (R3, R11) */
+} ptycho_itype;
+
+#define PTYCHO_MAX_MODES 8
+
+/* Parameters; fill with ptycho_default_params() then override. */
+typedef struct {
+    int batch_size;     /* EPIE_MB / LSQML: frames per minibatch; 0 = all J (full batch)           */
+    int probe_start;    /* first iteration (0-based, global counter) that updates the probe
+                           ("after which iteration to update the probe")              */
+    float delta_blend;  /* DM: blend regulariser delta of (n + eps x_old)/(d + eps)  (R5), 1e-2    */
+    float delta_obj;    /* minibatch: dO = n_O/(d_O + delta_obj  * max_r sum_k|P_k|^2) (R8), 1.0   */
+    float delta_probe;  /* minibatch: dP = n_P/(d_P + delta_probe* max_r d_P)          (R8), 1.0   */
+    float alpha_obj;    /* EPIE_MB step on dO, 1.0                                                 */
+    float alpha_probe;  /* EPIE_MB step on dP, 1.0                                                 */
+    float lsq_lambda;   /* LSQML Tikhonov factor on the 2x2 diagonal (R9), 0.1                     */
+    float pbound;       /* relaxed modulus projection: per-frame power bound, mean squared
+                           amplitude error per pixel in counts; 0 = exact projection (R6)          */
+    int disable_dm;     /* 1 = do not reserve the DM exit-wave store (J*K*N*N complex64) in the
+                           workspace; ptycho_iterate(PTYCHO_DM) then returns PTYCHO_ESTATE          */
+    int deterministic;  /* 1 = fixed-order gather accumulation of the overlap sums: results are
+                           bit-reproducible run to run; 0 = tiled atomics                          */
+    const int32_t *batch_order; /* HOST pointer or NULL.  NULL: strided batches, n_b = ceil(J/B),
+                           batch b = { j : j mod n_b = b } (R8).  Else a permutation of 0..J-1;
+                           batch b = its entries [b*B, (b+1)*B).  Copied at init.                  */
+} ptycho_params;
+
+void ptycho_default_params(ptycho_params *p);
+
+/* Bytes of device workspace ptycho_init needs for these sizes (0 on invalid sizes).  It holds
+ * O, P, the DM exit-wave store (J*K*N*N complex64), the overlap canvases, the transform scratch,
+ * the sort tables and, if the intensities are passed from host memory, a copy of them
+ * (`intensities_on_host` != 0). */
+size_t ptycho_workspace_bytes(int obj_h, int obj_w, int n, int n_modes, int n_pos,
+                              ptycho_itype itype, int intensities_on_host,
+                              const ptycho_params *params /* NULL = defaults */);
+
+/* Create a context.  object: obj_h*obj_w complex64; probe: n_modes*n*n complex64; pos_yx:
+ * n_pos*(y,x) int32 top-left corners; intensities: n_pos*n*n of `itype` in FFT order.
+ * object, probe and positions are COPIED.  intensities are BORROWED when the pointer is device
+ * memory (it must outlive the context) and copied into the workspace when it is host memory.
+ * workspace: device memory of at least ptycho_workspace_bytes(), 256-byte aligned, owned by the
+ * caller, must outlive the context.  cuda_stream: a cudaStream_t (NULL = default stream); all
+ * work of this context is issued on it.  Fixes the DM blend constants from the initial state:
+ * eps_O = delta max_r sum_k|P_k|^2, eps_P = delta J max|O|^2 (R5).  Synchronises the stream. */
+ptycho_status ptycho_init(ptycho_ctx **out, const float *object, int obj_h, int obj_w,
+                          const float *probe, int n_modes, int n, const int32_t *pos_yx, int n_pos,
+                          const void *intensities, ptycho_itype itype, const ptycho_params *params,
+                          void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Run n_iters iterations of `alg` (one iteration = one pass over all J positions, R20).
+ * Asynchronous: kernels are queued on the context's stream and the call returns.  The iteration
+ * counter is global across calls (probe_start and the error history continue).  DM keeps the
+ * exit waves psi_j; if they are not valid (first DM call, or a minibatch algorithm ran since)
+ * they are first set to psi_j = P O_j (R4).  Per frame the cycle is: exit wave psi_O = P O_j
+ * (DM: reflector 2 psi_O - psi_j), forward FFT, error term and modulus projection onto sqrt(I_j)
+ * (relaxed when pbound > 0), inverse FFT, exit-wave update, overlap scatter-add of object and
+ * probe sums, then the normalising update. */
+ptycho_status ptycho_iterate(ptycho_ctx *ctx, ptycho_alg alg, int n_iters);
+
+/* Copy the current state out (synchronises the stream).  out: host or device. */
+ptycho_status ptycho_fetch_object(ptycho_ctx *ctx, float *out /* obj_h*obj_w*2 */);
+ptycho_status ptycho_fetch_probe(ptycho_ctx *ctx, float *out /* n_modes*n*n*2 */);
+/* Error history E_t = sum_j sum_q (sqrt I_j - A_j)^2 / sum_j sum_q I_j over unmasked pixels, A_j
+ * the amplitude of the wave transformed in iteration t (R7, C3).  out: HOST, up to cap values;
+ * *n_written = number of iterations run so far (may exceed cap). */
+ptycho_status ptycho_fetch_error(ptycho_ctx *ctx, double *out, int cap, int *n_written);
+/* Exit waves of `count` frames idx[0..count) (caller's frame numbering; idx is a HOST pointer).
+ * After DM: the stored psi_j.  Otherwise PTYCHO_ESTATE.  out: count*n_modes*n*n*2 floats. */
+ptycho_status ptycho_fetch_exit_waves(ptycho_ctx *ctx, const int32_t *idx, int count, float *out);
+/* Revised waves psi_F = F^-1[Pi_M F[P O_j]] of the CURRENT object and probe for frames idx
+ * (one forward/projection/inverse pass, no state change); used for teacher-forced parity of the
+ * minibatch algorithms. */
+ptycho_status ptycho_revised_waves(ptycho_ctx *ctx, const int32_t *idx, int count, float *out);
+/* LSQML: the (a, b) steps applied so far, in batch order; out: HOST, up to cap pairs. */
+ptycho_status ptycho_fetch_steps(ptycho_ctx *ctx, double *out_ab, int cap, int *n_written);
+
+/* Overwrite state (teacher forcing, checkpoint restore).  Source: host or device. */
+ptycho_status ptycho_set_object(ptycho_ctx *ctx, const float *object);
+ptycho_status ptycho_set_probe(ptycho_ctx *ctx, const float *probe);
+ptycho_status ptycho_set_exit_waves(ptycho_ctx *ctx, const float *psi /* n_pos*n_modes*n*n*2 */);
+
+/* Data-fit error of the current O, P: the E above evaluated for F[P O_j] (one FFT pass, no
+ * state change; R7).  Synchronises. */
+ptycho_status ptycho_eval_error(ptycho_ctx *ctx, double *out);
+
+/* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
+long long ptycho_launch_count(const ptycho_ctx *ctx);
+
+const char *ptycho_last_error(const ptycho_ctx *ctx); /* never NULL; "" if none */
+void ptycho_destroy(ptycho_ctx *ctx);                 /* frees host state; the workspace is the caller's */
+
+/* Unit-test entry points of single kernels (tier T2).  Device pointers. */
+/* Batched 2-D complex64 FFT of `count` n x n frames, in place, on `cuda_stream`. */
+ptycho_status ptycho_test_fft2(float *data, int n, int count, int inverse, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PTYCHO_B200_H */

@@ -1,0 +1,531 @@
+// kernels.cuh -- the projection-cycle kernels for sm_100a.
+//
+// Pipeline per chunk of frames ("three-pass, L2-resident"):
+//   k_rows_fwd : a1 exit wave (+ a2 DM reflector, + DM lagged probe sums) fused into the load of
+//                the row FFTs (a3, x direction); writes the half-transformed frame to scratch S.
+//   k_cols     : column FFTs (a3, y direction), a4 per-frame error partials, a5 modulus
+//                projection (exact scale; the relaxed blend is applied in k_rows_inv, which is
+//                equivalent by linearity of F^-1), inverse column FFTs (a6), back to S.
+//   k_rows_inv : inverse row FFTs (a6) fused with a7 exit-wave update and a8/a9 overlap
+//                scatter-adds (vector red.global.add) of the object and probe sums.
+// S is sized so that a chunk stays resident in the 126 MB L2; HBM sees psi in/out and I only.
+#pragma once
+#include <cstdint>
+#include "fft_core.cuh"
+
+namespace ptycho {
+
+struct YX { int y, x; };
+
+enum RowFwdMode { RF_EXIT = 0, RF_DM = 1, RF_PLAIN = 2 };
+enum ColMode { CM_FULL = 0, CM_ERRONLY = 1, CM_PLAIN_FWD = 2, CM_PLAIN_INV = 3 };
+enum RowInvMode { RI_MINIBATCH = 0, RI_DM = 1, RI_REVISED = 2, RI_PLAIN = 3 };
+
+constexpr int kThreads = 256;
+
+struct FrameArgs {
+    const float2* __restrict__ O;   // object H x W
+    int W;
+    const float2* __restrict__ P;   // K x N x N
+    int K;
+    float2* psi;                    // DM: exit-wave store of this launch's first slot (slot-major)
+    const YX* __restrict__ pos;     // J positions, caller numbering
+    const int* __restrict__ frames; // caller frame id of each slot of this launch
+    float2* S;                      // scratch: nframes x K x N x N
+    const void* __restrict__ I;     // intensities, caller numbering
+    int itype;                      // 0 f32, 1 u16
+    float* e_part;                  // per slot: NCB error partials (this launch's first slot)
+    float2* nO; float* dO;          // object canvases H x W
+    float2* nP; float* dP;          // probe canvases K x N x N, N x N
+    float pbound;
+    float2* out;                    // RI_REVISED: nframes x K x N x N
+    const float2* __restrict__ tw;  // twiddles [ka*T + b]
+    const float2* __restrict__ twi; // twiddles [b*E + ka]
+};
+
+template <int N> struct Geo {
+    static constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T;
+    static constexpr int LPB = kThreads / T;                     // lines per CTA
+    static constexpr int LS_ROW = LineSmem<N>::SIZE + ((T == 8 && (LineSmem<N>::SIZE % 16) != 8) ? 8 : 0);
+    static constexpr int LS_COL = LineSmem<N>::SIZE | 1;         // odd: lanes run along lines
+    static constexpr int NCB = N / LPB;                          // column blocks (= row blocks) per frame
+    static constexpr size_t smem_rows = (size_t)(LPB * LS_ROW + 2 * N) * sizeof(float2);
+    static size_t smem_cols(int K) {
+        return (size_t)(LPB * LS_COL + 2 * N) * sizeof(float2) + (K > 1 ? (size_t)K * E * kThreads * sizeof(float2) : 0) + 64;
+    }
+};
+
+__device__ __forceinline__ void load_tw(float2* s_tw, const float2* tw, const float2* twi, int n) {
+    for (int i = threadIdx.x; i < n; i += kThreads) { s_tw[i] = tw[i]; s_tw[n + i] = twi[i]; }
+}
+
+__device__ __forceinline__ float load_intensity(const void* I, int itype, size_t idx) {
+    if (itype == 1) {
+        const unsigned short v = __ldg(reinterpret_cast<const unsigned short*>(I) + idx);
+        return v == 65535 ? -1.0f : (float)v;
+    }
+    return __ldg(reinterpret_cast<const float*>(I) + idx);
+}
+
+__device__ __forceinline__ void red_add(float2* p, float2 v) { atomicAdd(p, v); }
+__device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
+
+// ------------------------------------------------------------------------------------------
+// a1/a2/a3: exit wave (+ reflector) -> forward row FFTs -> S.   grid (NCB, nframes)
+// ------------------------------------------------------------------------------------------
+template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_fwd(FrameArgs a) {
+    using G = Geo<N>;
+    constexpr int E = G::E, T = G::T;
+    extern __shared__ float2 sm[];
+    float2* s_tw = sm + G::LPB * G::LS_ROW;
+    load_tw(s_tw, a.tw, a.twi, N);
+    const int l = threadIdx.x / T, t = threadIdx.x % T;
+    float2* sx = sm + l * G::LS_ROW;
+    const int slot = blockIdx.y, y = blockIdx.x * G::LPB + l;
+    const size_t fr = (size_t)slot * a.K * N * N;
+    __syncthreads();
+
+    if (MODE == RF_PLAIN) {
+        float2 v[E];
+        float2* row = a.S + fr + (size_t)y * N;
+#pragma unroll
+        for (int i = 0; i < E; ++i) v[i] = row[t + T * i];
+        fft_line_fwd<N>(v, t, sx, s_tw);
+#pragma unroll
+        for (int r = 0; r < E; ++r) row[freq_b<N>(t, r)] = v[r];
+        return;
+    }
+
+    const YX p0 = a.pos[a.frames[slot]];
+    const float2* orow = a.O + (size_t)(p0.y + y) * a.W + p0.x;
+    float2 o[E];
+#pragma unroll
+    for (int i = 0; i < E; ++i) o[i] = __ldg(orow + t + T * i);
+    for (int k = 0; k < a.K; ++k) {
+        const size_t off = ((size_t)k * N + y) * N;
+        float2 v[E];
+#pragma unroll
+        for (int i = 0; i < E; ++i) v[i] = cmul(__ldg(a.P + off + t + T * i), o[i]);   // psi_O = P_k O_j
+        if (MODE == RF_DM) {
+            const float2* prow = a.psi + fr + off;
+#pragma unroll
+            for (int i = 0; i < E; ++i) {
+                const float2 s = prow[t + T * i];
+                red_add(a.nP + off + t + T * i, cmulc(s, o[i]));                        // conj(O_j) psi_j (lagged, R4)
+                v[i] = make_float2(2.f * v[i].x - s.x, 2.f * v[i].y - s.y);             // reflector
+            }
+        }
+        fft_line_fwd<N>(v, t, sx, s_tw);
+        float2* srow = a.S + fr + off;
+#pragma unroll
+        for (int r = 0; r < E; ++r) srow[freq_b<N>(t, r)] = v[r];
+        __syncthreads();
+    }
+    if (MODE == RF_DM) {
+#pragma unroll
+        for (int i = 0; i < E; ++i) red_add(a.dP + (size_t)y * N + t + T * i, o[i].x * o[i].x + o[i].y * o[i].y);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a3 (columns) / a4 / a5 / a6 (columns).   grid (NCB, nframes); CTA = LPB columns x T threads,
+// lanes run along the columns so that every global access is LPB*8 contiguous bytes.
+// ------------------------------------------------------------------------------------------
+template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_cols(FrameArgs a) {
+    using G = Geo<N>;
+    constexpr int E = G::E, T = G::T, CB = G::LPB;
+    extern __shared__ float2 sm[];
+    float2* s_tw = sm + CB * G::LS_COL;
+    float2* stage = s_tw + 2 * N;                         // K > 1: [k][r][tid]
+    __shared__ float s_red[kThreads / 32];
+    load_tw(s_tw, a.tw, a.twi, N);
+    const int c = threadIdx.x % CB, t = threadIdx.x / CB;
+    float2* sx = sm + c * G::LS_COL;
+    const int slot = blockIdx.y, col = blockIdx.x * CB + c;
+    const size_t fr = (size_t)slot * a.K * N * N;
+    __syncthreads();
+
+    if (MODE == CM_PLAIN_FWD || MODE == CM_PLAIN_INV) {
+        float2 v[E];
+        float2* base = a.S + fr + col;
+        if (MODE == CM_PLAIN_FWD) {
+#pragma unroll
+            for (int i = 0; i < E; ++i) v[i] = base[(size_t)(t + T * i) * N];
+            fft_line_fwd<N>(v, t, sx, s_tw);
+#pragma unroll
+            for (int r = 0; r < E; ++r) base[(size_t)freq_b<N>(t, r) * N] = v[r];
+        } else {
+#pragma unroll
+            for (int r = 0; r < E; ++r) v[r] = base[(size_t)freq_b<N>(t, r) * N];
+            fft_line_inv<N>(v, t, sx, s_tw + N);
+#pragma unroll
+            for (int r = 0; r < E; ++r) base[(size_t)pos_a_inv<N>(t, r) * N] = v[r];
+        }
+        return;
+    }
+
+    const size_t ibase = (size_t)a.frames[slot] * N * N + col;
+    float amp2[E];
+#pragma unroll
+    for (int r = 0; r < E; ++r) amp2[r] = 0.f;
+    float2 v[E];
+    for (int k = 0; k < a.K; ++k) {
+        const float2* base = a.S + fr + (size_t)k * N * N + col;
+#pragma unroll
+        for (int i = 0; i < E; ++i) v[i] = base[(size_t)(t + T * i) * N];
+        fft_line_fwd<N>(v, t, sx, s_tw);
+#pragma unroll
+        for (int r = 0; r < E; ++r) amp2[r] += v[r].x * v[r].x + v[r].y * v[r].y;
+        if (a.K > 1) {
+#pragma unroll
+            for (int r = 0; r < E; ++r) stage[((size_t)k * E + r) * kThreads + threadIdx.x] = v[r];
+        }
+        __syncthreads();
+    }
+    // a4 error term and a5 scale.  scale[r] carries the 1/N^2 of F^-1.
+    constexpr float inv_n2 = 1.0f / ((float)N * (float)N);
+    float err = 0.f;
+    float scale[E];
+    bool zero_amp = false;
+#pragma unroll
+    for (int r = 0; r < E; ++r) {
+        const float in = load_intensity(a.I, a.itype, ibase + (size_t)freq_b<N>(t, r) * N);
+        const float amp = sqrtf(amp2[r]);
+        if (in >= 0.f) {
+            const float sq = sqrtf(in), d = sq - amp;
+            err = fmaf(d, d, err);
+            if (amp > 0.f) scale[r] = sq / amp * inv_n2;
+            else { scale[r] = -sq * inv_n2; zero_amp = true; }   // R2: flagged by the sign
+        } else scale[r] = inv_n2;                                 // R3: masked, keep Phi
+    }
+    // block reduction of the error partial (fixed order: deterministic)
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) err += __shfl_xor_sync(0xffffffffu, err, s);
+    if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = err;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float tot = 0.f;
+        for (int w = 0; w < kThreads / 32; ++w) tot += s_red[w];
+        a.e_part[(size_t)slot * G::NCB + blockIdx.x] = tot;
+    }
+    if (MODE == CM_ERRONLY) return;
+
+    for (int k = 0; k < a.K; ++k) {
+        if (a.K > 1) {
+#pragma unroll
+            for (int r = 0; r < E; ++r) v[r] = stage[((size_t)k * E + r) * kThreads + threadIdx.x];
+        }
+#pragma unroll
+        for (int r = 0; r < E; ++r) {
+            if (zero_amp && scale[r] < 0.f) v[r] = make_float2(k == 0 ? -scale[r] : 0.f, 0.f);
+            else { v[r].x *= scale[r]; v[r].y *= scale[r]; }
+        }
+        fft_line_inv<N>(v, t, sx, s_tw + N);
+        float2* base = a.S + fr + (size_t)k * N * N + col;
+#pragma unroll
+        for (int r = 0; r < E; ++r) base[(size_t)pos_a_inv<N>(t, r) * N] = v[r];
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a6 (rows) / a7 / a8 / a9: inverse row FFTs -> revised wave -> exit-wave update -> scatter-add.
+// grid (NCB, nframes)
+// ------------------------------------------------------------------------------------------
+template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_inv(FrameArgs a) {
+    using G = Geo<N>;
+    constexpr int E = G::E, T = G::T;
+    extern __shared__ float2 sm[];
+    float2* s_tw = sm + G::LPB * G::LS_ROW;
+    load_tw(s_tw, a.tw, a.twi, N);
+    const int l = threadIdx.x / T, t = threadIdx.x % T;
+    float2* sx = sm + l * G::LS_ROW;
+    const int slot = blockIdx.y, y = blockIdx.x * G::LPB + l;
+    const size_t fr = (size_t)slot * a.K * N * N;
+    __syncthreads();
+
+    if (MODE == RI_PLAIN) {
+        float2 v[E];
+        float2* row = a.S + fr + (size_t)y * N;
+#pragma unroll
+        for (int r = 0; r < E; ++r) v[r] = row[freq_b<N>(t, r)];
+        fft_line_inv<N>(v, t, sx, s_tw + N);
+#pragma unroll
+        for (int r = 0; r < E; ++r) row[pos_a_inv<N>(t, r)] = v[r];
+        return;
+    }
+
+    // R6 relaxed projection: blend weight of this frame from its error partials (fixed order)
+    float rb = 0.f;
+    if (a.pbound > 0.f) {
+        float e = 0.f;
+        for (int i = 0; i < G::NCB; ++i) e += a.e_part[(size_t)slot * G::NCB + i];
+        e *= 1.0f / ((float)N * (float)N);
+        rb = (e <= a.pbound) ? 1.0f : sqrtf(a.pbound / e);
+    }
+    const YX p0 = a.pos[a.frames[slot]];
+    const size_t obase = (size_t)(p0.y + y) * a.W + p0.x;
+    float2 o[E];
+#pragma unroll
+    for (int r = 0; r < E; ++r) o[r] = __ldg(a.O + obase + pos_a_inv<N>(t, r));
+    float2 accO[E];
+    float accD[E];
+#pragma unroll
+    for (int r = 0; r < E; ++r) { accO[r] = make_float2(0.f, 0.f); accD[r] = 0.f; }
+
+    for (int k = 0; k < a.K; ++k) {
+        const size_t off = ((size_t)k * N + y) * N;
+        float2 v[E];
+        const float2* srow = a.S + fr + off;
+#pragma unroll
+        for (int r = 0; r < E; ++r) v[r] = srow[freq_b<N>(t, r)];
+        fft_line_inv<N>(v, t, sx, s_tw + N);            // v = F^-1[exact projection]
+#pragma unroll
+        for (int r = 0; r < E; ++r) {
+            const int x = pos_a_inv<N>(t, r);
+            const float2 p = __ldg(a.P + off + x);
+            const float2 po = cmul(p, o[r]);            // psi_O
+            float2 w;
+            if (MODE == RI_DM) {
+                float2* ps = a.psi + fr + off + x;
+                const float2 s = *ps;
+                const float2 phi = make_float2(2.f * po.x - s.x, 2.f * po.y - s.y);
+                const float2 pf = make_float2(fmaf(rb, phi.x - v[r].x, v[r].x), fmaf(rb, phi.y - v[r].y, v[r].y));
+                w = make_float2(s.x + pf.x - po.x, s.y + pf.y - po.y);     // a7, beta = 1
+                *ps = w;
+            } else {
+                const float2 pf = make_float2(fmaf(rb, po.x - v[r].x, v[r].x), fmaf(rb, po.y - v[r].y, v[r].y));
+                if (MODE == RI_REVISED) { a.out[fr + off + x] = pf; continue; }
+                w = make_float2(pf.x - po.x, pf.y - po.y);                 // chi
+                red_add(a.nP + off + x, cmulc(w, o[r]));                   // a9 conj(O_j) chi
+            }
+            accO[r] = cadd(accO[r], cmulc(w, p));                          // a8 conj(P_k) w
+            accD[r] = fmaf(p.x, p.x, fmaf(p.y, p.y, accD[r]));
+        }
+        __syncthreads();
+    }
+    if (MODE == RI_REVISED) return;
+#pragma unroll
+    for (int r = 0; r < E; ++r) {
+        const int x = pos_a_inv<N>(t, r);
+        red_add(a.nO + obase + x, accO[r]);
+        red_add(a.dO + obase + x, accD[r]);
+        if (MODE == RI_MINIBATCH) red_add(a.dP + (size_t)y * N + x, o[r].x * o[r].x + o[r].y * o[r].y);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// small element-wise / reduction kernels (a10, a11)
+// ------------------------------------------------------------------------------------------
+// psi_j = P O_j for every slot (R4 initial exit waves).  grid (N*N*K / 256, nslots)
+__global__ void k_init_psi(float2* psi, const float2* __restrict__ O, int W, const float2* __restrict__ P, int K,
+                           int n, const YX* __restrict__ pos, const int* __restrict__ frames) {
+    const int slot = blockIdx.y;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;   // over K*n*n
+    const size_t nn = (size_t)n * n;
+    if (i >= nn * K) return;
+    const size_t q = i % nn;
+    const int y = (int)(q / n), x = (int)(q % n);
+    const YX p0 = pos[frames[slot]];
+    psi[(size_t)slot * K * nn + i] = cmul(P[i], O[(size_t)(p0.y + y) * W + p0.x + x]);
+}
+
+// gather stored exit waves of listed slots into out (fetch) or scatter from in (set)
+__global__ void k_copy_frames(float2* dst, const float2* src, const int* __restrict__ dst_idx,
+                              const int* __restrict__ src_idx, size_t per_frame) {
+    const size_t d = dst_idx ? (size_t)dst_idx[blockIdx.y] : blockIdx.y;
+    const size_t s = src_idx ? (size_t)src_idx[blockIdx.y] : blockIdx.y;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < per_frame; i += (size_t)gridDim.x * blockDim.x)
+        dst[d * per_frame + i] = src[s * per_frame + i];
+}
+
+struct Scalars {            // device-resident scalars (no host round trip inside iterate)
+    float max_p2;           // max_r sum_k |P_k|^2 of the current probe
+    float max_dp;           // max_r d_P of the current batch
+    float step_a, step_b;   // steps applied by the apply kernels
+    double sum_I;           // sum of unmasked intensities
+    float eps_O, eps_P;     // DM blend constants (fixed at init)
+    unsigned int max_bits;  // scratch for atomicMax on non-negative floats
+};
+
+// max over r of sum_k |P_k(r)|^2 -> sc->max_p2.  single CTA of 1024 threads.
+__global__ void k_probe_max(const float2* __restrict__ P, int K, int nn, Scalars* sc) {
+    __shared__ float s[32];
+    float m = 0.f;
+    for (int q = threadIdx.x; q < nn; q += blockDim.x) {
+        float v = 0.f;
+        for (int k = 0; k < K; ++k) { const float2 p = P[(size_t)k * nn + q]; v += p.x * p.x + p.y * p.y; }
+        m = fmaxf(m, v);
+    }
+    for (int d = 16; d > 0; d >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, d));
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) { for (int w = 1; w < (int)blockDim.x / 32; ++w) m = fmaxf(m, s[w]); sc->max_p2 = m; }
+}
+// max over r of d_P(r) -> sc->max_dp.  single CTA.
+__global__ void k_real_max(const float* __restrict__ d, int nn, Scalars* sc) {
+    __shared__ float s[32];
+    float m = 0.f;
+    for (int q = threadIdx.x; q < nn; q += blockDim.x) m = fmaxf(m, d[q]);
+    for (int dd = 16; dd > 0; dd >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, dd));
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) { for (int w = 1; w < (int)blockDim.x / 32; ++w) m = fmaxf(m, s[w]); sc->max_dp = m; }
+}
+// max |O|^2 at init (for eps_P); uses atomicMax on the bit pattern of non-negative floats.
+__global__ void k_abs2_max(const float2* __restrict__ a, size_t n, Scalars* sc) {
+    float m = 0.f;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        m = fmaxf(m, a[i].x * a[i].x + a[i].y * a[i].y);
+    for (int d = 16; d > 0; d >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, d));
+    if ((threadIdx.x & 31) == 0) atomicMax(&sc->max_bits, __float_as_uint(m));
+}
+
+// a10 DM: x <- (n + eps x)/(d + eps); zero the canvases.  which = 0 object (eps_O), 1 probe (eps_P);
+// d is shared by the `modes` planes of n.
+__global__ void k_dm_blend(float2* x, float2* n, float* d, size_t plane, int modes, const Scalars* sc, int which,
+                           int update) {
+    const float eps = which ? sc->eps_P : sc->eps_O;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < plane; i += (size_t)gridDim.x * blockDim.x) {
+        const float inv = 1.0f / (d[i] + eps);
+        for (int k = 0; k < modes; ++k) {
+            const size_t q = (size_t)k * plane + i;
+            if (update) { const float2 xv = x[q], nv = n[q]; x[q] = make_float2((nv.x + eps * xv.x) * inv, (nv.y + eps * xv.y) * inv); }
+            n[q] = make_float2(0.f, 0.f);
+        }
+        d[i] = 0.f;
+    }
+}
+
+// minibatch directions: n <- n / (d + delta * max)  (in place), optional LSQML partial sums
+//   part[2*block + 0] += sum |dir|^2 d     (A11 or A22)
+//   part[2*block + 1] += sum Re conj(dir) n_before   (b1 or b2)
+// which = 0: object (max = max_p2), 1: probe (max = max_dp).
+__global__ void k_direction(float2* n, const float* __restrict__ d, size_t plane, int modes, float delta,
+                            const Scalars* sc, int which, double* part) {
+    const float reg = delta * (which ? sc->max_dp : sc->max_p2);
+    double a = 0.0, b = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < plane; i += (size_t)gridDim.x * blockDim.x) {
+        const float dv = d[i], inv = 1.0f / (dv + reg);
+        for (int k = 0; k < modes; ++k) {
+            const size_t q = (size_t)k * plane + i;
+            const float2 nv = n[q];
+            const float2 dir = make_float2(nv.x * inv, nv.y * inv);
+            n[q] = dir;
+            if (part) {
+                a += (double)((dir.x * dir.x + dir.y * dir.y) * dv);
+                b += (double)(dir.x * nv.x + dir.y * nv.y);
+            }
+        }
+    }
+    if (part) {
+        __shared__ double sa[32], sb[32];
+        for (int s = 16; s > 0; s >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, s); b += __shfl_xor_sync(0xffffffffu, b, s); }
+        if ((threadIdx.x & 31) == 0) { sa[threadIdx.x >> 5] = a; sb[threadIdx.x >> 5] = b; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < (int)blockDim.x / 32; ++w) { a += sa[w]; b += sb[w]; }
+            part[2 * blockIdx.x] = a; part[2 * blockIdx.x + 1] = b;
+        }
+    }
+}
+
+// LSQML cross term A12 = Re sum_j sum_r T(r) conj(dO[r_j+r]) O[r_j+r],  T = sum_k conj(P_k) dP_k.
+// grid (nframes); part[block] = this frame's sum.
+__global__ void k_lsq_cross(const float2* __restrict__ O, const float2* __restrict__ dO, int W,
+                            const float2* __restrict__ P, const float2* __restrict__ dPk, int K, int n,
+                            const YX* __restrict__ pos, const int* __restrict__ frames, double* part) {
+    const YX p0 = pos[frames[blockIdx.x]];
+    const int nn = n * n;
+    double acc = 0.0;
+    for (int q = threadIdx.x; q < nn; q += blockDim.x) {
+        const int y = q / n, x = q % n;
+        float2 tq = make_float2(0.f, 0.f);
+        for (int k = 0; k < K; ++k) tq = cadd(tq, cmulc(dPk[(size_t)k * nn + q], P[(size_t)k * nn + q]));
+        const size_t o = (size_t)(p0.y + y) * W + p0.x + x;
+        const float2 s = cmulc(O[o], dO[o]);           // conj(dO) O
+        acc += (double)(tq.x * s.x - tq.y * s.y);
+    }
+    __shared__ double sa[32];
+    for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
+    if ((threadIdx.x & 31) == 0) sa[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) { for (int w = 1; w < (int)blockDim.x / 32; ++w) acc += sa[w]; part[blockIdx.x] = acc; }
+}
+
+// a11: sum the partials in fixed order, solve the 2x2 system (R9), publish the steps.
+__global__ void k_lsq_solve(const double* partO, int nO, const double* partP, int nP, const double* partX, int nX,
+                            float lambda, int update_probe, Scalars* sc, double* steps_out) {
+    if (threadIdx.x || blockIdx.x) return;
+    double A11 = 0, b1 = 0, A22 = 0, b2 = 0, A12 = 0;
+    for (int i = 0; i < nO; ++i) { A11 += partO[2 * i]; b1 += partO[2 * i + 1]; }
+    for (int i = 0; i < nP; ++i) { A22 += partP[2 * i]; b2 += partP[2 * i + 1]; }
+    for (int i = 0; i < nX; ++i) A12 += partX[i];
+    const double l = 1.0 + (double)lambda;
+    double a, b;
+    if (!update_probe) { a = (A11 > 0) ? b1 / (A11 * l) : 0.0; b = 0.0; }
+    else {
+        const double det = A11 * l * A22 * l - A12 * A12;
+        if (!(det > 0) || !isfinite(det)) { a = 0; b = 0; }
+        else { a = (b1 * A22 * l - A12 * b2) / det; b = (A11 * l * b2 - A12 * b1) / det; }
+    }
+    sc->step_a = (float)a; sc->step_b = (float)b;
+    steps_out[0] = a; steps_out[1] = b;
+}
+__global__ void k_set_steps(Scalars* sc, float a, float b, double* steps_out) {
+    sc->step_a = a; sc->step_b = b;
+    if (steps_out) { steps_out[0] = a; steps_out[1] = b; }
+}
+
+// x += step * dir; zero dir and d.  which = 0: step_a, 1: step_b.
+__global__ void k_apply(float2* x, float2* dir, float* d, size_t plane, int modes, const Scalars* sc, int which,
+                        int update) {
+    const float st = which ? sc->step_b : sc->step_a;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < plane; i += (size_t)gridDim.x * blockDim.x) {
+        for (int k = 0; k < modes; ++k) {
+            const size_t q = (size_t)k * plane + i;
+            if (update) { const float2 dv = dir[q]; float2 xv = x[q]; xv.x = fmaf(st, dv.x, xv.x); xv.y = fmaf(st, dv.y, xv.y); x[q] = xv; }
+            dir[q] = make_float2(0.f, 0.f);
+        }
+        d[i] = 0.f;
+    }
+}
+
+// sum of unmasked intensities in double (init).  part[block]; then k_finish_sum.
+__global__ void k_sum_intensity(const void* __restrict__ I, int itype, size_t count, double* part) {
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (size_t)gridDim.x * blockDim.x) {
+        const float v = load_intensity(I, itype, i);
+        if (v >= 0.f) acc += (double)v;
+    }
+    __shared__ double sa[32];
+    for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
+    if ((threadIdx.x & 31) == 0) sa[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) { for (int w = 1; w < (int)blockDim.x / 32; ++w) acc += sa[w]; part[blockIdx.x] = acc; }
+}
+__global__ void k_finish_sum_I(const double* part, int n, Scalars* sc) {
+    if (threadIdx.x || blockIdx.x) return;
+    double s = 0; for (int i = 0; i < n; ++i) s += part[i];
+    sc->sum_I = s;
+}
+// E_t = (sum of all error partials, fixed order, double) / sum_I.  single CTA of 1024 threads.
+__global__ void k_sum_error(const float* __restrict__ e_part, size_t count, const Scalars* sc, double* out) {
+    __shared__ double sa[32];
+    double acc = 0.0;
+    for (size_t i = threadIdx.x; i < count; i += blockDim.x) acc += (double)e_part[i];
+    for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
+    if ((threadIdx.x & 31) == 0) sa[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)blockDim.x / 32; ++w) acc += sa[w];
+        *out = acc / (sc->sum_I > 0 ? sc->sum_I : 1.0);
+    }
+}
+__global__ void k_finish_init(Scalars* sc, float delta, int J, int which) {
+    if (threadIdx.x || blockIdx.x) return;
+    if (which == 0) sc->eps_O = delta * sc->max_p2;
+    else { sc->eps_P = delta * (float)J * __uint_as_float(sc->max_bits); }
+}
+
+}  // namespace ptycho

@@ -1,0 +1,610 @@
+// ptycho_api.cu -- host side of the C ABI declared in include/ptycho_b200.h.
+//
+// Holds no arithmetic of the method except the sequencing of iterations, chunks and minibatches
+// (readings R4, R8, R20); every step of the cycle runs in the kernels of
+// kernels.cuh.  There is no CPU fallback: without a CUDA device every call fails with
+// PTYCHO_ECUDA.
+#include "../../include/ptycho_b200.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <numeric>
+#include <string>
+#include <vector>
+
+#include "kernels.cuh"
+
+using namespace ptycho;
+
+namespace {
+
+constexpr int kErrCap = 1 << 16;    // iterations of error history kept
+constexpr int kStepCap = 1 << 18;   // (a, b) pairs kept
+constexpr int kRedBlocks = 1024;    // blocks of the canvas reductions / element-wise kernels
+
+struct Carver {                     // bump allocator over the caller's workspace (256-byte aligned)
+    char* base;
+    size_t off = 0;
+    explicit Carver(void* b) : base(static_cast<char*>(b)) {}
+    template <class T> T* take(size_t count) {
+        off = (off + 255) & ~size_t(255);
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += count * sizeof(T);
+        return p;
+    }
+};
+
+}  // namespace
+
+struct ptycho_ctx {
+    int H = 0, W = 0, N = 0, K = 0, J = 0, itype = 0;
+    ptycho_params par{};
+    cudaStream_t stream = nullptr;
+    // device state (inside the workspace)
+    float2 *O = nullptr, *P = nullptr, *psi = nullptr, *S = nullptr, *nO = nullptr, *nP = nullptr;
+    float *dO = nullptr, *dP = nullptr, *e_part = nullptr, *e_tmp = nullptr;
+    float2 *tw = nullptr, *twi = nullptr;
+    YX* pos = nullptr;
+    int *dm_frames = nullptr, *mb_frames = nullptr, *tmp_idx = nullptr, *slot_of = nullptr;
+    Scalars* sc = nullptr;
+    double *err_hist = nullptr, *steps = nullptr, *partO = nullptr, *partP = nullptr, *partX = nullptr, *scratch_d = nullptr;
+    const void* I = nullptr;
+    // host state
+    int chunk = 1;
+    std::vector<int> dm_order;                 // slot -> caller frame
+    std::vector<int> slot_of_h;                // caller frame -> slot
+    std::vector<int> mb_offsets;               // batch b = mb_frames[mb_offsets[b] .. mb_offsets[b+1])
+    int t = 0;                                 // global iteration counter
+    long long n_steps = 0;
+    bool psi_valid = false;
+    long long launches = 0;
+    std::string err;
+};
+
+namespace {
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            if (c) c->err = std::string(#call) + ": " + cudaGetErrorString(e_);                    \
+            return PTYCHO_ECUDA;                                                                   \
+        }                                                                                          \
+    } while (0)
+
+ptycho_status fail(ptycho_ctx* c, ptycho_status s, const char* msg) {
+    if (c) c->err = msg;
+    return s;
+}
+
+bool valid_n(int n) { return n == 64 || n == 128 || n == 256 || n == 512; }
+
+int chunk_frames(int n, int K, int J) {
+    double mb = 32.0;
+    if (const char* e = getenv("PTYCHO_CHUNK_MB")) mb = atof(e) > 0 ? atof(e) : mb;
+    long long per = (long long)K * n * n * 8;
+    long long c = (long long)(mb * 1048576.0) / per;
+    return (int)std::max<long long>(1, std::min<long long>(c, J));
+}
+
+size_t cols_smem(int n, int K) {
+    switch (n) {
+        case 64: return Geo<64>::smem_cols(K);
+        case 128: return Geo<128>::smem_cols(K);
+        case 256: return Geo<256>::smem_cols(K);
+        default: return Geo<512>::smem_cols(K);
+    }
+}
+int ncb_of(int n) { return n == 64 ? Geo<64>::NCB : n == 128 ? Geo<128>::NCB : n == 256 ? Geo<256>::NCB : Geo<512>::NCB; }
+
+// Lays the workspace out; with base == nullptr only measures it.
+size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
+    Carver w(base);
+    const size_t HW = (size_t)c->H * c->W, nn = (size_t)c->N * c->N, knn = nn * c->K;
+    c->O = w.take<float2>(HW);
+    c->P = w.take<float2>(knn);
+    c->nO = w.take<float2>(HW);
+    c->dO = w.take<float>(HW);
+    c->nP = w.take<float2>(knn);
+    c->dP = w.take<float>(nn);
+    c->S = w.take<float2>((size_t)c->chunk * knn);
+    c->e_part = w.take<float>((size_t)c->J * ncb_of(c->N));
+    c->e_tmp = w.take<float>((size_t)c->J * ncb_of(c->N));
+    c->tw = w.take<float2>(c->N);
+    c->twi = w.take<float2>(c->N);
+    c->pos = w.take<YX>(c->J);
+    c->dm_frames = w.take<int>(c->J);
+    c->mb_frames = w.take<int>(c->J);
+    c->tmp_idx = w.take<int>(c->J);
+    c->slot_of = w.take<int>(c->J);
+    c->sc = w.take<Scalars>(1);
+    c->err_hist = w.take<double>(kErrCap);
+    c->steps = w.take<double>(2 * (size_t)kStepCap);
+    c->partO = w.take<double>(2 * kRedBlocks);
+    c->partP = w.take<double>(2 * kRedBlocks);
+    c->partX = w.take<double>(c->J);
+    c->scratch_d = w.take<double>(kRedBlocks);
+    if (!c->par.disable_dm) c->psi = w.take<float2>((size_t)c->J * knn);
+    if (copy_I) c->I = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
+    return (w.off + 255) & ~size_t(255);
+}
+
+bool is_device_ptr(const void* p) {
+    cudaPointerAttributes at{};
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+template <int N> ptycho_status set_attrs(ptycho_ctx* c) {
+    const int rows = (int)Geo<N>::smem_rows, cols = (int)Geo<N>::smem_cols(c->K);
+    if (cols > 227 * 1024) return fail(c, PTYCHO_EUNSUPPORTED, "too many probe modes for this frame size (column-pass staging exceeds shared memory)");
+    CU(cudaFuncSetAttribute(k_rows_fwd<N, RF_EXIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_rows_fwd<N, RF_DM>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_rows_fwd<N, RF_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_rows_inv<N, RI_MINIBATCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_rows_inv<N, RI_DM>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_rows_inv<N, RI_REVISED>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_rows_inv<N, RI_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_cols<N, CM_FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
+    CU(cudaFuncSetAttribute(k_cols<N, CM_ERRONLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
+    CU(cudaFuncSetAttribute(k_cols<N, CM_PLAIN_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
+    CU(cudaFuncSetAttribute(k_cols<N, CM_PLAIN_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
+    return PTYCHO_OK;
+}
+
+void host_twiddles(int n, int E, int T, std::vector<float2>& tw, std::vector<float2>& twi) {
+    tw.resize(n); twi.resize(n);
+    for (int ka = 0; ka < E; ++ka)
+        for (int b = 0; b < T; ++b) {
+            const double ang = -2.0 * M_PI * (double)b * ka / n;
+            const float2 w = make_float2((float)cos(ang), (float)sin(ang));
+            tw[ka * T + b] = w;
+            twi[b * E + ka] = w;
+        }
+}
+
+FrameArgs base_args(const ptycho_ctx* c) {
+    FrameArgs a{};
+    a.O = c->O; a.W = c->W; a.P = c->P; a.K = c->K; a.pos = c->pos; a.S = c->S; a.I = c->I; a.itype = c->itype;
+    a.nO = c->nO; a.dO = c->dO; a.nP = c->nP; a.dP = c->dP; a.pbound = c->par.pbound; a.tw = c->tw; a.twi = c->twi;
+    return a;
+}
+
+// The three passes over one chunk.  fwd/col/inv select the kernel variants.
+template <int N> void launch_passes(ptycho_ctx* c, const FrameArgs& a, int nframes, int fwd, int col, int inv) {
+    using G = Geo<N>;
+    const dim3 grid(G::NCB, nframes), blk(kThreads);
+    const size_t sr = G::smem_rows, scs = G::smem_cols(c->K);
+    cudaStream_t s = c->stream;
+    if (fwd == RF_EXIT) k_rows_fwd<N, RF_EXIT><<<grid, blk, sr, s>>>(a);
+    else if (fwd == RF_DM) k_rows_fwd<N, RF_DM><<<grid, blk, sr, s>>>(a);
+    else if (fwd == RF_PLAIN) k_rows_fwd<N, RF_PLAIN><<<grid, blk, sr, s>>>(a);
+    if (fwd >= 0) ++c->launches;
+    if (col == CM_FULL) k_cols<N, CM_FULL><<<grid, blk, scs, s>>>(a);
+    else if (col == CM_ERRONLY) k_cols<N, CM_ERRONLY><<<grid, blk, scs, s>>>(a);
+    else if (col == CM_PLAIN_FWD) k_cols<N, CM_PLAIN_FWD><<<grid, blk, scs, s>>>(a);
+    else if (col == CM_PLAIN_INV) k_cols<N, CM_PLAIN_INV><<<grid, blk, scs, s>>>(a);
+    if (col >= 0) ++c->launches;
+    if (inv == RI_MINIBATCH) k_rows_inv<N, RI_MINIBATCH><<<grid, blk, sr, s>>>(a);
+    else if (inv == RI_DM) k_rows_inv<N, RI_DM><<<grid, blk, sr, s>>>(a);
+    else if (inv == RI_REVISED) k_rows_inv<N, RI_REVISED><<<grid, blk, sr, s>>>(a);
+    else if (inv == RI_PLAIN) k_rows_inv<N, RI_PLAIN><<<grid, blk, sr, s>>>(a);
+    if (inv >= 0) ++c->launches;
+}
+
+void passes(ptycho_ctx* c, const FrameArgs& a, int nframes, int fwd, int col, int inv) {
+    switch (c->N) {
+        case 64: launch_passes<64>(c, a, nframes, fwd, col, inv); break;
+        case 128: launch_passes<128>(c, a, nframes, fwd, col, inv); break;
+        case 256: launch_passes<256>(c, a, nframes, fwd, col, inv); break;
+        default: launch_passes<512>(c, a, nframes, fwd, col, inv); break;
+    }
+}
+
+int ew_blocks(size_t n) { return (int)std::min<size_t>(kRedBlocks, (n + 255) / 256); }
+
+// spatial order (H6): tiles of N/2 rows, boustrophedon in x, so that consecutive frames overlap
+void spatial_sort(std::vector<int>& idx, const int32_t* pos, int n) {
+    const int tile = std::max(1, n / 2);
+    std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) {
+        const int ra = pos[2 * a] / tile, rb = pos[2 * b] / tile;
+        if (ra != rb) return ra < rb;
+        const int xa = pos[2 * a + 1], xb = pos[2 * b + 1];
+        return (ra & 1) ? xa > xb : xa < xb;
+    });
+}
+
+ptycho_status dm_iteration(ptycho_ctx* c) {
+    const size_t nn = (size_t)c->N * c->N, knn = nn * c->K, HW = (size_t)c->H * c->W;
+    const int ncb = ncb_of(c->N);
+    if (!c->psi_valid) {
+        const dim3 g((unsigned)((knn + 255) / 256), c->J);
+        k_init_psi<<<g, 256, 0, c->stream>>>(c->psi, c->O, c->W, c->P, c->K, c->N, c->pos, c->dm_frames);
+        ++c->launches;
+        c->psi_valid = true;
+    }
+    for (int s0 = 0; s0 < c->J; s0 += c->chunk) {
+        const int nf = std::min(c->chunk, c->J - s0);
+        FrameArgs a = base_args(c);
+        a.psi = c->psi + (size_t)s0 * knn;
+        a.frames = c->dm_frames + s0;
+        a.e_part = c->e_part + (size_t)s0 * ncb;
+        passes(c, a, nf, RF_DM, CM_FULL, RI_DM);
+    }
+    const int upd = c->t >= c->par.probe_start;
+    k_dm_blend<<<ew_blocks(HW), 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1);
+    k_dm_blend<<<ew_blocks(nn), 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd);
+    c->launches += 2;
+    return PTYCHO_OK;
+}
+
+ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
+    const size_t nn = (size_t)c->N * c->N, HW = (size_t)c->H * c->W;
+    const int ncb = ncb_of(c->N);
+    const int upd = c->t >= c->par.probe_start;
+    const int nb = (int)c->mb_offsets.size() - 1;
+    for (int b = 0; b < nb; ++b) {
+        const int b0 = c->mb_offsets[b], b1 = c->mb_offsets[b + 1];
+        k_probe_max<<<1, 1024, 0, c->stream>>>(c->P, c->K, (int)nn, c->sc);
+        ++c->launches;
+        for (int s0 = b0; s0 < b1; s0 += c->chunk) {
+            const int nf = std::min(c->chunk, b1 - s0);
+            FrameArgs a = base_args(c);
+            a.frames = c->mb_frames + s0;
+            a.e_part = c->e_part + (size_t)s0 * ncb;
+            passes(c, a, nf, RF_EXIT, CM_FULL, RI_MINIBATCH);
+        }
+        const bool lsq = alg == PTYCHO_LSQML;
+        const int gO = ew_blocks(HW), gP = ew_blocks(nn);
+        k_direction<<<gO, 256, 0, c->stream>>>(c->nO, c->dO, HW, 1, c->par.delta_obj, c->sc, 0, lsq ? c->partO : nullptr);
+        ++c->launches;
+        if (upd) {
+            k_real_max<<<1, 1024, 0, c->stream>>>(c->dP, (int)nn, c->sc);
+            k_direction<<<gP, 256, 0, c->stream>>>(c->nP, c->dP, nn, c->K, c->par.delta_probe, c->sc, 1, lsq ? c->partP : nullptr);
+            c->launches += 2;
+        }
+        double* step_slot = c->n_steps < kStepCap ? c->steps + 2 * c->n_steps : nullptr;
+        if (lsq) {
+            if (upd) {
+                k_lsq_cross<<<b1 - b0, 256, 0, c->stream>>>(c->O, c->nO, c->W, c->P, c->nP, c->K, c->N, c->pos,
+                                                             c->mb_frames + b0, c->partX);
+                ++c->launches;
+            }
+            k_lsq_solve<<<1, 32, 0, c->stream>>>(c->partO, gO, c->partP, upd ? gP : 0, c->partX, upd ? b1 - b0 : 0,
+                                                  c->par.lsq_lambda, upd, c->sc, step_slot ? step_slot : c->scratch_d);
+        } else {
+            k_set_steps<<<1, 1, 0, c->stream>>>(c->sc, c->par.alpha_obj, upd ? c->par.alpha_probe : 0.f, step_slot);
+        }
+        ++c->launches;
+        ++c->n_steps;
+        k_apply<<<gO, 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1);
+        k_apply<<<gP, 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd);
+        c->launches += 2;
+    }
+    c->psi_valid = false;
+    return PTYCHO_OK;
+}
+
+}  // namespace
+
+// =========================================================================================
+// C ABI
+// =========================================================================================
+extern "C" {
+
+void ptycho_default_params(ptycho_params* p) {
+    if (!p) return;
+    memset(p, 0, sizeof(*p));
+    p->delta_blend = 1e-2f;
+    p->delta_obj = 1.0f;
+    p->delta_probe = 1.0f;
+    p->alpha_obj = 1.0f;
+    p->alpha_probe = 1.0f;
+    p->lsq_lambda = 0.1f;
+}
+
+size_t ptycho_workspace_bytes(int obj_h, int obj_w, int n, int n_modes, int n_pos, ptycho_itype itype,
+                              int intensities_on_host, const ptycho_params* params) {
+    if (!valid_n(n) || n_modes < 1 || n_modes > PTYCHO_MAX_MODES || n_pos < 1 || obj_h < n || obj_w < n) return 0;
+    ptycho_ctx tmp;
+    tmp.H = obj_h; tmp.W = obj_w; tmp.N = n; tmp.K = n_modes; tmp.J = n_pos; tmp.itype = itype;
+    if (params) tmp.par = *params; else ptycho_default_params(&tmp.par);
+    tmp.chunk = chunk_frames(n, n_modes, n_pos);
+    return layout(&tmp, nullptr, intensities_on_host != 0);
+}
+
+ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int obj_w, const float* probe,
+                          int n_modes, int n, const int32_t* pos_yx, int n_pos, const void* intensities,
+                          ptycho_itype itype, const ptycho_params* params, void* workspace, size_t workspace_bytes,
+                          void* cuda_stream) {
+    ptycho_ctx* c = nullptr;
+    if (!out) return PTYCHO_EINVAL;
+    *out = nullptr;
+    if (!object || !probe || !pos_yx || !intensities || !workspace) return PTYCHO_EINVAL;
+    if (!valid_n(n) || n_modes < 1 || n_pos < 1 || obj_h < n || obj_w < n) return PTYCHO_EINVAL;
+    if (itype != PTYCHO_I_F32 && itype != PTYCHO_I_U16) return PTYCHO_EINVAL;
+    if (n_modes > PTYCHO_MAX_MODES) return PTYCHO_EUNSUPPORTED;
+    ptycho_params par;
+    if (params) par = *params; else ptycho_default_params(&par);
+    if (par.batch_size < 0 || par.pbound < 0 || par.delta_blend <= 0 || par.delta_obj <= 0 || par.delta_probe <= 0)
+        return PTYCHO_EINVAL;
+    if (par.deterministic) return PTYCHO_EUNSUPPORTED;   // sorted-tile gather mode: not built yet
+    if (cols_smem(n, n_modes) > 227 * 1024) return PTYCHO_EUNSUPPORTED;
+
+    // positions: copy, check bounds (R10), accept host or device memory
+    std::vector<int32_t> pos(2 * (size_t)n_pos);
+    if (is_device_ptr(pos_yx)) {
+        if (cudaMemcpy(pos.data(), pos_yx, pos.size() * 4, cudaMemcpyDeviceToHost) != cudaSuccess) return PTYCHO_ECUDA;
+    } else memcpy(pos.data(), pos_yx, pos.size() * 4);
+    for (int j = 0; j < n_pos; ++j) {
+        const int y = pos[2 * j], x = pos[2 * j + 1];
+        if (y < 0 || x < 0 || y + n > obj_h || x + n > obj_w) return PTYCHO_EBOUNDS;
+    }
+    if (par.batch_order) {                                  // must be a permutation
+        std::vector<char> seen(n_pos, 0);
+        for (int i = 0; i < n_pos; ++i) {
+            const int v = par.batch_order[i];
+            if (v < 0 || v >= n_pos || seen[v]) return PTYCHO_EINVAL;
+            seen[v] = 1;
+        }
+    }
+    if (!is_device_ptr(workspace)) return PTYCHO_EINVAL;
+
+    c = new ptycho_ctx;
+    c->H = obj_h; c->W = obj_w; c->N = n; c->K = n_modes; c->J = n_pos; c->itype = itype; c->par = par;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->chunk = chunk_frames(n, n_modes, n_pos);
+    const bool dev_I = is_device_ptr(intensities);
+    const size_t need = layout(c, nullptr, !dev_I);
+    if (workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 255)) { delete c; return PTYCHO_ENOMEM; }
+    layout(c, workspace, !dev_I);
+    if (dev_I) c->I = intensities;
+
+#define CUI(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { fprintf(stderr, "ptycho_init: %s: %s\n", #call, cudaGetErrorString(e_)); delete c; return PTYCHO_ECUDA; } } while (0)
+    ptycho_status st = PTYCHO_OK;
+    switch (n) {
+        case 64: st = set_attrs<64>(c); break;
+        case 128: st = set_attrs<128>(c); break;
+        case 256: st = set_attrs<256>(c); break;
+        default: st = set_attrs<512>(c); break;
+    }
+    if (st != PTYCHO_OK) { fprintf(stderr, "ptycho_init: %s\n", c->err.c_str()); delete c; return st; }
+
+    const size_t HW = (size_t)obj_h * obj_w, nn = (size_t)n * n, knn = nn * n_modes;
+    cudaStream_t s = c->stream;
+    CUI(cudaMemcpyAsync(c->O, object, HW * 8, cudaMemcpyDefault, s));
+    CUI(cudaMemcpyAsync(c->P, probe, knn * 8, cudaMemcpyDefault, s));
+    if (!dev_I) CUI(cudaMemcpyAsync(const_cast<void*>(c->I), intensities, (size_t)n_pos * nn * (itype == PTYCHO_I_U16 ? 2 : 4), cudaMemcpyDefault, s));
+    CUI(cudaMemcpyAsync(c->pos, pos.data(), pos.size() * 4, cudaMemcpyHostToDevice, s));
+    CUI(cudaMemsetAsync(c->nO, 0, HW * 8, s));
+    CUI(cudaMemsetAsync(c->dO, 0, HW * 4, s));
+    CUI(cudaMemsetAsync(c->nP, 0, knn * 8, s));
+    CUI(cudaMemsetAsync(c->dP, 0, nn * 4, s));
+    CUI(cudaMemsetAsync(c->sc, 0, sizeof(Scalars), s));
+    CUI(cudaMemsetAsync(c->err_hist, 0, sizeof(double) * kErrCap, s));
+
+    std::vector<float2> tw, twi;
+    const int E = n == 64 ? 8 : n == 512 ? 32 : 16, T = n / E;
+    host_twiddles(n, E, T, tw, twi);
+    CUI(cudaMemcpyAsync(c->tw, tw.data(), n * 8, cudaMemcpyHostToDevice, s));
+    CUI(cudaMemcpyAsync(c->twi, twi.data(), n * 8, cudaMemcpyHostToDevice, s));
+
+    // frame orders: DM = all frames, spatially sorted; minibatch = batches (R8), each sorted
+    c->dm_order.resize(n_pos);
+    std::iota(c->dm_order.begin(), c->dm_order.end(), 0);
+    spatial_sort(c->dm_order, pos.data(), n);
+    c->slot_of_h.resize(n_pos);
+    for (int sidx = 0; sidx < n_pos; ++sidx) c->slot_of_h[c->dm_order[sidx]] = sidx;
+    std::vector<int> mb;
+    mb.reserve(n_pos);
+    c->mb_offsets.assign(1, 0);
+    const int B = par.batch_size;
+    if (B <= 0 || B >= n_pos) {
+        mb = c->dm_order;
+        c->mb_offsets.push_back(n_pos);
+    } else if (par.batch_order) {
+        for (int s0 = 0; s0 < n_pos; s0 += B) {
+            std::vector<int> fr(par.batch_order + s0, par.batch_order + std::min(n_pos, s0 + B));
+            spatial_sort(fr, pos.data(), n);
+            mb.insert(mb.end(), fr.begin(), fr.end());
+            c->mb_offsets.push_back((int)mb.size());
+        }
+    } else {
+        const int nb = (n_pos + B - 1) / B;
+        for (int b = 0; b < nb; ++b) {
+            std::vector<int> fr;
+            for (int j = b; j < n_pos; j += nb) fr.push_back(j);
+            spatial_sort(fr, pos.data(), n);
+            mb.insert(mb.end(), fr.begin(), fr.end());
+            c->mb_offsets.push_back((int)mb.size());
+        }
+    }
+    c->par.batch_order = nullptr;   // copied; the caller's pointer is not kept
+    CUI(cudaMemcpyAsync(c->dm_frames, c->dm_order.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
+    CUI(cudaMemcpyAsync(c->mb_frames, mb.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
+    CUI(cudaMemcpyAsync(c->slot_of, c->slot_of_h.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
+
+    // init-time constants on the device: eps_O, eps_P (R5), sum_I (C3)
+    k_probe_max<<<1, 1024, 0, s>>>(c->P, c->K, (int)nn, c->sc);
+    k_finish_init<<<1, 1, 0, s>>>(c->sc, par.delta_blend, n_pos, 0);
+    k_abs2_max<<<ew_blocks(HW), 256, 0, s>>>(c->O, HW, c->sc);
+    k_finish_init<<<1, 1, 0, s>>>(c->sc, par.delta_blend, n_pos, 1);
+    k_sum_intensity<<<kRedBlocks, 256, 0, s>>>(c->I, itype, (size_t)n_pos * nn, c->scratch_d);
+    k_finish_sum_I<<<1, 1, 0, s>>>(c->scratch_d, kRedBlocks, c->sc);
+    c->launches += 6;
+    CUI(cudaStreamSynchronize(s));
+    CUI(cudaGetLastError());
+#undef CUI
+    *out = c;
+    return PTYCHO_OK;
+}
+
+ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
+    if (!c || n_iters < 0) return PTYCHO_EINVAL;
+    if (alg != PTYCHO_EPIE_MB && alg != PTYCHO_DM && alg != PTYCHO_LSQML) return fail(c, PTYCHO_EINVAL, "unknown algorithm");
+    if (alg == PTYCHO_DM && !c->psi) return fail(c, PTYCHO_ESTATE, "DM needs the exit-wave store (disable_dm was set)");
+    for (int it = 0; it < n_iters; ++it) {
+        ptycho_status st = alg == PTYCHO_DM ? dm_iteration(c) : minibatch_iteration(c, alg);
+        if (st != PTYCHO_OK) return st;
+        double* slot = c->err_hist + (c->t < kErrCap ? c->t : kErrCap - 1);
+        k_sum_error<<<1, 1024, 0, c->stream>>>(c->e_part, (size_t)c->J * ncb_of(c->N), c->sc, slot);
+        ++c->launches;
+        ++c->t;
+    }
+    CU(cudaGetLastError());
+    return PTYCHO_OK;
+}
+
+ptycho_status ptycho_fetch_object(ptycho_ctx* c, float* out) {
+    if (!c || !out) return PTYCHO_EINVAL;
+    CU(cudaMemcpyAsync(out, c->O, (size_t)c->H * c->W * 8, cudaMemcpyDefault, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return PTYCHO_OK;
+}
+ptycho_status ptycho_fetch_probe(ptycho_ctx* c, float* out) {
+    if (!c || !out) return PTYCHO_EINVAL;
+    CU(cudaMemcpyAsync(out, c->P, (size_t)c->K * c->N * c->N * 8, cudaMemcpyDefault, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return PTYCHO_OK;
+}
+ptycho_status ptycho_fetch_error(ptycho_ctx* c, double* out, int cap, int* n_written) {
+    if (!c || (!out && cap > 0) || cap < 0) return PTYCHO_EINVAL;
+    const int n = std::min(std::min(c->t, cap), kErrCap);
+    if (n > 0) CU(cudaMemcpyAsync(out, c->err_hist, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (n_written) *n_written = c->t;
+    return PTYCHO_OK;
+}
+ptycho_status ptycho_fetch_steps(ptycho_ctx* c, double* out, int cap, int* n_written) {
+    if (!c || (!out && cap > 0) || cap < 0) return PTYCHO_EINVAL;
+    const int n = (int)std::min<long long>(std::min<long long>(c->n_steps, cap), kStepCap);
+    if (n > 0) CU(cudaMemcpyAsync(out, c->steps, sizeof(double) * 2 * n, cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (n_written) *n_written = (int)c->n_steps;
+    return PTYCHO_OK;
+}
+
+ptycho_status ptycho_set_object(ptycho_ctx* c, const float* object) {
+    if (!c || !object) return PTYCHO_EINVAL;
+    CU(cudaMemcpyAsync(c->O, object, (size_t)c->H * c->W * 8, cudaMemcpyDefault, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return PTYCHO_OK;
+}
+ptycho_status ptycho_set_probe(ptycho_ctx* c, const float* probe) {
+    if (!c || !probe) return PTYCHO_EINVAL;
+    CU(cudaMemcpyAsync(c->P, probe, (size_t)c->K * c->N * c->N * 8, cudaMemcpyDefault, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return PTYCHO_OK;
+}
+
+// Exit waves move through the scratch S in chunks so that host buffers of any size work.
+ptycho_status ptycho_fetch_exit_waves(ptycho_ctx* c, const int32_t* idx, int count, float* out) {
+    if (!c || !idx || !out || count < 0) return PTYCHO_EINVAL;
+    if (!c->psi || !c->psi_valid) return fail(c, PTYCHO_ESTATE, "no exit waves stored (run DM or set them first)");
+    const size_t knn = (size_t)c->K * c->N * c->N;
+    std::vector<int> slots(count);
+    for (int i = 0; i < count; ++i) {
+        if (idx[i] < 0 || idx[i] >= c->J) return fail(c, PTYCHO_EINVAL, "frame index out of range");
+        slots[i] = c->slot_of_h[idx[i]];
+    }
+    for (int s0 = 0; s0 < count; s0 += c->chunk) {
+        const int nf = std::min(c->chunk, count - s0);
+        CU(cudaMemcpyAsync(c->tmp_idx, slots.data() + s0, nf * 4, cudaMemcpyHostToDevice, c->stream));
+        k_copy_frames<<<dim3(64, nf), 256, 0, c->stream>>>(c->S, c->psi, nullptr, c->tmp_idx, knn);
+        ++c->launches;
+        CU(cudaMemcpyAsync(out + (size_t)s0 * knn * 2, c->S, (size_t)nf * knn * 8, cudaMemcpyDefault, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+    }
+    return PTYCHO_OK;
+}
+ptycho_status ptycho_set_exit_waves(ptycho_ctx* c, const float* psi) {
+    if (!c || !psi) return PTYCHO_EINVAL;
+    if (!c->psi) return fail(c, PTYCHO_ESTATE, "no exit-wave store (disable_dm was set)");
+    const size_t knn = (size_t)c->K * c->N * c->N;
+    for (int j0 = 0; j0 < c->J; j0 += c->chunk) {
+        const int nf = std::min(c->chunk, c->J - j0);
+        CU(cudaMemcpyAsync(c->S, psi + (size_t)j0 * knn * 2, (size_t)nf * knn * 8, cudaMemcpyDefault, c->stream));
+        k_copy_frames<<<dim3(64, nf), 256, 0, c->stream>>>(c->psi, c->S, c->slot_of + j0, nullptr, knn);
+        ++c->launches;
+    }
+    CU(cudaStreamSynchronize(c->stream));
+    c->psi_valid = true;
+    return PTYCHO_OK;
+}
+
+ptycho_status ptycho_revised_waves(ptycho_ctx* c, const int32_t* idx, int count, float* out) {
+    if (!c || !idx || !out || count < 0) return PTYCHO_EINVAL;
+    for (int i = 0; i < count; ++i)
+        if (idx[i] < 0 || idx[i] >= c->J) return fail(c, PTYCHO_EINVAL, "frame index out of range");
+    const size_t knn = (size_t)c->K * c->N * c->N;
+    for (int s0 = 0; s0 < count; s0 += c->chunk) {
+        const int nf = std::min(c->chunk, count - s0);
+        CU(cudaMemcpyAsync(c->tmp_idx, idx + s0, nf * 4, cudaMemcpyHostToDevice, c->stream));
+        FrameArgs a = base_args(c);
+        a.frames = c->tmp_idx;
+        a.e_part = c->e_tmp;
+        a.out = c->S;   // in place: every CTA reads its rows of S before it writes them
+        passes(c, a, nf, RF_EXIT, CM_FULL, RI_REVISED);
+        CU(cudaMemcpyAsync(out + (size_t)s0 * knn * 2, c->S, (size_t)nf * knn * 8, cudaMemcpyDefault, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+    }
+    return PTYCHO_OK;
+}
+
+ptycho_status ptycho_eval_error(ptycho_ctx* c, double* out) {
+    if (!c || !out) return PTYCHO_EINVAL;
+    const int ncb = ncb_of(c->N);
+    for (int s0 = 0; s0 < c->J; s0 += c->chunk) {
+        const int nf = std::min(c->chunk, c->J - s0);
+        FrameArgs a = base_args(c);
+        a.frames = c->dm_frames + s0;
+        a.e_part = c->e_tmp + (size_t)s0 * ncb;
+        passes(c, a, nf, RF_EXIT, CM_ERRONLY, -1);
+    }
+    k_sum_error<<<1, 1024, 0, c->stream>>>(c->e_tmp, (size_t)c->J * ncb, c->sc, c->scratch_d);
+    ++c->launches;
+    CU(cudaMemcpyAsync(out, c->scratch_d, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return PTYCHO_OK;
+}
+
+long long ptycho_launch_count(const ptycho_ctx* c) { return c ? c->launches : 0; }
+const char* ptycho_last_error(const ptycho_ctx* c) { return c ? c->err.c_str() : ""; }
+void ptycho_destroy(ptycho_ctx* c) { delete c; }
+
+__global__ void k_scale(float2* d, size_t n, float s) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) { d[i].x *= s; d[i].y *= s; }
+}
+
+ptycho_status ptycho_test_fft2(float* data, int n, int count, int inverse, void* cuda_stream) {
+    if (!data || !valid_n(n) || count < 1) return PTYCHO_EINVAL;
+    ptycho_ctx tmp;
+    ptycho_ctx* c = &tmp;
+    c->N = n; c->K = 1; c->stream = static_cast<cudaStream_t>(cuda_stream);
+    ptycho_status st = n == 64 ? set_attrs<64>(c) : n == 128 ? set_attrs<128>(c) : n == 256 ? set_attrs<256>(c) : set_attrs<512>(c);
+    if (st != PTYCHO_OK) return st;
+    std::vector<float2> tw, twi;
+    const int E = n == 64 ? 8 : n == 512 ? 32 : 16;
+    host_twiddles(n, E, n / E, tw, twi);
+    float2* d_tw = nullptr;
+    CU(cudaMalloc(&d_tw, 2 * n * sizeof(float2)));
+    CU(cudaMemcpy(d_tw, tw.data(), n * 8, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(d_tw + n, twi.data(), n * 8, cudaMemcpyHostToDevice));
+    FrameArgs a{};
+    a.S = reinterpret_cast<float2*>(data); a.K = 1; a.tw = d_tw; a.twi = d_tw + n;
+    if (!inverse) passes(c, a, count, RF_PLAIN, CM_PLAIN_FWD, -1);
+    else {
+        passes(c, a, count, -1, CM_PLAIN_INV, RI_PLAIN);
+        const size_t tot = (size_t)count * n * n;
+        k_scale<<<ew_blocks(tot), 256, 0, c->stream>>>(a.S, tot, 1.0f / ((float)n * n));
+    }
+    CU(cudaStreamSynchronize(c->stream));
+    CU(cudaGetLastError());
+    cudaFree(d_tw);
+    return PTYCHO_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,187 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerances (BASELINE.json north_star): per-iteration exit-wave and object relative L2 <= 1e-4,
+<= 1e-3 after 50 iterations.  Integer/bit-exact parts: frame order bookkeeping (fetch by index).
+"""
+import numpy as np
+import pytest
+
+from paper_2202_03144_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_ITER = 1e-4
+TOL_RUN = 1e-3
+
+
+def rel(a, b):
+    a, b = np.asarray(a, np.complex128).ravel(), np.asarray(b, np.complex128).ravel()
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2202_03144_b200 import binding
+    binding.lib()
+    return binding
+
+
+def make(B, s, **par):
+    return B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(**par))
+
+
+# ------------------------------------------------------------------------------ T2: FFT alone
+@pytest.mark.parametrize("n", [64, 128, 256, 512])
+def test_fft2_vs_oracle(B, oracle_mod, n):
+    import torch
+    rng = np.random.default_rng(n)
+    x = (rng.standard_normal((5, n, n)) + 1j * rng.standard_normal((5, n, n))).astype(np.complex64)
+    d = torch.from_numpy(x).cuda()
+    f = B.test_fft2(d.clone()).cpu().numpy()
+    want = np.stack([oracle_mod.fft2(v) for v in x])
+    assert rel(f, want) < 2e-6
+    back = B.test_fft2(torch.from_numpy(want.astype(np.complex64)).cuda(), inverse=True).cpu().numpy()
+    assert rel(back, x) < 2e-6
+
+
+# ------------------------------------------------------------- T3/T4 on config 0 (full size)
+@pytest.mark.parametrize("probe_start", [10 ** 9, 0])
+def test_cfg0_dm_free_running(B, oracle_mod, probe_start):
+    s = synth.make_config(0)
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(probe_start=probe_start))
+    g = make(B, s, probe_start=probe_start)
+    for it in range(10):
+        o.iterate("DM", 1)
+        g.iterate("DM", 1)
+        assert rel(g.fetch_object(), o.O) < TOL_RUN, it
+    assert rel(g.fetch_exit_waves(), o.psi) < TOL_RUN
+    assert rel(g.fetch_probe(), o.P) < TOL_RUN
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+    sel = np.array([5, 63, 0, 17], np.int32)                 # caller numbering survives the sort
+    assert rel(g.fetch_exit_waves(sel), o.psi[sel]) < TOL_RUN
+
+
+def test_cfg0_dm_teacher_forced(B, oracle_mod):
+    s = synth.make_config(0)
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities)
+    g = make(B, s)
+    o.iterate("DM", 1)
+    g.iterate("DM", 1)
+    for it in range(1, 6):
+        g.set_object(o.O)
+        g.set_probe(o.P)
+        g.set_exit_waves(o.psi.astype(np.complex64))
+        o.iterate("DM", 1)
+        g.iterate("DM", 1)
+        assert rel(g.fetch_exit_waves(), o.psi) < TOL_ITER, it
+        assert rel(g.fetch_object(), o.O) < TOL_ITER, it
+        assert rel(g.fetch_probe(), o.P) < TOL_ITER, it
+
+
+@pytest.mark.parametrize("alg", ["EPIE_MB", "LSQML"])
+def test_cfg0_minibatch(B, oracle_mod, alg):
+    s = synth.make_config(0)
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(batch_size=16), keep_revised=True)
+    g = make(B, s, batch_size=16)
+    for it in range(10):
+        rv = g.revised_waves()                                # of the current (pre-iteration) state
+        o.iterate(alg, 1)
+        g.iterate(alg, 1)
+        if it == 0:
+            pass
+        assert rel(g.fetch_object(), o.O) < TOL_RUN, it
+        assert rel(g.fetch_probe(), o.P) < TOL_RUN, it
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3, atol=1e-9)
+    if alg == "LSQML":
+        assert np.allclose(g.fetch_steps(), np.array(o.steps), rtol=2e-3)
+    assert g.eval_error() == pytest.approx(o.eval_error(), rel=2e-3)
+
+
+def test_revised_waves_teacher_forced(B, oracle_mod):
+    """Full-batch ePIE: the oracle's revised waves of iteration t belong to the state before it."""
+    s = synth.make_config(0)
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, keep_revised=True)
+    g = make(B, s)
+    for it in range(3):
+        g.set_object(o.O)
+        g.set_probe(o.P)
+        rv = g.revised_waves()
+        o.iterate("EPIE_MB", 1)
+        g.iterate("EPIE_MB", 1)
+        assert rel(rv, o.revised) < TOL_ITER
+        assert rel(g.fetch_object(), o.O) < TOL_ITER and rel(g.fetch_probe(), o.P) < TOL_ITER
+
+
+# -------------------------------------------------- every size, modes, uint16, masks, pbound
+@pytest.mark.parametrize("n,h,side,step,k,alg,kw", [
+    (64, 160, 5, 13, 1, "DM", dict(pbound=0.2)),
+    (64, 160, 5, 13, 3, "LSQML", dict(batch_size=7)),
+    (64, 160, 5, 13, 2, "DM", dict(pbound=0.1)),
+    (128, 300, 5, 31, 1, "EPIE_MB", dict(batch_size=10)),
+    (128, 300, 5, 31, 1, "DM", dict(pbound=0.12)),
+    (256, 520, 4, 61, 1, "DM", dict(pbound=0.5)),
+    (256, 520, 4, 61, 3, "LSQML", dict(batch_size=6)),
+    (256, 520, 3, 90, 1, "EPIE_MB", dict(batch_size=4, probe_start=2)),
+    (512, 900, 3, 150, 1, "DM", dict(pbound=0.5)),
+    (512, 900, 2, 200, 2, "LSQML", dict()),
+])
+def test_sizes_modes_uint16(B, oracle_mod, n, h, side, step, k, alg, kw):
+    s = synth.make_custom(n, h, side, step, k=k, peak=2e4, dtype=np.uint16, jitter=3, seed=n + k,
+                          probe_kind="zone" if alg == "DM" else "disk")
+    s.intensities[1, 3, 5] = 65535                             # a masked pixel (R3)
+    s.intensities[2, 0, 0] = 65535
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, kw)
+    g = make(B, s, **kw)
+    for it in range(4):
+        o.iterate(alg, 1)
+        g.iterate(alg, 1)
+        assert rel(g.fetch_object(), o.O) < TOL_ITER * (it + 1), it
+        assert rel(g.fetch_probe(), o.P) < TOL_ITER * (it + 1), it
+    if alg == "DM":
+        assert rel(g.fetch_exit_waves(), o.psi) < 4 * TOL_ITER
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+
+
+def test_switching_algorithms_and_state(B, oracle_mod):
+    """DM after a minibatch algorithm re-initialises psi = P O_j; the counter is global."""
+    s = synth.make_config(0)
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(batch_size=16, probe_start=3))
+    g = make(B, s, batch_size=16, probe_start=3)
+    for alg, n in (("DM", 2), ("EPIE_MB", 2), ("DM", 2), ("LSQML", 1)):
+        o.iterate(alg, n)
+        g.iterate(alg, n)
+    assert rel(g.fetch_object(), o.O) < TOL_RUN and rel(g.fetch_probe(), o.P) < TOL_RUN
+    assert len(g.fetch_error()) == 7
+    with pytest.raises(B.PtychoError):
+        g.fetch_exit_waves()                                   # ESTATE: a minibatch ran last
+
+
+def test_error_codes(B):
+    s = synth.make_config(0)
+    bad = s.pos.copy()
+    bad[3, 1] = 192 - 63
+    with pytest.raises(B.PtychoError, match="EBOUNDS"):
+        B.Ptycho(s.obj0, s.probe0, bad, s.intensities)
+    with pytest.raises(B.PtychoError):
+        B.Ptycho(s.obj0, s.probe0[:, :48, :48], s.pos, s.intensities[:, :48, :48])
+    g = B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(disable_dm=1))
+    with pytest.raises(B.PtychoError, match="ESTATE"):
+        g.iterate("DM", 1)
+    g.iterate("EPIE_MB", 1)
+    assert g.launch_count() > 0
+
+
+def test_device_resident_inputs(B, oracle_mod):
+    """Device pointers are accepted everywhere (intensities borrowed, state fetched to device)."""
+    import torch
+    s = synth.make_config(0)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    g = B.Ptycho(dev(s.obj0.astype(np.complex64)), dev(s.probe0.astype(np.complex64)), s.pos,
+                 dev(s.intensities), B.default_params())
+    g.iterate("DM", 3)
+    out = torch.empty((192, 192), dtype=torch.complex64, device="cuda")
+    g.fetch_object(out)
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities).iterate("DM", 3)
+    assert rel(out.cpu().numpy(), o.O) < TOL_RUN

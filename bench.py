@@ -1,0 +1,312 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the projection cycle (BASELINE.json `metric`).
+
+    python bench.py --gpus N --steps K --warmup W            # this build (CUDA path, C ABI)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle as it stands
+
+A "step" is one DM iteration over all J scan positions of config 2 (BASELINE.json configs[2]: DM,
+256x256 frames, 10 000 Fermat-spiral positions, 4096^2 object, uint16 Poisson counts) -- the
+configuration the metric "diffraction patterns/sec per DM iteration (256x256, 1 B200)" is quoted
+on.  `value` = J * K / (device time of K iterations), inputs resident in HBM; `e2e` = the same
+through the C ABI from pinned HOST buffers: ptycho_init (H2D of intensities, object, probe,
+positions) + one DM iteration + ptycho_fetch_error, all inside the timed region.
+N > 1: the path does not shard in this build ("replicas only"): every rank
+reconstructs its own replica scan, no data-path collective; time = max over ranks.
+
+Prints ONE JSON line (rank 0).  Inputs are seeded synthetic scans (paper_2202_03144_b200/synth.py).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+_ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, _ROOT)
+
+METRIC = "diffraction patterns/sec per DM iteration (256x256, 1 B200); % HBM roofline"
+UNIT = "patterns/s"
+CFG = 2                      # BASELINE.json configs[2]
+REF_SAMPLE = 256             # frames of the bounded oracle sample (first positions of the same scan)
+
+
+def algorithmic_bytes_per_pattern(n: int, k: int, bytes_i: int) -> int:
+    """DM streams psi in, psi out and I in: N^2 (16 K + b_I)."""
+    return n * n * (16 * k + bytes_i)
+
+
+def measured_peaks():
+    p = os.path.join(_ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# --------------------------------------------------------------------------- clocks during the run
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML every `period` seconds."""
+
+    BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
+    NOTE = {"sw_power_cap": 0x4, "hw_power_brake": 0x80, "sync_boost": 0x10}
+
+    def __init__(self, index: int, period: float = 0.01, uuid: str | None = None):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples: list[tuple[float, int, int]] = []
+        self.max_mhz = None
+        self._stop_ev = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:                                             # CUDA_VISIBLE_DEVICES may renumber
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid) if uuid and not uuid.startswith("GPU-") else uuid)
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:                               # NVML missing: report that
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        while not self._stop_ev.is_set():
+            try:
+                mhz = int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                try:
+                    rs = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    rs = int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                self.samples.append((time.perf_counter(), mhz, rs))
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_ev.set()
+
+    def summary(self, t0: float, t1: float) -> dict:
+        if not self.ok:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml_unavailable"]}
+        inside = [(m, r) for (t, m, r) in self.samples if t0 <= t <= t1]
+        if not inside:                                       # region shorter than one period
+            inside = [(m, r) for (_, m, r) in self.samples[-3:]]
+        mhz = sorted(m for m, _ in inside)
+        bits = 0
+        for _, r in inside:
+            bits |= r
+        reasons = [k for k, v in {**self.BAD, **self.NOTE}.items() if bits & v]
+        return {"sm_mhz": mhz[len(mhz) // 2] if mhz else None, "sm_max_mhz": self.max_mhz,
+                "reasons": reasons, "samples": len(inside)}
+
+
+# --------------------------------------------------------------------------- reference arm (oracle)
+def run_oracle_sample(steps: int, warmup: int, sample: int = REF_SAMPLE):
+    """Times the CPU oracle (oracle/, as it stands) on the first `sample` positions of config 2:
+    one step = one oracle DM iteration over those frames.  Returns (patterns/s, ms/step, cores)."""
+    import oracle
+    from paper_2202_03144_b200 import synth
+    oracle.build()
+    s = synth.make_config(CFG, n_pos=sample)
+    o = oracle.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(pbound=s.params["pbound"]))
+    for _ in range(warmup):
+        o.iterate("DM", 1)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.iterate("DM", 1)
+    dt = time.perf_counter() - t0
+    cores = int(os.environ.get("OMP_NUM_THREADS", 0)) or (os.cpu_count() or 1)
+    return sample * steps / dt, dt / steps * 1e3, cores
+
+
+def reference_line(args) -> dict:
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    val, ms, cores = run_oracle_sample(steps, warmup)
+    sample = (f"first {REF_SAMPLE} of the 10000 positions of config 2 (same generator), "
+              f"one oracle DM iteration (fp64, OpenMP over frames) per step")
+    return {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "cfg2 DM 256x256 J=10000 H=4096 u16 (bounded sample)", "sample_frames": REF_SAMPLE},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+
+
+# --------------------------------------------------------------------------- this build's arm
+def dist_env():
+    return (int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)),
+            int(os.environ.get("WORLD_SIZE", 1)))
+
+
+def max_over_ranks(x: float, world: int, device=None) -> float:
+    """Slowest rank's time (the contract's max over ranks); identity for a single process."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device if dist.get_backend() == "nccl" else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def barrier(world: int):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def ours_line(args) -> dict | None:
+    import torch
+    rank, local, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the projection cycle has no CPU path "
+                         "(use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_2202_03144_b200 import binding, synth
+    binding.lib()                                            # fails loudly if the .so is missing
+
+    steps, warmup = max(1, args.steps), max(3, args.warmup)
+    s = synth.make_config(CFG, n_pos=args.n_pos, replica=rank, threads=max(2, (os.cpu_count() or 8) // world))
+    J, N, K = s.n_pos, s.n, s.n_modes
+    par = dict(pbound=s.params["pbound"])
+    obj0 = torch.from_numpy(s.obj0.astype(np.complex64))
+    probe0 = torch.from_numpy(s.probe0.astype(np.complex64))
+    inten_h = torch.from_numpy(s.intensities).pin_memory()
+    obj_h, probe_h = obj0.pin_memory(), probe0.pin_memory()
+
+    # ---- device-resident timing: inputs in HBM before the timed region
+    inten_d = inten_h.to(dev)
+    g = binding.Ptycho(obj0.to(dev), probe0.to(dev), s.pos, inten_d, binding.default_params(**par), device=dev)
+    stream = torch.cuda.current_stream(dev)
+    for _ in range(warmup):
+        g.iterate("DM", 1)
+    try:
+        uuid = str(torch.cuda.get_device_properties(dev).uuid)
+    except Exception:
+        uuid = None
+    sampler = ClockSampler(local, uuid=uuid)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(dev)
+    barrier(world)
+    g.profile(True)
+    l0 = g.launch_count()
+    t0 = time.perf_counter()
+    e0.record(stream)
+    for _ in range(steps):
+        g.iterate("DM", 1)
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    t1 = time.perf_counter()
+    barrier(world)
+    ms = max_over_ranks(float(e0.elapsed_time(e1)), world, dev)
+    launches = g.launch_count() - l0
+    prof = g.profile_fetch()
+    g.profile(False)
+    clocks = sampler.summary(t0, t1)
+    err_hist = g.fetch_error()
+    assert np.all(np.isfinite(err_hist)), "non-finite error history"
+    g.destroy()
+    del g, inten_d
+    torch.cuda.empty_cache()
+
+    # ---- end to end through the C ABI from pinned host buffers (H2D + iterate + D2H inside)
+    e2e_steps = min(steps, 10)
+    h2d = inten_h.numel() * inten_h.element_size() + obj_h.numel() * 8 + probe_h.numel() * 8 + s.pos.nbytes
+    e2e_ms = []
+    for i in range(e2e_steps + 1):
+        torch.cuda.synchronize(dev)
+        barrier(world)
+        e0.record(stream)
+        ge = binding.Ptycho(obj_h, probe_h, s.pos, inten_h, binding.default_params(**par), device=dev)
+        ge.iterate("DM", 1)
+        ev = ge.fetch_error()                                # D2H of the step's result (8 bytes)
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        if i > 0:                                            # first one is the warm-up (allocator)
+            e2e_ms.append(float(e0.elapsed_time(e1)))
+        assert np.isfinite(ev[-1])
+        ge.destroy()
+        del ge
+    sampler.stop()
+    e2e_ms_step = max_over_ranks(sum(e2e_ms) / len(e2e_ms), world, dev)
+
+    # ---- roofline of the dominant kernel chain
+    peak, peak_src = measured_peaks()
+    chain = ("rows_fwd", "cols", "rows_inv")
+    chain_ms = sum(prof[k][0] for k in chain)
+    bytes_i = s.intensities.dtype.itemsize
+    alg_bytes = algorithmic_bytes_per_pattern(N, K, bytes_i)
+    achieved = alg_bytes * J * steps / (chain_ms * 1e-3) / 1e9 if chain_ms > 0 else 0.0
+    n_chain = sum(prof[k][1] for k in chain)
+    roofline = {
+        "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "traffic": None, "peak_source": peak_src,
+        "kernel": "k_rows_fwd+k_cols+k_rows_inv chain (one chunk of frames per launch triple)",
+        "algorithmic_bytes_per_pattern": alg_bytes,
+        "launches_timed": n_chain, "avg_launch_ms": chain_ms / max(n_chain, 1),
+        "kernel_ms_per_step": {k: prof[k][0] / steps for k in prof},
+        "step_frac_of_hbm_roofline": (alg_bytes * J * steps * world / (ms * 1e-3) / 1e9) / (peak * world),
+    }
+    line = {
+        "metric": METRIC, "value": J * steps * world / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+        "steps": steps, "warmup": warmup, "ms_per_step": ms / steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"cfg2 DM {N}x{N} J={J} H={s.obj0.shape[0]} u16 K={K} pbound={par['pbound']}",
+                   "l2": "inputs larger than L2 (psi %.2f GB + I %.2f GB streamed per step)" % (J * K * N * N * 8 / 1e9, J * N * N * bytes_i / 1e9),
+                   "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "e2e_step": "ptycho_init from pinned host buffers + 1 DM iteration + ptycho_fetch_error",
+                   "e2e_steps": e2e_steps},
+        "clocks": clocks,
+        "e2e": {"value": J * world / (e2e_ms_step * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": 8, "ms_per_step": e2e_ms_step},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "error_first_last": [float(err_hist[0]), float(err_hist[-1])],
+    }
+    if world == 1 and rank == 0 and not args.no_cpu_baseline:
+        val, _, cores = run_oracle_sample(steps=6, warmup=1)
+        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"first {REF_SAMPLE} positions of config 2, 6 oracle DM iterations (fp64, OpenMP)"}
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return line if rank == 0 else None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n-pos", type=int, default=None, help="truncate the scan (debugging only; invalidates the metric)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank, _, world = dist_env()
+    if args.impl == "reference":
+        if rank == 0:
+            print(json.dumps(reference_line(args)), flush=True)
+        return
+    line = ours_line(args)
+    if line is not None:
+        print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()

@@ -138,6 +138,22 @@ ptycho_status ptycho_set_exit_waves(ptycho_ctx *ctx, const float *psi /* n_pos*n
  * state change; R7).  Synchronises. */
 ptycho_status ptycho_eval_error(ptycho_ctx *ctx, double *out);
 
+/* Per-kernel-class device timing (SURVEY.md 8(d) "Evidence to collect"; bench.py's roofline
+ * object).  ptycho_profile(ctx, 1) resets the totals and makes every later launch of this context
+ * be bracketed by two cudaEvents on the context's stream; ptycho_profile(ctx, 0) stops that.
+ * ptycho_profile_fetch synchronises the stream and returns, for one class, the summed device
+ * time of its launches (ms) and their number since the last reset. */
+typedef enum {
+    PTYCHO_K_ROWS_FWD = 0, /* a1-a3: exit wave, reflector, forward row FFTs                      */
+    PTYCHO_K_COLS = 1,     /* a3-a6: column FFTs, error, modulus projection, inverse column FFTs */
+    PTYCHO_K_ROWS_INV = 2, /* a6-a9: inverse row FFTs, exit-wave update, overlap scatter-add     */
+    PTYCHO_K_UPDATE = 3,   /* a10/a11: normalising updates, step solve, error sum                */
+    PTYCHO_K_OTHER = 4,    /* initial exit waves, frame copies of fetch/set                      */
+    PTYCHO_KCLASS_COUNT = 5
+} ptycho_kclass;
+ptycho_status ptycho_profile(ptycho_ctx *ctx, int enable);
+ptycho_status ptycho_profile_fetch(ptycho_ctx *ctx, int kclass, double *total_ms, long long *n_launches);
+
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 long long ptycho_launch_count(const ptycho_ctx *ctx);
 

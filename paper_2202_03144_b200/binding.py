@@ -18,6 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_CSRC, "libptycho_b200.so")
 ALG = {"EPIE_MB": 0, "DM": 1, "LSQML": 2}
+KCLASS = ["rows_fwd", "cols", "rows_inv", "update", "other"]   # ptycho_kclass
 STATUS = ["OK", "EINVAL", "EBOUNDS", "EUNSUPPORTED", "ENOMEM", "ECUDA", "ESTATE"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "128"]
@@ -72,6 +73,8 @@ def lib():
         l.ptycho_fetch_exit_waves.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         l.ptycho_revised_waves.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         l.ptycho_eval_error.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        l.ptycho_profile.argtypes = [C.c_void_p, C.c_int]
+        l.ptycho_profile_fetch.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         l.ptycho_launch_count.restype = C.c_longlong
         l.ptycho_launch_count.argtypes = [C.c_void_p]
         l.ptycho_last_error.restype = C.c_char_p
@@ -221,6 +224,18 @@ class Ptycho:
         v = C.c_double()
         self._check(self._l.ptycho_eval_error(self._h, C.byref(v)))
         return v.value
+
+    def profile(self, enable: bool = True):
+        self._check(self._l.ptycho_profile(self._h, int(enable)))
+
+    def profile_fetch(self) -> dict:
+        """{class name: (total device ms, launches)} since the last profile(True)."""
+        out = {}
+        for i, name in enumerate(KCLASS):
+            ms, n = C.c_double(), C.c_longlong()
+            self._check(self._l.ptycho_profile_fetch(self._h, i, C.byref(ms), C.byref(n)))
+            out[name] = (ms.value, n.value)
+        return out
 
     def launch_count(self) -> int:
         return int(self._l.ptycho_launch_count(self._h))

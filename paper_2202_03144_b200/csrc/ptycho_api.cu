@@ -62,6 +62,13 @@ struct ptycho_ctx {
     bool psi_valid = false;
     long long launches = 0;
     std::string err;
+    // per-kernel-class CUDA-event timing (ptycho_profile): (class, start, stop) of every launch
+    bool prof = false;
+    struct ProfEv { int cls; cudaEvent_t a, b; };
+    std::vector<ProfEv> prof_ev;
+    double prof_ms[PTYCHO_KCLASS_COUNT] = {};
+    long long prof_n[PTYCHO_KCLASS_COUNT] = {};
+    ~ptycho_ctx() { for (auto& e : prof_ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); } }
 };
 
 namespace {
@@ -79,6 +86,19 @@ ptycho_status fail(ptycho_ctx* c, ptycho_status s, const char* msg) {
     if (c) c->err = msg;
     return s;
 }
+
+// Brackets one launch with events when profiling is on; counts it either way.
+struct Timed {
+    ptycho_ctx* c; int cls; cudaEvent_t a = nullptr, b = nullptr;
+    Timed(ptycho_ctx* c_, int cls_) : c(c_), cls(cls_) {
+        if (c->prof) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, c->stream); }
+    }
+    ~Timed() {
+        ++c->launches;
+        if (c->prof) { cudaEventRecord(b, c->stream); c->prof_ev.push_back({cls, a, b}); }
+    }
+};
+#define LAUNCH(c, cls, ...) do { Timed t_(c, cls); __VA_ARGS__; } while (0)
 
 bool valid_n(int n) { return n == 64 || n == 128 || n == 256 || n == 512; }
 
@@ -179,20 +199,23 @@ template <int N> void launch_passes(ptycho_ctx* c, const FrameArgs& a, int nfram
     const dim3 grid(G::NCB, nframes), blk(kThreads);
     const size_t sr = G::smem_rows, scs = G::smem_cols(c->K);
     cudaStream_t s = c->stream;
-    if (fwd == RF_EXIT) k_rows_fwd<N, RF_EXIT><<<grid, blk, sr, s>>>(a);
-    else if (fwd == RF_DM) k_rows_fwd<N, RF_DM><<<grid, blk, sr, s>>>(a);
-    else if (fwd == RF_PLAIN) k_rows_fwd<N, RF_PLAIN><<<grid, blk, sr, s>>>(a);
-    if (fwd >= 0) ++c->launches;
-    if (col == CM_FULL) k_cols<N, CM_FULL><<<grid, blk, scs, s>>>(a);
-    else if (col == CM_ERRONLY) k_cols<N, CM_ERRONLY><<<grid, blk, scs, s>>>(a);
-    else if (col == CM_PLAIN_FWD) k_cols<N, CM_PLAIN_FWD><<<grid, blk, scs, s>>>(a);
-    else if (col == CM_PLAIN_INV) k_cols<N, CM_PLAIN_INV><<<grid, blk, scs, s>>>(a);
-    if (col >= 0) ++c->launches;
-    if (inv == RI_MINIBATCH) k_rows_inv<N, RI_MINIBATCH><<<grid, blk, sr, s>>>(a);
-    else if (inv == RI_DM) k_rows_inv<N, RI_DM><<<grid, blk, sr, s>>>(a);
-    else if (inv == RI_REVISED) k_rows_inv<N, RI_REVISED><<<grid, blk, sr, s>>>(a);
-    else if (inv == RI_PLAIN) k_rows_inv<N, RI_PLAIN><<<grid, blk, sr, s>>>(a);
-    if (inv >= 0) ++c->launches;
+    if (fwd >= 0) LAUNCH(c, PTYCHO_K_ROWS_FWD, {
+        if (fwd == RF_EXIT) k_rows_fwd<N, RF_EXIT><<<grid, blk, sr, s>>>(a);
+        else if (fwd == RF_DM) k_rows_fwd<N, RF_DM><<<grid, blk, sr, s>>>(a);
+        else k_rows_fwd<N, RF_PLAIN><<<grid, blk, sr, s>>>(a);
+    });
+    if (col >= 0) LAUNCH(c, PTYCHO_K_COLS, {
+        if (col == CM_FULL) k_cols<N, CM_FULL><<<grid, blk, scs, s>>>(a);
+        else if (col == CM_ERRONLY) k_cols<N, CM_ERRONLY><<<grid, blk, scs, s>>>(a);
+        else if (col == CM_PLAIN_FWD) k_cols<N, CM_PLAIN_FWD><<<grid, blk, scs, s>>>(a);
+        else k_cols<N, CM_PLAIN_INV><<<grid, blk, scs, s>>>(a);
+    });
+    if (inv >= 0) LAUNCH(c, PTYCHO_K_ROWS_INV, {
+        if (inv == RI_MINIBATCH) k_rows_inv<N, RI_MINIBATCH><<<grid, blk, sr, s>>>(a);
+        else if (inv == RI_DM) k_rows_inv<N, RI_DM><<<grid, blk, sr, s>>>(a);
+        else if (inv == RI_REVISED) k_rows_inv<N, RI_REVISED><<<grid, blk, sr, s>>>(a);
+        else k_rows_inv<N, RI_PLAIN><<<grid, blk, sr, s>>>(a);
+    });
 }
 
 void passes(ptycho_ctx* c, const FrameArgs& a, int nframes, int fwd, int col, int inv) {
@@ -222,8 +245,7 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
     const int ncb = ncb_of(c->N);
     if (!c->psi_valid) {
         const dim3 g((unsigned)((knn + 255) / 256), c->J);
-        k_init_psi<<<g, 256, 0, c->stream>>>(c->psi, c->O, c->W, c->P, c->K, c->N, c->pos, c->dm_frames);
-        ++c->launches;
+        LAUNCH(c, PTYCHO_K_OTHER, (k_init_psi<<<g, 256, 0, c->stream>>>(c->psi, c->O, c->W, c->P, c->K, c->N, c->pos, c->dm_frames)));
         c->psi_valid = true;
     }
     for (int s0 = 0; s0 < c->J; s0 += c->chunk) {
@@ -235,9 +257,8 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         passes(c, a, nf, RF_DM, CM_FULL, RI_DM);
     }
     const int upd = c->t >= c->par.probe_start;
-    k_dm_blend<<<ew_blocks(HW), 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1);
-    k_dm_blend<<<ew_blocks(nn), 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd);
-    c->launches += 2;
+    LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(HW), 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1)));
+    LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(nn), 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd)));
     return PTYCHO_OK;
 }
 
@@ -248,8 +269,7 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
     const int nb = (int)c->mb_offsets.size() - 1;
     for (int b = 0; b < nb; ++b) {
         const int b0 = c->mb_offsets[b], b1 = c->mb_offsets[b + 1];
-        k_probe_max<<<1, 1024, 0, c->stream>>>(c->P, c->K, (int)nn, c->sc);
-        ++c->launches;
+        LAUNCH(c, PTYCHO_K_UPDATE, (k_probe_max<<<1, 1024, 0, c->stream>>>(c->P, c->K, (int)nn, c->sc)));
         for (int s0 = b0; s0 < b1; s0 += c->chunk) {
             const int nf = std::min(c->chunk, b1 - s0);
             FrameArgs a = base_args(c);
@@ -259,30 +279,25 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
         }
         const bool lsq = alg == PTYCHO_LSQML;
         const int gO = ew_blocks(HW), gP = ew_blocks(nn);
-        k_direction<<<gO, 256, 0, c->stream>>>(c->nO, c->dO, HW, 1, c->par.delta_obj, c->sc, 0, lsq ? c->partO : nullptr);
-        ++c->launches;
+        LAUNCH(c, PTYCHO_K_UPDATE, (k_direction<<<gO, 256, 0, c->stream>>>(c->nO, c->dO, HW, 1, c->par.delta_obj, c->sc, 0, lsq ? c->partO : nullptr)));
         if (upd) {
-            k_real_max<<<1, 1024, 0, c->stream>>>(c->dP, (int)nn, c->sc);
-            k_direction<<<gP, 256, 0, c->stream>>>(c->nP, c->dP, nn, c->K, c->par.delta_probe, c->sc, 1, lsq ? c->partP : nullptr);
-            c->launches += 2;
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_real_max<<<1, 1024, 0, c->stream>>>(c->dP, (int)nn, c->sc)));
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_direction<<<gP, 256, 0, c->stream>>>(c->nP, c->dP, nn, c->K, c->par.delta_probe, c->sc, 1, lsq ? c->partP : nullptr)));
         }
         double* step_slot = c->n_steps < kStepCap ? c->steps + 2 * c->n_steps : nullptr;
         if (lsq) {
             if (upd) {
-                k_lsq_cross<<<b1 - b0, 256, 0, c->stream>>>(c->O, c->nO, c->W, c->P, c->nP, c->K, c->N, c->pos,
-                                                             c->mb_frames + b0, c->partX);
-                ++c->launches;
+                LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_cross<<<b1 - b0, 256, 0, c->stream>>>(c->O, c->nO, c->W, c->P, c->nP, c->K, c->N, c->pos,
+                                                                                        c->mb_frames + b0, c->partX)));
             }
-            k_lsq_solve<<<1, 32, 0, c->stream>>>(c->partO, gO, c->partP, upd ? gP : 0, c->partX, upd ? b1 - b0 : 0,
-                                                  c->par.lsq_lambda, upd, c->sc, step_slot ? step_slot : c->scratch_d);
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_solve<<<1, 32, 0, c->stream>>>(c->partO, gO, c->partP, upd ? gP : 0, c->partX, upd ? b1 - b0 : 0,
+                                                                            c->par.lsq_lambda, upd, c->sc, step_slot ? step_slot : c->scratch_d)));
         } else {
-            k_set_steps<<<1, 1, 0, c->stream>>>(c->sc, c->par.alpha_obj, upd ? c->par.alpha_probe : 0.f, step_slot);
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_set_steps<<<1, 1, 0, c->stream>>>(c->sc, c->par.alpha_obj, upd ? c->par.alpha_probe : 0.f, step_slot)));
         }
-        ++c->launches;
         ++c->n_steps;
-        k_apply<<<gO, 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1);
-        k_apply<<<gP, 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd);
-        c->launches += 2;
+        LAUNCH(c, PTYCHO_K_UPDATE, (k_apply<<<gO, 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1)));
+        LAUNCH(c, PTYCHO_K_UPDATE, (k_apply<<<gP, 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd)));
     }
     c->psi_valid = false;
     return PTYCHO_OK;
@@ -450,8 +465,7 @@ ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
         ptycho_status st = alg == PTYCHO_DM ? dm_iteration(c) : minibatch_iteration(c, alg);
         if (st != PTYCHO_OK) return st;
         double* slot = c->err_hist + (c->t < kErrCap ? c->t : kErrCap - 1);
-        k_sum_error<<<1, 1024, 0, c->stream>>>(c->e_part, (size_t)c->J * ncb_of(c->N), c->sc, slot);
-        ++c->launches;
+        LAUNCH(c, PTYCHO_K_UPDATE, (k_sum_error<<<1, 1024, 0, c->stream>>>(c->e_part, (size_t)c->J * ncb_of(c->N), c->sc, slot)));
         ++c->t;
     }
     CU(cudaGetLastError());
@@ -513,8 +527,7 @@ ptycho_status ptycho_fetch_exit_waves(ptycho_ctx* c, const int32_t* idx, int cou
     for (int s0 = 0; s0 < count; s0 += c->chunk) {
         const int nf = std::min(c->chunk, count - s0);
         CU(cudaMemcpyAsync(c->tmp_idx, slots.data() + s0, nf * 4, cudaMemcpyHostToDevice, c->stream));
-        k_copy_frames<<<dim3(64, nf), 256, 0, c->stream>>>(c->S, c->psi, nullptr, c->tmp_idx, knn);
-        ++c->launches;
+        LAUNCH(c, PTYCHO_K_OTHER, (k_copy_frames<<<dim3(64, nf), 256, 0, c->stream>>>(c->S, c->psi, nullptr, c->tmp_idx, knn)));
         CU(cudaMemcpyAsync(out + (size_t)s0 * knn * 2, c->S, (size_t)nf * knn * 8, cudaMemcpyDefault, c->stream));
         CU(cudaStreamSynchronize(c->stream));
     }
@@ -527,8 +540,7 @@ ptycho_status ptycho_set_exit_waves(ptycho_ctx* c, const float* psi) {
     for (int j0 = 0; j0 < c->J; j0 += c->chunk) {
         const int nf = std::min(c->chunk, c->J - j0);
         CU(cudaMemcpyAsync(c->S, psi + (size_t)j0 * knn * 2, (size_t)nf * knn * 8, cudaMemcpyDefault, c->stream));
-        k_copy_frames<<<dim3(64, nf), 256, 0, c->stream>>>(c->psi, c->S, c->slot_of + j0, nullptr, knn);
-        ++c->launches;
+        LAUNCH(c, PTYCHO_K_OTHER, (k_copy_frames<<<dim3(64, nf), 256, 0, c->stream>>>(c->psi, c->S, c->slot_of + j0, nullptr, knn)));
     }
     CU(cudaStreamSynchronize(c->stream));
     c->psi_valid = true;
@@ -564,10 +576,32 @@ ptycho_status ptycho_eval_error(ptycho_ctx* c, double* out) {
         a.e_part = c->e_tmp + (size_t)s0 * ncb;
         passes(c, a, nf, RF_EXIT, CM_ERRONLY, -1);
     }
-    k_sum_error<<<1, 1024, 0, c->stream>>>(c->e_tmp, (size_t)c->J * ncb, c->sc, c->scratch_d);
-    ++c->launches;
+    LAUNCH(c, PTYCHO_K_OTHER, (k_sum_error<<<1, 1024, 0, c->stream>>>(c->e_tmp, (size_t)c->J * ncb, c->sc, c->scratch_d)));
     CU(cudaMemcpyAsync(out, c->scratch_d, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
+    return PTYCHO_OK;
+}
+
+ptycho_status ptycho_profile(ptycho_ctx* c, int enable) {
+    if (!c) return PTYCHO_EINVAL;
+    CU(cudaStreamSynchronize(c->stream));
+    for (auto& e : c->prof_ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    c->prof_ev.clear();
+    for (int i = 0; i < PTYCHO_KCLASS_COUNT; ++i) { c->prof_ms[i] = 0; c->prof_n[i] = 0; }
+    c->prof = enable != 0;
+    return PTYCHO_OK;
+}
+ptycho_status ptycho_profile_fetch(ptycho_ctx* c, int kclass, double* total_ms, long long* n_launches) {
+    if (!c || kclass < 0 || kclass >= PTYCHO_KCLASS_COUNT) return PTYCHO_EINVAL;
+    CU(cudaStreamSynchronize(c->stream));
+    for (auto& e : c->prof_ev) {                       // fold finished events into the totals
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, e.a, e.b) == cudaSuccess) { c->prof_ms[e.cls] += ms; ++c->prof_n[e.cls]; }
+        cudaEventDestroy(e.a); cudaEventDestroy(e.b);
+    }
+    c->prof_ev.clear();
+    if (total_ms) *total_ms = c->prof_ms[kclass];
+    if (n_launches) *n_launches = c->prof_n[kclass];
     return PTYCHO_OK;
 }
 

@@ -145,8 +145,9 @@ def model_intensity(obj, probe, pos, threads: int = 8, chunk: int = 64):
 
 def simulate(obj, probe, pos, peak, poisson_seed, dtype, threads: int = 8):
     """R19: scale the probe so the brightest noiseless pixel equals `peak`, then draw Poisson
-    counts (one child stream of `poisson_seed` per 64-frame chunk).  `peak=None`: noiseless
-    float32, no scaling (cfg0).  uint16: counts clipped to 65535 = mask sentinel (R11)."""
+    counts (one child stream of `poisson_seed` per 64-frame chunk, so the result does not depend
+    on the thread count).  `peak=None`: noiseless float32, no scaling (cfg0).  uint16: counts
+    clipped to 65535 = mask sentinel (R11)."""
     j, n = len(pos), probe.shape[-1]
     if peak is None:
         out = np.empty((j, n, n), np.float32)
@@ -157,26 +158,32 @@ def simulate(obj, probe, pos, peak, poisson_seed, dtype, threads: int = 8):
     probe = probe * np.sqrt(peak / mx)
     out = np.empty((j, n, n), dtype)
     seeds = np.random.SeedSequence(poisson_seed).spawn((j + 63) // 64)
-    nf_sum, nf_cnt = 0.0, 0
-    for s, lam in model_intensity(obj, probe, pos, threads):
+
+    def chunk(s):
+        lam = _model_chunk(obj, probe, pos[s:s + 64])
         cnt = np.random.default_rng(seeds[s // 64]).poisson(lam)
         if dtype == np.uint16:
             cnt = np.minimum(cnt, MASK_U16)
             ok = cnt < MASK_U16
         else:
             ok = np.ones(cnt.shape, bool)
-        nf_sum += float(np.sum((np.sqrt(cnt[ok]) - np.sqrt(lam[ok])) ** 2))
-        nf_cnt += int(ok.sum())
         out[s:s + len(lam)] = cnt
+        return float(np.sum((np.sqrt(cnt[ok]) - np.sqrt(lam[ok])) ** 2)), int(ok.sum())
+
+    with ThreadPoolExecutor(threads) as ex:
+        parts = list(ex.map(chunk, range(0, j, 64)))
+    nf_sum, nf_cnt = sum(p[0] for p in parts), sum(p[1] for p in parts)
     return probe, out, nf_sum / max(nf_cnt, 1)
 
 
 # ----------------------------------------------------------------------------- the configs
-def make_config(i: int, n_pos: int | None = None, threads: int = 8, scale: int = 1) -> Scan:
+def make_config(i: int, n_pos: int | None = None, threads: int = 8, scale: int = 1, replica: int = 0) -> Scan:
     """Config i of BASELINE.json / SURVEY.md 8(d).  `n_pos` truncates the scan (first n_pos
     positions of the same generator; used where the oracle cannot hold the full scan).
-    `scale` > 1 divides N, H and the probe radius (same recipe, reduced size, for CPU tests)."""
-    so, sj, sp = 1000 + i, 2000 + i, 3000 + i
+    `scale` > 1 divides N, H and the probe radius (same recipe, reduced size, for CPU tests).
+    `replica` r > 0 shifts every seed by 10*r: an independent scan of the same shape (bench.py
+    --gpus N runs one replica per GPU)."""
+    so, sj, sp = 1000 + i + 10 * replica, 2000 + i + 10 * replica, 3000 + i + 10 * replica
     s = scale
     if i == 0:
         n, h, alg, its = 64 // s, 192 // s, "DM", 10

@@ -149,7 +149,8 @@ typedef enum {
     PTYCHO_K_ROWS_INV = 2, /* a6-a9: inverse row FFTs, exit-wave update, overlap scatter-add     */
     PTYCHO_K_UPDATE = 3,   /* a10/a11: normalising updates, step solve, error sum                */
     PTYCHO_K_OTHER = 4,    /* initial exit waves, frame copies of fetch/set                      */
-    PTYCHO_KCLASS_COUNT = 5
+    PTYCHO_K_MEGA = 5,     /* a1-a9 of a whole DM iteration in one persistent kernel (dm_mega.cuh) */
+    PTYCHO_KCLASS_COUNT = 6
 } ptycho_kclass;
 ptycho_status ptycho_profile(ptycho_ctx *ctx, int enable);
 ptycho_status ptycho_profile_fetch(ptycho_ctx *ctx, int kclass, double *total_ms, long long *n_launches);

@@ -18,7 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_CSRC, "libptycho_b200.so")
 ALG = {"EPIE_MB": 0, "DM": 1, "LSQML": 2}
-KCLASS = ["rows_fwd", "cols", "rows_inv", "update", "other"]   # ptycho_kclass
+KCLASS = ["rows_fwd", "cols", "rows_inv", "update", "other", "mega"]   # ptycho_kclass
 STATUS = ["OK", "EINVAL", "EBOUNDS", "EUNSUPPORTED", "ENOMEM", "ECUDA", "ESTATE"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "128"]
@@ -40,7 +40,7 @@ class Params(C.Structure):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """nvcc the CUDA library in-tree for sm_100a (cross-compiles without a GPU)."""
-    srcs = [os.path.join(_CSRC, f) for f in ("ptycho_api.cu", "kernels.cuh", "fft_core.cuh")]
+    srcs = [os.path.join(_CSRC, f) for f in ("ptycho_api.cu", "kernels.cuh", "fft_core.cuh", "dm_mega.cuh")]
     srcs.append(os.path.join(os.path.dirname(_HERE), "include", "ptycho_b200.h"))
     if not force and os.path.exists(LIB_PATH) and all(os.path.getmtime(LIB_PATH) >= os.path.getmtime(s) for s in srcs):
         return LIB_PATH

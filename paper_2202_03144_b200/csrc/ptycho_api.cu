@@ -16,6 +16,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "dm_mega.cuh"
 
 using namespace ptycho;
 
@@ -54,6 +55,9 @@ struct ptycho_ctx {
     const void* I = nullptr;
     // host state
     int chunk = 1;
+    // DM megakernel (dm_mega.cuh): frames per wave, wave lag between passes, ring slots, grid
+    int mega_M = 0, mega_D = 0, mega_R = 0, mega_grid = 0;
+    int* mega_ctr = nullptr;                   // device: [head | pad to 64 ints | cnt1[J] | cnt2[J] | cnt3[J]]
     std::vector<int> dm_order;                 // slot -> caller frame
     std::vector<int> slot_of_h;                // caller frame -> slot
     std::vector<int> mb_offsets;               // batch b = mb_frames[mb_offsets[b] .. mb_offsets[b+1])
@@ -110,6 +114,19 @@ int chunk_frames(int n, int K, int J) {
     return (int)std::max<long long>(1, std::min<long long>(c, J));
 }
 
+int env_int(const char* name, int dflt) {
+    const char* e = getenv(name);
+    return (e && *e) ? atoi(e) : dflt;
+}
+// DM megakernel parameters (single-mode DM only): M frames per wave, D waves of lag, ring R.
+void mega_config(ptycho_ctx* c) {
+    c->mega_M = c->mega_D = c->mega_R = 0;
+    if (c->K != 1 || c->par.disable_dm || !env_int("PTYCHO_MEGA", 1)) return;
+    c->mega_M = std::max(1, std::min(env_int("PTYCHO_MEGA_M", 4), c->J));
+    c->mega_D = std::max(1, env_int("PTYCHO_MEGA_D", 4));
+    c->mega_R = (2 * c->mega_D + 1) * c->mega_M;
+}
+
 size_t cols_smem(int n, int K) {
     switch (n) {
         case 64: return Geo<64>::smem_cols(K);
@@ -130,7 +147,8 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
     c->dO = w.take<float>(HW);
     c->nP = w.take<float2>(knn);
     c->dP = w.take<float>(nn);
-    c->S = w.take<float2>((size_t)c->chunk * knn);
+    c->S = w.take<float2>((size_t)std::max(c->chunk, c->mega_R) * knn);
+    c->mega_ctr = w.take<int>(64 + 3 * (size_t)c->J);
     c->e_part = w.take<float>((size_t)c->J * ncb_of(c->N));
     c->e_tmp = w.take<float>((size_t)c->J * ncb_of(c->N));
     c->tw = w.take<float2>(c->N);
@@ -172,6 +190,12 @@ template <int N> ptycho_status set_attrs(ptycho_ctx* c) {
     CU(cudaFuncSetAttribute(k_cols<N, CM_ERRONLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
     CU(cudaFuncSetAttribute(k_cols<N, CM_PLAIN_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
     CU(cudaFuncSetAttribute(k_cols<N, CM_PLAIN_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
+    CU(cudaFuncSetAttribute(k_dm_mega<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
+    int per_sm = 0, dev = 0, sms = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_dm_mega<N>, kThreads, MegaGeo<N>::smem));
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    c->mega_grid = std::max(1, per_sm) * sms;
     return PTYCHO_OK;
 }
 
@@ -248,6 +272,26 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         LAUNCH(c, PTYCHO_K_OTHER, (k_init_psi<<<g, 256, 0, c->stream>>>(c->psi, c->O, c->W, c->P, c->K, c->N, c->pos, c->dm_frames)));
         c->psi_valid = true;
     }
+    const int upd = c->t >= c->par.probe_start;
+    if (c->mega_M > 0) {
+        MegaArgs m{};
+        m.f = base_args(c);
+        m.f.psi = c->psi; m.f.frames = c->dm_frames; m.f.e_part = c->e_part;
+        m.J = c->J; m.M = c->mega_M; m.D = c->mega_D; m.R = c->mega_R; m.nW = (c->J + m.M - 1) / m.M;
+        m.update_probe = upd;
+        m.head = c->mega_ctr; m.cnt1 = c->mega_ctr + 64; m.cnt2 = m.cnt1 + c->J; m.cnt3 = m.cnt2 + c->J;
+        CU(cudaMemsetAsync(c->mega_ctr, 0, sizeof(int) * (64 + 3 * (size_t)c->J), c->stream));
+        const long long items = (long long)(m.nW + 2 * m.D) * 3 * ncb;
+        const int grid = (int)std::min<long long>(items, c->mega_grid);
+        LAUNCH(c, PTYCHO_K_MEGA, {
+            switch (c->N) {
+                case 64: k_dm_mega<64><<<grid, kThreads, MegaGeo<64>::smem, c->stream>>>(m); break;
+                case 128: k_dm_mega<128><<<grid, kThreads, MegaGeo<128>::smem, c->stream>>>(m); break;
+                case 256: k_dm_mega<256><<<grid, kThreads, MegaGeo<256>::smem, c->stream>>>(m); break;
+                default: k_dm_mega<512><<<grid, kThreads, MegaGeo<512>::smem, c->stream>>>(m); break;
+            }
+        });
+    } else
     for (int s0 = 0; s0 < c->J; s0 += c->chunk) {
         const int nf = std::min(c->chunk, c->J - s0);
         FrameArgs a = base_args(c);
@@ -256,7 +300,6 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         a.e_part = c->e_part + (size_t)s0 * ncb;
         passes(c, a, nf, RF_DM, CM_FULL, RI_DM);
     }
-    const int upd = c->t >= c->par.probe_start;
     LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(HW), 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1)));
     LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(nn), 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd)));
     return PTYCHO_OK;
@@ -328,6 +371,7 @@ size_t ptycho_workspace_bytes(int obj_h, int obj_w, int n, int n_modes, int n_po
     tmp.H = obj_h; tmp.W = obj_w; tmp.N = n; tmp.K = n_modes; tmp.J = n_pos; tmp.itype = itype;
     if (params) tmp.par = *params; else ptycho_default_params(&tmp.par);
     tmp.chunk = chunk_frames(n, n_modes, n_pos);
+    mega_config(&tmp);
     return layout(&tmp, nullptr, intensities_on_host != 0);
 }
 
@@ -372,6 +416,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     c->H = obj_h; c->W = obj_w; c->N = n; c->K = n_modes; c->J = n_pos; c->itype = itype; c->par = par;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     c->chunk = chunk_frames(n, n_modes, n_pos);
+    mega_config(c);
     const bool dev_I = is_device_ptr(intensities);
     const size_t need = layout(c, nullptr, !dev_I);
     if (workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 255)) { delete c; return PTYCHO_ENOMEM; }

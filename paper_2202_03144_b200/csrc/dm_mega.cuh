@@ -54,6 +54,32 @@ __device__ __forceinline__ void slot_wait(const int* cnt, int target) {
     }
     __syncthreads();
 }
+// Warp-granular forms: the row passes keep every line inside one warp, so warps signal and wait on
+// their own and drift apart in phase (one warp's loads overlap another warp's butterflies).
+__device__ __forceinline__ void warp_signal(int* cnt) {
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) {
+        __threadfence();
+        asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(cnt) : "memory");
+    }
+}
+__device__ __forceinline__ void warp_wait(const int* cnt, int target) {
+    if ((threadIdx.x & 31) == 0) {
+        while (ld_acquire_gpu(cnt) < target) __nanosleep(64);
+    }
+    __syncwarp();
+}
+__device__ __forceinline__ float rsqrt_fast(float x) {
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float sqrt_fast(float x) {
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+constexpr int kWarps = kThreads / 32;
 
 template <int N> struct MegaGeo {
     using G = Geo<N>;
@@ -76,7 +102,6 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
     for (int i = 0; i < E; ++i) { accN[i] = make_float2(0.f, 0.f); accD[i] = 0.f; }
     const int s_end = min(m.J, (wave + 1) * m.M);
     for (int slot = wave * m.M; slot < s_end; ++slot) {
-        if (slot >= m.R) slot_wait(m.cnt3 + slot - m.R, G::NCB);          // ring slot free again
         const YX p0 = a.pos[a.frames[slot]];
         const float2* orow = a.O + (size_t)(p0.y + y) * a.W + p0.x;
         const float2* prow = a.psi + (size_t)slot * N * N + off;
@@ -94,11 +119,12 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
             }
             v[i] = make_float2(fmaf(2.f, po.x, -s.x), fmaf(2.f, po.y, -s.y));   // reflector
         }
-        fft_line_fwd<N>(v, t, sx, s_tw);
+        fft_line_fwd<N, true>(v, t, sx, s_tw);
+        if (slot >= m.R) warp_wait(m.cnt3 + slot - m.R, G::NCB * kWarps);  // ring slot free again
         float2* srow = a.S + (size_t)(slot % m.R) * N * N + off;
 #pragma unroll
         for (int r = 0; r < E; ++r) __stcg(srow + freq_b<N>(t, r), v[r]);
-        slot_signal(m.cnt1 + slot);
+        warp_signal(m.cnt1 + slot);
     }
     if (m.update_probe) {
 #pragma unroll
@@ -119,9 +145,9 @@ template <int N> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, i
     float2* sx = sm + c * G::LS_COL;
     const int col = blk * CB + c;
     constexpr float inv_n2 = 1.0f / ((float)N * (float)N);
+    constexpr float kAmp2Floor = 1e-30f;
     const int s_end = min(m.J, (wave + 1) * m.M);
     for (int slot = wave * m.M; slot < s_end; ++slot) {
-        slot_wait(m.cnt1 + slot, G::NCB);
         float2* base = a.S + (size_t)(slot % m.R) * N * N + col;
         const size_t ibase = (size_t)a.frames[slot] * N * N + col;
         float in[E];
@@ -133,6 +159,7 @@ template <int N> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, i
                 in[r] = u == 65535 ? -1.0f : (float)u;
             } else in[r] = __ldcs(reinterpret_cast<const float*>(a.I) + idx);
         }
+        warp_wait(m.cnt1 + slot, G::NCB * kWarps);
         float2 v[E];
 #pragma unroll
         for (int i = 0; i < E; ++i) v[i] = __ldcg(base + (size_t)(t + T * i) * N);
@@ -140,12 +167,14 @@ template <int N> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, i
         float err = 0.f;
 #pragma unroll
         for (int r = 0; r < E; ++r) {
-            const float a2 = v[r].x * v[r].x + v[r].y * v[r].y;
-            const float amp = sqrtf(a2);
+            const float a2 = fmaf(v[r].x, v[r].x, v[r].y * v[r].y);
+            const bool pos = a2 > kAmp2Floor;                               // R2: below this |Phi| counts as 0
+            const float ra = pos ? rsqrt_fast(a2) : 0.f;
+            const float amp = a2 * ra;
             if (in[r] >= 0.f) {
-                const float sq = sqrtf(in[r]), d = sq - amp;
+                const float sq = sqrt_fast(in[r]), d = sq - amp;
                 err = fmaf(d, d, err);
-                if (amp > 0.f) { const float sc = d / amp * inv_n2; v[r].x *= sc; v[r].y *= sc; }   // (s - 1)/N^2
+                if (pos) { const float sc = d * ra * inv_n2; v[r].x *= sc; v[r].y *= sc; }          // (s - 1)/N^2
                 else v[r] = make_float2(sq * inv_n2, 0.f);                  // R2: Phi' - Phi = sqrt(I)
             } else v[r] = make_float2(0.f, 0.f);                            // R3: masked, Phi' - Phi = 0
         }
@@ -176,7 +205,7 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
     const size_t off = (size_t)y * N;
     const int s_end = min(m.J, (wave + 1) * m.M);
     for (int slot = wave * m.M; slot < s_end; ++slot) {
-        slot_wait(m.cnt2 + slot, G::NCB);
+        warp_wait(m.cnt2 + slot, G::NCB);
         float keep = 1.f;                                                   // 1 - rb  (R6)
         if (a.pbound > 0.f) {
             float e = 0.f;
@@ -190,7 +219,7 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
         float2 v[E];
 #pragma unroll
         for (int r = 0; r < E; ++r) v[r] = __ldcg(srow + freq_b<N>(t, r));
-        fft_line_inv<N>(v, t, sx, s_tw + N);                                // v = F^-1[(s-1) Phi]
+        fft_line_inv<N, true>(v, t, sx, s_tw + N);                          // v = F^-1[(s-1) Phi]
         float2* prow = a.psi + (size_t)slot * N * N + off;
 #pragma unroll
         for (int r = 0; r < E; ++r) {
@@ -202,7 +231,7 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
             red_add(a.nO + obase + x, cmulc(w, p));                         // a8 conj(P) psi_j
             red_add(a.dO + obase + x, fmaf(p.x, p.x, p.y * p.y));
         }
-        slot_signal(m.cnt3 + slot);
+        warp_signal(m.cnt3 + slot);
     }
 }
 

@@ -96,7 +96,13 @@ template <int N> __device__ __forceinline__ constexpr int pos_a_inv(int b, int r
 // Forward line, A -> B.  v[a] = x[t + T*a] on entry (natural a); v[r] = X[freq_b(t, r)] on exit.
 // sx: this line's exchange region; tw[ka*T + b] = exp(-2 pi i b ka / N).  All threads of the CTA
 // must call (contains __syncthreads).
-template <int N> __device__ __forceinline__ void fft_line_fwd(float2 (&v)[FftCfg<N>::E], int t, float2* sx,
+template <bool WARP> __device__ __forceinline__ void line_sync() {
+    if (WARP) __syncwarp(); else __syncthreads();
+}
+
+// WARP = true: every line's T threads sit in one warp (row passes), so the exchange needs only a
+// warp barrier and warps run independently of one another.
+template <int N, bool WARP = false> __device__ __forceinline__ void fft_line_fwd(float2 (&v)[FftCfg<N>::E], int t, float2* sx,
                                                               const float2* __restrict__ tw) {
     constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T, LD = LineSmem<N>::LD;
     dft_reg<E, false>(v);
@@ -107,7 +113,7 @@ template <int N> __device__ __forceinline__ void fft_line_fwd(float2 (&v)[FftCfg
         if (ka) y = cmul(y, tw[ka * T + t]);
         sx[ka * LD + t] = y;
     }
-    __syncthreads();
+    line_sync<WARP>();
 #pragma unroll
     for (int m = 0; m < E / T; ++m) {
         float2 u[T];
@@ -122,7 +128,7 @@ template <int N> __device__ __forceinline__ void fft_line_fwd(float2 (&v)[FftCfg
 // Inverse line, B -> A (unnormalised).  v[r] = X[freq_b(t, r)] on entry; v[r] = x[pos_a_inv(t, r)]
 // on exit.  twi[b*E + ka] = exp(-2 pi i b ka / N) (same values as tw, transposed so that lanes,
 // which run along ka here, read consecutive words).  Contains __syncthreads.
-template <int N> __device__ __forceinline__ void fft_line_inv(float2 (&v)[FftCfg<N>::E], int t, float2* sx,
+template <int N, bool WARP = false> __device__ __forceinline__ void fft_line_inv(float2 (&v)[FftCfg<N>::E], int t, float2* sx,
                                                               const float2* __restrict__ twi) {
     constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T, LD = LineSmem<N>::LD;
 #pragma unroll
@@ -138,7 +144,7 @@ template <int N> __device__ __forceinline__ void fft_line_inv(float2 (&v)[FftCfg
             sx[ka * LD + b] = b ? cmulc(u[i], twi[b * E + ka]) : u[i];
         }
     }
-    __syncthreads();
+    line_sync<WARP>();
 #pragma unroll
     for (int ka = 0; ka < E; ++ka) v[ka] = sx[ka * LD + t];
     dft_reg<E, true>(v);

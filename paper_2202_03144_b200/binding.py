@@ -16,7 +16,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
-LIB_PATH = os.path.join(_CSRC, "libptycho_b200.so")
+LIB_PATH = os.environ.get("PTYCHO_B200_LIB") or os.path.join(_CSRC, "libptycho_b200.so")   # override: a debug build
 ALG = {"EPIE_MB": 0, "DM": 1, "LSQML": 2}
 KCLASS = ["rows_fwd", "cols", "rows_inv", "update", "other", "mega"]   # ptycho_kclass
 STATUS = ["OK", "EINVAL", "EBOUNDS", "EUNSUPPORTED", "ENOMEM", "ECUDA", "ESTATE"]

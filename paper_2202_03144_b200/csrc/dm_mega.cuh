@@ -29,6 +29,9 @@ struct MegaArgs {
     FrameArgs f;        // psi = slot 0 of the store; S = ring base; frames = slot -> caller frame; e_part [J][NCB]
     int J, M, D, R, nW;
     int update_probe;   // accumulate the lagged probe sums (a9) in pass 1
+    int flags;          // experiment switches: 1 = no L2 prefetch, 4 = immediate signals
+    const void* It;     // intensities re-tiled at init into pass-2 register order (k_tile_intensity)
+    const YX* spos;     // [J] position of each SLOT (pos[frames[slot]], one load instead of two chained)
     int* head;          // queue head
     int* cnt1;          // [J] pass-1 blocks done per slot
     int* cnt2;          // [J] pass-2 blocks done
@@ -75,6 +78,21 @@ __device__ __forceinline__ void warp_wait(const int* cnt, int target) {
     }
     __syncwarp();
 }
+// HBM -> L2 ahead of use (no register or shared-memory cost); bytes is a multiple of 16.
+__device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void l2_prefetch(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// A signal is sent one slot LATE (after the next slot's butterflies): by then the stores it covers
+// have landed and the release fence (MEMBAR.GPU) does not stall the warp (ncu: 1.8 warps per issue
+// were sitting in that fence).
+struct Deferred {
+    int* cnt = nullptr;
+    __device__ __forceinline__ void flush_warp() { if (cnt) { warp_signal(cnt); cnt = nullptr; } }
+    __device__ __forceinline__ void flush_cta_after_barrier() {   // caller: a CTA barrier has passed since the stores
+        if (cnt) { if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(cnt) : "memory"); cnt = nullptr; }
+    }
+};
 __device__ __forceinline__ float rsqrt_fast(float x) {
     float r;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
@@ -85,7 +103,51 @@ __device__ __forceinline__ float sqrt_fast(float x) {
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
 }
+#ifndef PTYCHO_MEGA_OCC
+#define PTYCHO_MEGA_OCC 2      // resident CTAs per SM the register budget is sized for (N < 512)
+#endif
 constexpr int kWarps = kThreads / 32;
+
+// Software phase profile (debug builds only, -DPTYCHO_PHASE_PROF): cycles per warp spent in each
+// phase of each pass, summed over lane 0 of every warp.  [pass 0..2][wait, load, compute, store] + [12] = item fetch
+#ifdef PTYCHO_PHASE_PROF
+__device__ unsigned long long g_phase[16];
+__shared__ unsigned long long s_phase[16];     // per CTA; flushed to g_phase when the kernel ends
+struct PhaseClock {
+    long long t; int base;
+    __device__ __forceinline__ void start(int pass) { base = 4 * pass; t = clock64(); }
+    __device__ __forceinline__ void lap(int phase) {
+        const long long n = clock64();
+        if ((threadIdx.x & 31) == 0) atomicAdd(&s_phase[base + phase], (unsigned long long)(n - t));
+        t = n;
+    }
+};
+#define PHASE_TOUCH(x) do { if ((x) == 1.2345e-33f) atomicAdd(&g_phase[15], 1ull); } while (0)
+#else
+struct PhaseClock {
+    __device__ __forceinline__ void start(int) {}
+    __device__ __forceinline__ void lap(int) {}
+};
+#define PHASE_TOUCH(x) do { } while (0)
+#endif
+
+// Init-time re-tiling of the intensities for pass 2 (run once).  The caller's
+// row-major frames make a column block a 32-byte piece every 2 N bytes of DRAM (measured: those
+// loads alone cost 3 ms of a 12 ms iteration); here the N x LPB block of (slot, blk) becomes one
+// contiguous piece, ordered so that thread tid of pass 2 reads its E values as 16-byte chunks:
+//   element (tid, r)  ->  chunk (r / EPC) * kThreads + tid, position r % EPC     (EPC = 16 / sizeof(T_I))
+// with value I[frames[slot]][row = freq_b(t, r)][col = blk * LPB + c], c = tid % LPB, t = tid / LPB.
+template <int N, typename TI> __global__ void __launch_bounds__(kThreads) k_tile_intensity(TI* __restrict__ out, const TI* __restrict__ I,
+                                                                                            const int* __restrict__ frames) {
+    using G = Geo<N>;
+    constexpr int E = G::E, CB = G::LPB, EPC = 16 / (int)sizeof(TI);
+    const int slot = blockIdx.y, blk = blockIdx.x, tid = threadIdx.x;
+    const int c = tid % CB, t = tid / CB;
+    const TI* src = I + (size_t)frames[slot] * N * N + blk * CB + c;
+    TI* dst = out + ((size_t)slot * G::NCB + blk) * N * CB;
+#pragma unroll
+    for (int r = 0; r < E; ++r) dst[((size_t)(r / EPC) * kThreads + tid) * EPC + r % EPC] = src[(size_t)freq_b<N>(t, r) * N];
+}
 
 template <int N> struct MegaGeo {
     using G = Geo<N>;
@@ -94,11 +156,12 @@ template <int N> struct MegaGeo {
 };
 
 // ---- pass 1: a1 exit wave, a2 reflector, a9 lagged probe sums, a3 forward row FFTs -> S --------
-template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, int blk, int wave, float2* sm, const float2* s_tw) {
+template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, int blk, int wave, float2* sm, const float2* s_tw,
+                                                            Deferred& df) {
     using G = Geo<N>;
-    constexpr int E = G::E, T = G::T;
+    constexpr int E = G::E, T = G::T, LW = 32 / T;
     const FrameArgs& a = m.f;
-    const int l = threadIdx.x / T, t = threadIdx.x % T;
+    const int l = threadIdx.x / T, t = threadIdx.x % T, lane = threadIdx.x & 31;
     float2* sx = sm + l * G::LS_ROW;
     const int y = blk * G::LPB + l;
     const size_t off = (size_t)y * N;
@@ -106,14 +169,25 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
     float accD[E];
 #pragma unroll
     for (int i = 0; i < E; ++i) { accN[i] = make_float2(0.f, 0.f); accD[i] = 0.f; }
-    const int s_end = min(m.J, (wave + 1) * m.M);
-    for (int slot = wave * m.M; slot < s_end; ++slot) {
-        const YX p0 = a.pos[a.frames[slot]];
+    const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
+    {   // psi of the NEXT wave's slots (this warp's lines): start HBM -> L2 now
+        const int s = s_begin + m.M + lane;
+        if (!(m.flags & 1) && lane < m.M && s < m.J)
+            l2_prefetch_bulk(a.psi + (size_t)s * N * N + (size_t)(blk * G::LPB + (threadIdx.x >> 5) * LW) * N, LW * N * 8);
+    }
+    PhaseClock pc;
+    for (int slot = s_begin; slot < s_end; ++slot) {
+        pc.start(0);
+        if (slot >= m.R) warp_wait(m.cnt3 + slot - m.R, G::NCB * kWarps);    // ring slot free again
+        pc.lap(0);
+        const YX p0 = m.spos[slot];
         const float2* orow = a.O + (size_t)(p0.y + y) * a.W + p0.x;
         const float2* prow = a.psi + (size_t)slot * N * N + off;
         float2 v[E];
 #pragma unroll
-        for (int i = 0; i < E; ++i) v[i] = __ldcs(prow + t + T * i);      // psi_j: streamed from HBM once
+        for (int i = 0; i < E; ++i) v[i] = __ldcs(prow + t + T * i);      // psi_j: streamed once
+        PHASE_TOUCH(v[E - 1].x);
+        pc.lap(1);
 #pragma unroll
         for (int i = 0; i < E; ++i) {
             const float2 o = __ldg(orow + t + T * i);
@@ -126,11 +200,15 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
             v[i] = make_float2(fmaf(2.f, po.x, -s.x), fmaf(2.f, po.y, -s.y));   // reflector
         }
         fft_line_fwd<N, true>(v, t, sx, s_tw);
-        if (slot >= m.R) warp_wait(m.cnt3 + slot - m.R, G::NCB * kWarps);  // ring slot free again
+        __syncwarp();                                                       // sx is free for the next slot
+        pc.lap(2);
+        df.flush_warp();                                                    // previous slot's signal
         float2* srow = a.S + (size_t)(slot % m.R) * N * N + off;
 #pragma unroll
         for (int r = 0; r < E; ++r) __stcg(srow + freq_b<N>(t, r), v[r]);
-        warp_signal(m.cnt1 + slot);
+        df.cnt = m.cnt1 + slot;
+        if (m.flags & 4) df.flush_warp();
+        pc.lap(3);
     }
     if (m.update_probe) {
 #pragma unroll
@@ -143,7 +221,7 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
 
 // ---- pass 2: a3 column FFTs, a4 error partial, a5 modulus projection (as s - 1), a6 inverse columns
 template <int N> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, int blk, int wave, float2* sm, const float2* s_tw,
-                                                            float* s_red) {
+                                                            float* s_red, Deferred& df) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T, CB = G::LPB;
     const FrameArgs& a = m.f;
@@ -152,24 +230,48 @@ template <int N> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, i
     const int col = blk * CB + c;
     constexpr float inv_n2 = 1.0f / ((float)N * (float)N);
     constexpr float kAmp2Floor = 1e-30f;
-    const int s_end = min(m.J, (wave + 1) * m.M);
-    for (int slot = wave * m.M; slot < s_end; ++slot) {
-        float2* base = a.S + (size_t)(slot % m.R) * N * N + col;
-        const size_t ibase = (size_t)a.frames[slot] * N * N + col;
-        float in[E];
-#pragma unroll
-        for (int r = 0; r < E; ++r) {                                       // I_j: streamed from HBM once
-            const size_t idx = ibase + (size_t)freq_b<N>(t, r) * N;
-            if (a.itype == 1) {
-                const unsigned short u = __ldcs(reinterpret_cast<const unsigned short*>(a.I) + idx);
-                in[r] = u == 65535 ? -1.0f : (float)u;
-            } else in[r] = __ldcs(reinterpret_cast<const float*>(a.I) + idx);
-        }
+    const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
+    const size_t tile_bytes = (size_t)N * CB * (a.itype == 1 ? 2 : 4);   // this block's intensities of one slot: contiguous
+    if (!(m.flags & 1) && threadIdx.x < m.M) {                              // I of the NEXT wave: HBM -> L2 now
+        const int s = s_begin + m.M + threadIdx.x;
+        if (s < m.J) l2_prefetch_bulk(reinterpret_cast<const char*>(m.It) + ((size_t)s * G::NCB + blk) * tile_bytes, (uint32_t)tile_bytes);
+    }
+    PhaseClock pc;
+    for (int slot = s_begin; slot < s_end; ++slot) {
+        pc.start(1);
         warp_wait(m.cnt1 + slot, G::NCB * kWarps);
+        pc.lap(0);
+        float2* base = a.S + (size_t)(slot % m.R) * N * N + col;
         float2 v[E];
 #pragma unroll
         for (int i = 0; i < E; ++i) v[i] = __ldcg(base + (size_t)(t + T * i) * N);
-        fft_line_fwd<N>(v, t, sx, s_tw);
+        float in[E];                                                        // I_j: streamed once, 16-byte loads
+        {
+            const uint4* it = reinterpret_cast<const uint4*>(reinterpret_cast<const char*>(m.It) + ((size_t)slot * G::NCB + blk) * tile_bytes) + threadIdx.x;
+            if (a.itype == 1) {
+#pragma unroll
+                for (int j = 0; j < E / 8; ++j) {
+                    const uint4 q = __ldcs(it + j * kThreads);
+                    const unsigned w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const unsigned lo = w[k] & 0xffffu, hi = w[k] >> 16;
+                        in[8 * j + 2 * k] = lo == 65535u ? -1.0f : (float)lo;
+                        in[8 * j + 2 * k + 1] = hi == 65535u ? -1.0f : (float)hi;
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < E / 4; ++j) {
+                    const float4 q = __ldcs(reinterpret_cast<const float4*>(it) + j * kThreads);
+                    in[4 * j] = q.x; in[4 * j + 1] = q.y; in[4 * j + 2] = q.z; in[4 * j + 3] = q.w;
+                }
+            }
+        }
+        PHASE_TOUCH(v[E - 1].x + in[E - 1]);
+        pc.lap(1);
+        fft_line_fwd<N>(v, t, sx, s_tw);                                    // (CTA barrier inside)
+        df.flush_cta_after_barrier();                                       // previous slot's signal
         float err = 0.f;
 #pragma unroll
         for (int r = 0; r < E; ++r) {
@@ -194,14 +296,19 @@ template <int N> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, i
             for (int w = 0; w < kThreads / 32; ++w) tot += s_red[w];        // fixed order
             a.e_part[(size_t)slot * G::NCB + blk] = tot;
         }
+        pc.lap(2);
 #pragma unroll
         for (int r = 0; r < E; ++r) __stcg(base + (size_t)pos_a_inv<N>(t, r) * N, v[r]);
-        slot_signal(m.cnt2 + slot);
+        __syncthreads();                                                    // sx and s_red free; stores issued by all
+        df.cnt = m.cnt2 + slot;
+        if (m.flags & 4) df.flush_cta_after_barrier();
+        pc.lap(3);
     }
 }
 
 // ---- pass 3: a6 inverse row FFTs, a7 exit-wave update, a8 object scatter-add ---------------------
-template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, int blk, int wave, float2* sm, const float2* s_tw) {
+template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, int blk, int wave, float2* sm, const float2* s_tw,
+                                                            Deferred& df) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T;
     const FrameArgs& a = m.f;
@@ -209,9 +316,17 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
     float2* sx = sm + l * G::LS_ROW;
     const int y = blk * G::LPB + l;
     const size_t off = (size_t)y * N;
-    const int s_end = min(m.J, (wave + 1) * m.M);
-    for (int slot = wave * m.M; slot < s_end; ++slot) {
+    const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
+    PhaseClock pc;
+    for (int slot = s_begin; slot < s_end; ++slot) {
+        pc.start(2);
         warp_wait(m.cnt2 + slot, G::NCB);
+        pc.lap(0);
+        const float2* srow = a.S + (size_t)(slot % m.R) * N * N + off;
+        float2 v[E];
+#pragma unroll
+        for (int r = 0; r < E; ++r) v[r] = __ldcg(srow + freq_b<N>(t, r));
+        const YX p0 = m.spos[slot];
         float keep = 1.f;                                                   // 1 - rb  (R6)
         if (a.pbound > 0.f) {
             float e = 0.f;
@@ -219,13 +334,13 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
             e *= 1.0f / ((float)N * (float)N);
             keep = (e <= a.pbound) ? 0.f : 1.f - sqrtf(a.pbound / e);
         }
-        const YX p0 = a.pos[a.frames[slot]];
         const size_t obase = (size_t)(p0.y + y) * a.W + p0.x;
-        const float2* srow = a.S + (size_t)(slot % m.R) * N * N + off;
-        float2 v[E];
-#pragma unroll
-        for (int r = 0; r < E; ++r) v[r] = __ldcg(srow + freq_b<N>(t, r));
+        PHASE_TOUCH(v[E - 1].x + keep);
+        pc.lap(1);
         fft_line_inv<N, true>(v, t, sx, s_tw + N);                          // v = F^-1[(s-1) Phi]
+        __syncwarp();                                                       // sx is free for the next slot
+        pc.lap(2);
+        df.flush_warp();                                                    // previous slot's signal
         float2* prow = a.psi + (size_t)slot * N * N + off;
 #pragma unroll
         for (int r = 0; r < E; ++r) {
@@ -237,11 +352,13 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
             red_add(a.nO + obase + x, cmulc(w, p));                         // a8 conj(P) psi_j
             red_add(a.dO + obase + x, fmaf(p.x, p.x, p.y * p.y));
         }
-        warp_signal(m.cnt3 + slot);
+        df.cnt = m.cnt3 + slot;
+        if (m.flags & 4) df.flush_warp();
+        pc.lap(3);
     }
 }
 
-template <int N> __global__ void __launch_bounds__(kThreads, (N >= 512 ? 1 : 2)) k_dm_mega(MegaArgs m) {
+template <int N> __global__ void __launch_bounds__(kThreads, (N >= 512 ? 1 : PTYCHO_MEGA_OCC)) k_dm_mega(MegaArgs m) {
     using G = Geo<N>;
     extern __shared__ float2 sm[];
     float2* s_tw = sm + G::LPB * MegaGeo<N>::LINE;
@@ -250,20 +367,36 @@ template <int N> __global__ void __launch_bounds__(kThreads, (N >= 512 ? 1 : 2))
     load_tw(s_tw, m.f.tw, m.f.twi, N);
     const int per_qw = 3 * G::NCB;
     const int total = (m.nW + 2 * m.D) * per_qw;
+    Deferred df;
+    bool df_cta = false;                                      // the pending signal is a CTA-level one (pass 2)
+#ifdef PTYCHO_PHASE_PROF
+    if (threadIdx.x < 16) s_phase[threadIdx.x] = 0;
+    __syncthreads();
+#endif
+    PhaseClock pcf;
     for (;;) {
+        pcf.start(3);
         __syncthreads();
         if (threadIdx.x == 0) s_item = atomicAdd(m.head, 1);
         __syncthreads();
+        pcf.lap(0);
+        // the last slot's signal of the previous item: must go out before this item can block on a flag
+        if (df_cta) df.flush_cta_after_barrier(); else df.flush_warp();
         const int q = s_item;
         if (q >= total) break;
         const int qw = q / per_qw, idx = q % per_qw;
         const int kind = idx / G::NCB, blk = idx % G::NCB;    // 0: pass 3, 1: pass 2, 2: pass 1
         const int wave = qw - (2 - kind) * m.D;
         if (wave < 0 || wave >= m.nW) continue;
-        if (kind == 2) mega_pass1<N>(m, blk, wave, sm, s_tw);
-        else if (kind == 1) mega_pass2<N>(m, blk, wave, sm, s_tw, s_red);
-        else mega_pass3<N>(m, blk, wave, sm, s_tw);
+        df_cta = kind == 1;
+        if (kind == 2) mega_pass1<N>(m, blk, wave, sm, s_tw, df);
+        else if (kind == 1) mega_pass2<N>(m, blk, wave, sm, s_tw, s_red, df);
+        else mega_pass3<N>(m, blk, wave, sm, s_tw, df);
     }
+#ifdef PTYCHO_PHASE_PROF
+    __syncthreads();
+    if (threadIdx.x < 16) atomicAdd(&g_phase[threadIdx.x], s_phase[threadIdx.x]);
+#endif
 }
 
 }  // namespace ptycho

@@ -21,7 +21,10 @@ enum RowFwdMode { RF_EXIT = 0, RF_DM = 1, RF_PLAIN = 2 };
 enum ColMode { CM_FULL = 0, CM_ERRONLY = 1, CM_PLAIN_FWD = 2, CM_PLAIN_INV = 3 };
 enum RowInvMode { RI_MINIBATCH = 0, RI_DM = 1, RI_REVISED = 2, RI_PLAIN = 3 };
 
-constexpr int kThreads = 256;
+#ifndef PTYCHO_THREADS
+#define PTYCHO_THREADS 256
+#endif
+constexpr int kThreads = PTYCHO_THREADS;
 
 struct FrameArgs {
     const float2* __restrict__ O;   // object H x W

@@ -49,6 +49,8 @@ struct ptycho_ctx {
     float *dO = nullptr, *dP = nullptr, *e_part = nullptr, *e_tmp = nullptr;
     float2 *tw = nullptr, *twi = nullptr;
     YX* pos = nullptr;
+    void* It = nullptr;                        // intensities re-tiled for the DM megakernel
+    YX* spos = nullptr;                        // positions in DM slot order
     int *dm_frames = nullptr, *mb_frames = nullptr, *tmp_idx = nullptr, *slot_of = nullptr;
     Scalars* sc = nullptr;
     double *err_hist = nullptr, *steps = nullptr, *partO = nullptr, *partP = nullptr, *partX = nullptr, *scratch_d = nullptr;
@@ -119,12 +121,26 @@ int env_int(const char* name, int dflt) {
     return (e && *e) ? atoi(e) : dflt;
 }
 // DM megakernel parameters (single-mode DM only): M frames per wave, D waves of lag, ring R.
+int ncb_of(int n);
+// Queue geometry.  About grid / (3 NCB) queue waves are in flight at once; a pass-2 item must find its
+// pass-1 items finished, a pass-3 item its pass-2 items, and a pass-1 item the ring slot it overwrites
+// released, so the lag D and the ring slack X are a little more than that number (measured on cfg2:
+// D = X = 8 against D = 4, X = 0 is 9.3 ms against 12.4 ms), and M shrinks until the ring fits the L2 share.
 void mega_config(ptycho_ctx* c) {
     c->mega_M = c->mega_D = c->mega_R = 0;
     if (c->K != 1 || c->par.disable_dm || !env_int("PTYCHO_MEGA", 1)) return;
-    c->mega_M = std::max(1, std::min(env_int("PTYCHO_MEGA_M", 4), c->J));
-    c->mega_D = std::max(1, env_int("PTYCHO_MEGA_D", 4));
-    c->mega_R = (2 * c->mega_D + 1) * c->mega_M;
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) { int v = 0; if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v; }
+    cudaGetLastError();
+    const int grid = sms * (c->N >= 512 ? 1 : PTYCHO_MEGA_OCC);
+    const int inflight = (grid + 3 * ncb_of(c->N) - 1) / (3 * ncb_of(c->N));
+    c->mega_D = std::max(2, env_int("PTYCHO_MEGA_D", inflight + 2));
+    const int X = std::max(0, env_int("PTYCHO_MEGA_X", inflight + 2));
+    int M = std::max(1, std::min(env_int("PTYCHO_MEGA_M", 4), c->J));
+    const double ring_mb = env_int("PTYCHO_MEGA_RING_MB", 48);
+    while (M > 1 && (double)(2 * c->mega_D + 1 + X) * M * c->N * c->N * 8.0 > ring_mb * 1048576.0) --M;
+    c->mega_M = M;
+    c->mega_R = (2 * c->mega_D + 1 + X) * M;
 }
 
 size_t cols_smem(int n, int K) {
@@ -154,6 +170,7 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
     c->tw = w.take<float2>(c->N);
     c->twi = w.take<float2>(c->N);
     c->pos = w.take<YX>(c->J);
+    c->spos = w.take<YX>(c->J);
     c->dm_frames = w.take<int>(c->J);
     c->mb_frames = w.take<int>(c->J);
     c->tmp_idx = w.take<int>(c->J);
@@ -166,6 +183,7 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
     c->partX = w.take<double>(c->J);
     c->scratch_d = w.take<double>(kRedBlocks);
     if (!c->par.disable_dm) c->psi = w.take<float2>((size_t)c->J * knn);
+    if (c->mega_M > 0) c->It = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
     if (copy_I) c->I = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
     return (w.off + 255) & ~size_t(255);
 }
@@ -279,6 +297,9 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         m.f.psi = c->psi; m.f.frames = c->dm_frames; m.f.e_part = c->e_part;
         m.J = c->J; m.M = c->mega_M; m.D = c->mega_D; m.R = c->mega_R; m.nW = (c->J + m.M - 1) / m.M;
         m.update_probe = upd;
+        m.spos = c->spos;
+        m.It = c->It;
+        m.flags = env_int("PTYCHO_MEGA_FLAGS", 0);
         m.head = c->mega_ctr; m.cnt1 = c->mega_ctr + 64; m.cnt2 = m.cnt1 + c->J; m.cnt3 = m.cnt2 + c->J;
         CU(cudaMemsetAsync(c->mega_ctr, 0, sizeof(int) * (64 + 3 * (size_t)c->J), c->stream));
         const long long items = (long long)(m.nW + 2 * m.D) * 3 * ncb;
@@ -484,9 +505,20 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     }
     c->par.batch_order = nullptr;   // copied; the caller's pointer is not kept
     CUI(cudaMemcpyAsync(c->dm_frames, c->dm_order.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
+    std::vector<int32_t> spos(2 * (size_t)n_pos);
+    for (int sidx = 0; sidx < n_pos; ++sidx) { spos[2 * sidx] = pos[2 * c->dm_order[sidx]]; spos[2 * sidx + 1] = pos[2 * c->dm_order[sidx] + 1]; }
+    CUI(cudaMemcpyAsync(c->spos, spos.data(), spos.size() * 4, cudaMemcpyHostToDevice, s));
     CUI(cudaMemcpyAsync(c->mb_frames, mb.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
     CUI(cudaMemcpyAsync(c->slot_of, c->slot_of_h.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
 
+    if (c->mega_M > 0) {                                    // intensities in pass-2 tile order (dm_mega.cuh)
+        const dim3 g(ncb_of(n), n_pos);
+#define TILE_I(NN) do { if (itype == PTYCHO_I_U16) k_tile_intensity<NN, unsigned short><<<g, kThreads, 0, s>>>((unsigned short*)c->It, (const unsigned short*)c->I, c->dm_frames); \
+                        else k_tile_intensity<NN, float><<<g, kThreads, 0, s>>>((float*)c->It, (const float*)c->I, c->dm_frames); } while (0)
+        switch (n) { case 64: TILE_I(64); break; case 128: TILE_I(128); break; case 256: TILE_I(256); break; default: TILE_I(512); break; }
+#undef TILE_I
+        ++c->launches;
+    }
     // init-time constants on the device: eps_O, eps_P (R5), sum_I (C3)
     k_probe_max<<<1, 1024, 0, s>>>(c->P, c->K, (int)nn, c->sc);
     k_finish_init<<<1, 1, 0, s>>>(c->sc, par.delta_blend, n_pos, 0);
@@ -649,6 +681,17 @@ ptycho_status ptycho_profile_fetch(ptycho_ctx* c, int kclass, double* total_ms, 
     if (n_launches) *n_launches = c->prof_n[kclass];
     return PTYCHO_OK;
 }
+
+#ifdef PTYCHO_PHASE_PROF
+// debug builds only: copies and clears the phase-cycle counters of dm_mega.cuh
+int ptycho_debug_phase(unsigned long long* out16) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out16, ptycho::g_phase, 16 * sizeof(unsigned long long));
+    unsigned long long z[16] = {};
+    cudaMemcpyToSymbol(ptycho::g_phase, z, sizeof(z));
+    return 0;
+}
+#endif
 
 long long ptycho_launch_count(const ptycho_ctx* c) { return c ? c->launches : 0; }
 const char* ptycho_last_error(const ptycho_ctx* c) { return c ? c->err.c_str() : ""; }

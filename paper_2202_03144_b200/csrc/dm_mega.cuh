@@ -63,6 +63,7 @@ __device__ __forceinline__ void slot_wait(const int* cnt, int target) {
 // consumer polls with a relaxed load and then reads the producer's data only through ld.global.cg
 // (L2, the point of coherence); the producer orders its st.global.cg writes before the counter
 // increment with the release.  The poll's result is a control dependency of every later load.
+__device__ int g_nowait;   // debug: ignore the flags (racy; timing experiments only)
 __device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
     int v;
     asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -74,7 +75,7 @@ __device__ __forceinline__ void warp_signal(int* cnt) {
 }
 __device__ __forceinline__ void warp_wait(const int* cnt, int target) {
     if ((threadIdx.x & 31) == 0) {
-        while (ld_relaxed_gpu(cnt) < target) __nanosleep(64);
+        while (ld_relaxed_gpu(cnt) < target && !g_nowait) __nanosleep(64);
     }
     __syncwarp();
 }
@@ -152,7 +153,7 @@ template <int N, typename TI> __global__ void __launch_bounds__(kThreads) k_tile
 template <int N> struct MegaGeo {
     using G = Geo<N>;
     static constexpr int LINE = (G::LS_ROW > G::LS_COL ? G::LS_ROW : G::LS_COL);
-    static constexpr size_t smem = (size_t)(G::LPB * LINE + 2 * N) * sizeof(float2);
+    static constexpr size_t smem = (size_t)(G::LPB * LINE + 2 * N + G::LPB * N) * sizeof(float2);   // exchange, twiddles, probe rows
 };
 
 // ---- pass 1: a1 exit wave, a2 reflector, a9 lagged probe sums, a3 forward row FFTs -> S --------
@@ -170,6 +171,10 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
 #pragma unroll
     for (int i = 0; i < E; ++i) { accN[i] = make_float2(0.f, 0.f); accD[i] = 0.f; }
     const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
+    float2* sP = const_cast<float2*>(s_tw) + 2 * N + l * N;                                      // this line's probe row, kept for the M slots
+#pragma unroll
+    for (int i = 0; i < E; ++i) sP[t + T * i] = __ldg(a.P + off + t + T * i);
+    __syncwarp();
     {   // psi of the NEXT wave's slots (this warp's lines): start HBM -> L2 now
         const int s = s_begin + m.M + lane;
         if (!(m.flags & 1) && lane < m.M && s < m.J)
@@ -191,7 +196,7 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
 #pragma unroll
         for (int i = 0; i < E; ++i) {
             const float2 o = __ldg(orow + t + T * i);
-            const float2 po = cmul(__ldg(a.P + off + t + T * i), o);      // psi_O = P O_j
+            const float2 po = cmul(sP[t + T * i], o);                     // psi_O = P O_j
             const float2 s = v[i];
             if (m.update_probe) {
                 accN[i] = cadd(accN[i], cmulc(s, o));                     // conj(O_j) psi_j (lagged, R4)
@@ -317,6 +322,10 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
     const int y = blk * G::LPB + l;
     const size_t off = (size_t)y * N;
     const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
+    float2* sP = const_cast<float2*>(s_tw) + 2 * N + l * N;                                      // this line's probe row, kept for the M slots
+#pragma unroll
+    for (int i = 0; i < E; ++i) sP[t + T * i] = __ldg(a.P + off + t + T * i);
+    __syncwarp();
     PhaseClock pc;
     for (int slot = s_begin; slot < s_end; ++slot) {
         pc.start(2);
@@ -335,6 +344,9 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
             keep = (e <= a.pbound) ? 0.f : 1.f - sqrtf(a.pbound / e);
         }
         const size_t obase = (size_t)(p0.y + y) * a.W + p0.x;
+        float2 o[E];                                                        // O_j: in flight during the butterflies
+#pragma unroll
+        for (int r = 0; r < E; ++r) o[r] = __ldg(a.O + obase + pos_a_inv<N>(t, r));
         PHASE_TOUCH(v[E - 1].x + keep);
         pc.lap(1);
         fft_line_inv<N, true>(v, t, sx, s_tw + N);                          // v = F^-1[(s-1) Phi]
@@ -345,8 +357,8 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
 #pragma unroll
         for (int r = 0; r < E; ++r) {
             const int x = pos_a_inv<N>(t, r);
-            const float2 p = __ldg(a.P + off + x);
-            const float2 po = cmul(p, __ldg(a.O + obase + x));
+            const float2 p = sP[x];
+            const float2 po = cmul(p, o[r]);
             const float2 w = make_float2(fmaf(keep, v[r].x, po.x), fmaf(keep, v[r].y, po.y));   // a7
             __stcs(prow + x, w);
             red_add(a.nO + obase + x, cmulc(w, p));                         // a8 conj(P) psi_j
@@ -388,6 +400,7 @@ template <int N> __global__ void __launch_bounds__(kThreads, (N >= 512 ? 1 : PTY
         const int kind = idx / G::NCB, blk = idx % G::NCB;    // 0: pass 3, 1: pass 2, 2: pass 1
         const int wave = qw - (2 - kind) * m.D;
         if (wave < 0 || wave >= m.nW) continue;
+        if ((m.flags >> 8) & (1 << kind)) continue;               // debug: skip pass kinds (0x100 pass 3, 0x200 pass 2, 0x400 pass 1)
         df_cta = kind == 1;
         if (kind == 2) mega_pass1<N>(m, blk, wave, sm, s_tw, df);
         else if (kind == 1) mega_pass2<N>(m, blk, wave, sm, s_tw, s_red, df);

@@ -300,6 +300,7 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         m.spos = c->spos;
         m.It = c->It;
         m.flags = env_int("PTYCHO_MEGA_FLAGS", 0);
+        { int nw = (m.flags >> 8) ? 1 : 0; cudaMemcpyToSymbolAsync(g_nowait, &nw, sizeof(int), 0, cudaMemcpyHostToDevice, c->stream); }
         m.head = c->mega_ctr; m.cnt1 = c->mega_ctr + 64; m.cnt2 = m.cnt1 + c->J; m.cnt3 = m.cnt2 + c->J;
         CU(cudaMemsetAsync(c->mega_ctr, 0, sizeof(int) * (64 + 3 * (size_t)c->J), c->stream));
         const long long items = (long long)(m.nW + 2 * m.D) * 3 * ncb;

@@ -153,11 +153,11 @@ template <int N, typename TI> __global__ void __launch_bounds__(kThreads) k_tile
 template <int N> struct MegaGeo {
     using G = Geo<N>;
     static constexpr int LINE = (G::LS_ROW > G::LS_COL ? G::LS_ROW : G::LS_COL);
-    static constexpr size_t smem = (size_t)(G::LPB * LINE + 2 * N + G::LPB * N) * sizeof(float2);   // exchange, twiddles, probe rows
+    static constexpr size_t smem = (size_t)(G::LPB * LINE + 4 * N + G::LPB * N) * sizeof(float2);   // exchange, twiddles, probe rows
 };
 
 // ---- pass 1: a1 exit wave, a2 reflector, a9 lagged probe sums, a3 forward row FFTs -> S --------
-template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, int blk, int wave, float2* sm, const float2* s_tw,
+template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
                                                             Deferred& df) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T, LW = 32 / T;
@@ -166,12 +166,12 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
     float2* sx = sm + l * G::LS_ROW;
     const int y = blk * G::LPB + l;
     const size_t off = (size_t)y * N;
-    float2 accN[E];
+    float2 accN[E];                                                         // lagged probe sums of the M slots (R4)
     float accD[E];
 #pragma unroll
     for (int i = 0; i < E; ++i) { accN[i] = make_float2(0.f, 0.f); accD[i] = 0.f; }
     const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
-    float2* sP = const_cast<float2*>(s_tw) + 2 * N + l * N;                                      // this line's probe row, kept for the M slots
+    float2* sP = reinterpret_cast<float2*>(const_cast<float4*>(s_tw) + 2 * N) + l * N;   // this line's probe row, kept for the M slots
 #pragma unroll
     for (int i = 0; i < E; ++i) sP[t + T * i] = __ldg(a.P + off + t + T * i);
     __syncwarp();
@@ -225,7 +225,7 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
 }
 
 // ---- pass 2: a3 column FFTs, a4 error partial, a5 modulus projection (as s - 1), a6 inverse columns
-template <int N> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, int blk, int wave, float2* sm, const float2* s_tw,
+template <int N, bool U16> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
                                                             float* s_red, Deferred& df) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T, CB = G::LPB;
@@ -236,7 +236,7 @@ template <int N> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, i
     constexpr float inv_n2 = 1.0f / ((float)N * (float)N);
     constexpr float kAmp2Floor = 1e-30f;
     const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
-    const size_t tile_bytes = (size_t)N * CB * (a.itype == 1 ? 2 : 4);   // this block's intensities of one slot: contiguous
+    const size_t tile_bytes = (size_t)N * CB * (U16 ? 2 : 4);   // this block's intensities of one slot: contiguous
     if (!(m.flags & 1) && threadIdx.x < m.M) {                              // I of the NEXT wave: HBM -> L2 now
         const int s = s_begin + m.M + threadIdx.x;
         if (s < m.J) l2_prefetch_bulk(reinterpret_cast<const char*>(m.It) + ((size_t)s * G::NCB + blk) * tile_bytes, (uint32_t)tile_bytes);
@@ -250,30 +250,15 @@ template <int N> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, i
         float2 v[E];
 #pragma unroll
         for (int i = 0; i < E; ++i) v[i] = __ldcg(base + (size_t)(t + T * i) * N);
-        float in[E];                                                        // I_j: streamed once, 16-byte loads
+        // I_j: streamed once as 16-byte chunks, kept packed in registers until the projection
+        constexpr int NQ = U16 ? E / 8 : E / 4;
+        uint4 iq[NQ];
         {
             const uint4* it = reinterpret_cast<const uint4*>(reinterpret_cast<const char*>(m.It) + ((size_t)slot * G::NCB + blk) * tile_bytes) + threadIdx.x;
-            if (a.itype == 1) {
 #pragma unroll
-                for (int j = 0; j < E / 8; ++j) {
-                    const uint4 q = __ldcs(it + j * kThreads);
-                    const unsigned w[4] = {q.x, q.y, q.z, q.w};
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const unsigned lo = w[k] & 0xffffu, hi = w[k] >> 16;
-                        in[8 * j + 2 * k] = lo == 65535u ? -1.0f : (float)lo;
-                        in[8 * j + 2 * k + 1] = hi == 65535u ? -1.0f : (float)hi;
-                    }
-                }
-            } else {
-#pragma unroll
-                for (int j = 0; j < E / 4; ++j) {
-                    const float4 q = __ldcs(reinterpret_cast<const float4*>(it) + j * kThreads);
-                    in[4 * j] = q.x; in[4 * j + 1] = q.y; in[4 * j + 2] = q.z; in[4 * j + 3] = q.w;
-                }
-            }
+            for (int j = 0; j < NQ; ++j) iq[j] = __ldcs(it + j * kThreads);
         }
-        PHASE_TOUCH(v[E - 1].x + in[E - 1]);
+        PHASE_TOUCH(v[E - 1].x + __uint_as_float(iq[NQ - 1].w));
         pc.lap(1);
         fft_line_fwd<N>(v, t, sx, s_tw);                                    // (CTA barrier inside)
         df.flush_cta_after_barrier();                                       // previous slot's signal
@@ -284,8 +269,14 @@ template <int N> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, i
             const bool pos = a2 > kAmp2Floor;                               // R2: below this |Phi| counts as 0
             const float ra = pos ? rsqrt_fast(a2) : 0.f;
             const float amp = a2 * ra;
-            if (in[r] >= 0.f) {
-                const float sq = sqrt_fast(in[r]), d = sq - amp;
+            float inr;                                                      // R3: 65535 (u16) or a negative value = masked
+            if (U16) {
+                const unsigned w = (&iq[r / 8].x)[(r % 8) / 2];
+                const unsigned u = (r & 1) ? (w >> 16) : (w & 0xffffu);
+                inr = u == 65535u ? -1.0f : (float)u;
+            } else inr = __uint_as_float((&iq[r / 4].x)[r % 4]);
+            if (inr >= 0.f) {
+                const float sq = sqrt_fast(inr), d = sq - amp;
                 err = fmaf(d, d, err);
                 if (pos) { const float sc = d * ra * inv_n2; v[r].x *= sc; v[r].y *= sc; }          // (s - 1)/N^2
                 else v[r] = make_float2(sq * inv_n2, 0.f);                  // R2: Phi' - Phi = sqrt(I)
@@ -312,7 +303,7 @@ template <int N> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, i
 }
 
 // ---- pass 3: a6 inverse row FFTs, a7 exit-wave update, a8 object scatter-add ---------------------
-template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, int blk, int wave, float2* sm, const float2* s_tw,
+template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
                                                             Deferred& df) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T;
@@ -322,7 +313,7 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
     const int y = blk * G::LPB + l;
     const size_t off = (size_t)y * N;
     const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
-    float2* sP = const_cast<float2*>(s_tw) + 2 * N + l * N;                                      // this line's probe row, kept for the M slots
+    float2* sP = reinterpret_cast<float2*>(const_cast<float4*>(s_tw) + 2 * N) + l * N;                                      // this line's probe row, kept for the M slots
 #pragma unroll
     for (int i = 0; i < E; ++i) sP[t + T * i] = __ldg(a.P + off + t + T * i);
     __syncwarp();
@@ -370,10 +361,10 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
     }
 }
 
-template <int N> __global__ void __launch_bounds__(kThreads, (N >= 512 ? 1 : PTYCHO_MEGA_OCC)) k_dm_mega(MegaArgs m) {
+template <int N, bool U16> __global__ void __launch_bounds__(kThreads, (N >= 512 ? 1 : PTYCHO_MEGA_OCC)) k_dm_mega(MegaArgs m) {
     using G = Geo<N>;
-    extern __shared__ float2 sm[];
-    float2* s_tw = sm + G::LPB * MegaGeo<N>::LINE;
+    extern __shared__ __align__(16) float2 sm[];
+    float4* s_tw = reinterpret_cast<float4*>(sm + G::LPB * MegaGeo<N>::LINE);
     __shared__ float s_red[kThreads / 32];
     __shared__ int s_item;
     load_tw(s_tw, m.f.tw, m.f.twi, N);
@@ -403,7 +394,7 @@ template <int N> __global__ void __launch_bounds__(kThreads, (N >= 512 ? 1 : PTY
         if ((m.flags >> 8) & (1 << kind)) continue;               // debug: skip pass kinds (0x100 pass 3, 0x200 pass 2, 0x400 pass 1)
         df_cta = kind == 1;
         if (kind == 2) mega_pass1<N>(m, blk, wave, sm, s_tw, df);
-        else if (kind == 1) mega_pass2<N>(m, blk, wave, sm, s_tw, s_red, df);
+        else if (kind == 1) mega_pass2<N, U16>(m, blk, wave, sm, s_tw, s_red, df);
         else mega_pass3<N>(m, blk, wave, sm, s_tw, df);
     }
 #ifdef PTYCHO_PHASE_PROF

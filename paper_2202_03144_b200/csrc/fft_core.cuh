@@ -29,13 +29,28 @@ template <int R> __host__ __device__ constexpr int brev(int i) {
     return r;
 }
 
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
-    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+// Complex arithmetic on packed pairs.  sm_100a has two-wide fp32 instructions (FADD2 / FMUL2 / FFMA2,
+// PTX add/mul/fma.f32x2) whose operands can swap and negate their halves for free, so a complex add,
+// a rotation by +-i folded into an add, and each half of a complex multiply are ONE issue slot each.
+// The fp32 pipe rate is the same as for scalar code (measured: 127 against 125 lane-ops/clk/SM); what
+// halves is the number of instructions a warp has to issue, which is what bounds this kernel (ncu:
+// 40 % issue-active at 16 warps per SM, "wait" and "short scoreboard" stalls).
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {   // a * b
+    return __ffma2_rn(make_float2(a.y, a.x), make_float2(-b.y, b.y), __fmul2_rn(a, make_float2(b.x, b.x)));
 }
 __device__ __forceinline__ float2 cmulc(float2 a, float2 b) {  // a * conj(b)
-    return make_float2(fmaf(a.x, b.x, a.y * b.y), fmaf(a.y, b.x, -a.x * b.y));
+    return __ffma2_rn(make_float2(a.y, a.x), make_float2(b.y, -b.y), __fmul2_rn(a, make_float2(b.x, b.x)));
+}
+// Twiddle tables hold w = (c, s) as the four words {c, c, -s, s}: y * w and y * conj(w) are then one
+// FMUL2 and one FFMA2 with no register shuffling.
+__device__ __forceinline__ float4 tw_pack(float2 w) { return make_float4(w.x, w.x, -w.y, w.y); }
+__device__ __forceinline__ float2 cmul_tw(float2 y, float4 w) {
+    return __ffma2_rn(make_float2(y.y, y.x), make_float2(w.z, w.w), __fmul2_rn(y, make_float2(w.x, w.y)));
+}
+__device__ __forceinline__ float2 cmulc_tw(float2 y, float4 w) {
+    return __ffma2_rn(make_float2(y.y, y.x), make_float2(-w.z, -w.w), __fmul2_rn(y, make_float2(w.x, w.y)));
 }
 
 // cos(2 pi m / 32), sin(2 pi m / 32): literals so that unrolled butterflies get immediates.
@@ -52,12 +67,13 @@ __device__ __forceinline__ constexpr float sin32(int m) { return cos32(m - 8); }
 template <int R, bool INV> __device__ __forceinline__ float2 mul_root(float2 d, int m) {
     constexpr float h = 0.70710678118654752440f;
     if (m == 0) return d;
-    if (4 * m == R) return INV ? make_float2(-d.y, d.x) : make_float2(d.y, -d.x);
-    if (8 * m == R) return INV ? make_float2((d.x - d.y) * h, (d.x + d.y) * h) : make_float2((d.x + d.y) * h, (d.y - d.x) * h);
-    if (8 * m == 3 * R) return INV ? make_float2(-(d.x + d.y) * h, (d.x - d.y) * h) : make_float2((d.y - d.x) * h, -(d.x + d.y) * h);
+    if (4 * m == R) return INV ? make_float2(-d.y, d.x) : make_float2(d.y, -d.x);       // folds into the next add
+    if (8 * m == R)
+        return __fmul2_rn(__fadd2_rn(d, INV ? make_float2(-d.y, d.x) : make_float2(d.y, -d.x)), make_float2(h, h));
+    if (8 * m == 3 * R)
+        return __fmul2_rn(__fadd2_rn(make_float2(-d.x, -d.y), INV ? make_float2(-d.y, d.x) : make_float2(d.y, -d.x)), make_float2(h, h));
     const float c = cos32(m * (32 / R)), s = sin32(m * (32 / R));
-    return INV ? make_float2(fmaf(d.x, c, -d.y * s), fmaf(d.y, c, d.x * s))
-               : make_float2(fmaf(d.x, c, d.y * s), fmaf(d.y, c, -d.x * s));
+    return __ffma2_rn(make_float2(d.y, d.x), INV ? make_float2(-s, s) : make_float2(s, -s), __fmul2_rn(d, make_float2(c, c)));
 }
 
 // In-register R-point DFT (decimation in frequency).  In: v[n] natural.  Out: v[i] = Y[brev<R>(i)].
@@ -94,7 +110,7 @@ template <int N> __device__ __forceinline__ constexpr int pos_a_inv(int b, int r
 }
 
 // Forward line, A -> B.  v[a] = x[t + T*a] on entry (natural a); v[r] = X[freq_b(t, r)] on exit.
-// sx: this line's exchange region; tw[ka*T + b] = exp(-2 pi i b ka / N).  All threads of the CTA
+// sx: this line's exchange region; tw[ka*T + b] = tw_pack(exp(-2 pi i b ka / N)).  All threads of the CTA
 // must call (contains __syncthreads).
 template <bool WARP> __device__ __forceinline__ void line_sync() {
     if (WARP) __syncwarp(); else __syncthreads();
@@ -103,14 +119,14 @@ template <bool WARP> __device__ __forceinline__ void line_sync() {
 // WARP = true: every line's T threads sit in one warp (row passes), so the exchange needs only a
 // warp barrier and warps run independently of one another.
 template <int N, bool WARP = false> __device__ __forceinline__ void fft_line_fwd(float2 (&v)[FftCfg<N>::E], int t, float2* sx,
-                                                              const float2* __restrict__ tw) {
+                                                              const float4* __restrict__ tw) {
     constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T, LD = LineSmem<N>::LD;
     dft_reg<E, false>(v);
 #pragma unroll
     for (int i = 0; i < E; ++i) {
         const int ka = brev<E>(i);
         float2 y = v[i];
-        if (ka) y = cmul(y, tw[ka * T + t]);
+        if (ka) y = cmul_tw(y, tw[ka * T + t]);
         sx[ka * LD + t] = y;
     }
     line_sync<WARP>();
@@ -129,7 +145,7 @@ template <int N, bool WARP = false> __device__ __forceinline__ void fft_line_fwd
 // on exit.  twi[b*E + ka] = exp(-2 pi i b ka / N) (same values as tw, transposed so that lanes,
 // which run along ka here, read consecutive words).  Contains __syncthreads.
 template <int N, bool WARP = false> __device__ __forceinline__ void fft_line_inv(float2 (&v)[FftCfg<N>::E], int t, float2* sx,
-                                                              const float2* __restrict__ twi) {
+                                                              const float4* __restrict__ twi) {
     constexpr int E = FftCfg<N>::E, T = FftCfg<N>::T, LD = LineSmem<N>::LD;
 #pragma unroll
     for (int m = 0; m < E / T; ++m) {
@@ -141,7 +157,7 @@ template <int N, bool WARP = false> __device__ __forceinline__ void fft_line_inv
 #pragma unroll
         for (int i = 0; i < T; ++i) {
             const int b = brev<T>(i);
-            sx[ka * LD + b] = b ? cmulc(u[i], twi[b * E + ka]) : u[i];
+            sx[ka * LD + b] = b ? cmulc_tw(u[i], twi[b * E + ka]) : u[i];
         }
     }
     line_sync<WARP>();

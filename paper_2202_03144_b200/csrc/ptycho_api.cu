@@ -208,9 +208,10 @@ template <int N> ptycho_status set_attrs(ptycho_ctx* c) {
     CU(cudaFuncSetAttribute(k_cols<N, CM_ERRONLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
     CU(cudaFuncSetAttribute(k_cols<N, CM_PLAIN_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
     CU(cudaFuncSetAttribute(k_cols<N, CM_PLAIN_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
-    CU(cudaFuncSetAttribute(k_dm_mega<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
+    CU(cudaFuncSetAttribute(k_dm_mega<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
+    CU(cudaFuncSetAttribute(k_dm_mega<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
     int per_sm = 0, dev = 0, sms = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_dm_mega<N>, kThreads, MegaGeo<N>::smem));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_dm_mega<N, true>, kThreads, MegaGeo<N>::smem));
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     c->mega_grid = std::max(1, per_sm) * sms;
@@ -305,12 +306,13 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         CU(cudaMemsetAsync(c->mega_ctr, 0, sizeof(int) * (64 + 3 * (size_t)c->J), c->stream));
         const long long items = (long long)(m.nW + 2 * m.D) * 3 * ncb;
         const int grid = (int)std::min<long long>(items, c->mega_grid);
+        const bool u16 = c->itype == PTYCHO_I_U16;
         LAUNCH(c, PTYCHO_K_MEGA, {
             switch (c->N) {
-                case 64: k_dm_mega<64><<<grid, kThreads, MegaGeo<64>::smem, c->stream>>>(m); break;
-                case 128: k_dm_mega<128><<<grid, kThreads, MegaGeo<128>::smem, c->stream>>>(m); break;
-                case 256: k_dm_mega<256><<<grid, kThreads, MegaGeo<256>::smem, c->stream>>>(m); break;
-                default: k_dm_mega<512><<<grid, kThreads, MegaGeo<512>::smem, c->stream>>>(m); break;
+                case 64: if (u16) k_dm_mega<64, true><<<grid, kThreads, MegaGeo<64>::smem, c->stream>>>(m); else k_dm_mega<64, false><<<grid, kThreads, MegaGeo<64>::smem, c->stream>>>(m); break;
+                case 128: if (u16) k_dm_mega<128, true><<<grid, kThreads, MegaGeo<128>::smem, c->stream>>>(m); else k_dm_mega<128, false><<<grid, kThreads, MegaGeo<128>::smem, c->stream>>>(m); break;
+                case 256: if (u16) k_dm_mega<256, true><<<grid, kThreads, MegaGeo<256>::smem, c->stream>>>(m); else k_dm_mega<256, false><<<grid, kThreads, MegaGeo<256>::smem, c->stream>>>(m); break;
+                default: if (u16) k_dm_mega<512, true><<<grid, kThreads, MegaGeo<512>::smem, c->stream>>>(m); else k_dm_mega<512, false><<<grid, kThreads, MegaGeo<512>::smem, c->stream>>>(m); break;
             }
         });
     } else

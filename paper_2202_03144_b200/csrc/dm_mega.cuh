@@ -29,6 +29,7 @@ struct MegaArgs {
     FrameArgs f;        // psi = slot 0 of the store; S = ring base; frames = slot -> caller frame; e_part [J][NCB]
     int J, M, D, R, nW;
     int update_probe;   // accumulate the lagged probe sums (a9) in pass 1
+    int pf;             // slots ahead that the L2 prefetches reach (megakernel: M, the next wave; split kernels: the next chunk)
     int flags;          // experiment switches: 1 = no L2 prefetch, 4 = immediate signals
     const void* It;     // intensities re-tiled at init into pass-2 register order (k_tile_intensity)
     const YX* spos;     // [J] position of each SLOT (pos[frames[slot]], one load instead of two chained)
@@ -157,7 +158,7 @@ template <int N> struct MegaGeo {
 };
 
 // ---- pass 1: a1 exit wave, a2 reflector, a9 lagged probe sums, a3 forward row FFTs -> S --------
-template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
+template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
                                                             Deferred& df) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T, LW = 32 / T;
@@ -176,14 +177,14 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
     for (int i = 0; i < E; ++i) sP[t + T * i] = __ldg(a.P + off + t + T * i);
     __syncwarp();
     {   // psi of the NEXT wave's slots (this warp's lines): start HBM -> L2 now
-        const int s = s_begin + m.M + lane;
+        const int s = s_begin + m.pf + lane;
         if (!(m.flags & 1) && lane < m.M && s < m.J)
             l2_prefetch_bulk(a.psi + (size_t)s * N * N + (size_t)(blk * G::LPB + (threadIdx.x >> 5) * LW) * N, LW * N * 8);
     }
     PhaseClock pc;
     for (int slot = s_begin; slot < s_end; ++slot) {
         pc.start(0);
-        if (slot >= m.R) warp_wait(m.cnt3 + slot - m.R, G::NCB * kWarps);    // ring slot free again
+        if (SYNC && slot >= m.R) warp_wait(m.cnt3 + slot - m.R, G::NCB * kWarps);    // ring slot free again
         pc.lap(0);
         const YX p0 = m.spos[slot];
         const float2* orow = a.O + (size_t)(p0.y + y) * a.W + p0.x;
@@ -211,7 +212,7 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
         float2* srow = a.S + (size_t)(slot % m.R) * N * N + off;
 #pragma unroll
         for (int r = 0; r < E; ++r) __stcg(srow + freq_b<N>(t, r), v[r]);
-        df.cnt = m.cnt1 + slot;
+        if (SYNC) df.cnt = m.cnt1 + slot;
         if (m.flags & 4) df.flush_warp();
         pc.lap(3);
     }
@@ -225,7 +226,7 @@ template <int N> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, i
 }
 
 // ---- pass 2: a3 column FFTs, a4 error partial, a5 modulus projection (as s - 1), a6 inverse columns
-template <int N, bool U16> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
+template <int N, bool U16, bool SYNC = true> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
                                                             float* s_red, Deferred& df) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T, CB = G::LPB;
@@ -238,13 +239,13 @@ template <int N, bool U16> __device__ __forceinline__ void mega_pass2(const Mega
     const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
     const size_t tile_bytes = (size_t)N * CB * (U16 ? 2 : 4);   // this block's intensities of one slot: contiguous
     if (!(m.flags & 1) && threadIdx.x < m.M) {                              // I of the NEXT wave: HBM -> L2 now
-        const int s = s_begin + m.M + threadIdx.x;
+        const int s = s_begin + m.pf + threadIdx.x;
         if (s < m.J) l2_prefetch_bulk(reinterpret_cast<const char*>(m.It) + ((size_t)s * G::NCB + blk) * tile_bytes, (uint32_t)tile_bytes);
     }
     PhaseClock pc;
     for (int slot = s_begin; slot < s_end; ++slot) {
         pc.start(1);
-        warp_wait(m.cnt1 + slot, G::NCB * kWarps);
+        if (SYNC) warp_wait(m.cnt1 + slot, G::NCB * kWarps);
         pc.lap(0);
         float2* base = a.S + (size_t)(slot % m.R) * N * N + col;
         float2 v[E];
@@ -296,14 +297,14 @@ template <int N, bool U16> __device__ __forceinline__ void mega_pass2(const Mega
 #pragma unroll
         for (int r = 0; r < E; ++r) __stcg(base + (size_t)pos_a_inv<N>(t, r) * N, v[r]);
         __syncthreads();                                                    // sx and s_red free; stores issued by all
-        df.cnt = m.cnt2 + slot;
+        if (SYNC) df.cnt = m.cnt2 + slot;
         if (m.flags & 4) df.flush_cta_after_barrier();
         pc.lap(3);
     }
 }
 
 // ---- pass 3: a6 inverse row FFTs, a7 exit-wave update, a8 object scatter-add ---------------------
-template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
+template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
                                                             Deferred& df) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T;
@@ -320,7 +321,7 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
     PhaseClock pc;
     for (int slot = s_begin; slot < s_end; ++slot) {
         pc.start(2);
-        warp_wait(m.cnt2 + slot, G::NCB);
+        if (SYNC) warp_wait(m.cnt2 + slot, G::NCB);
         pc.lap(0);
         const float2* srow = a.S + (size_t)(slot % m.R) * N * N + off;
         float2 v[E];
@@ -355,7 +356,7 @@ template <int N> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, i
             red_add(a.nO + obase + x, cmulc(w, p));                         // a8 conj(P) psi_j
             red_add(a.dO + obase + x, fmaf(p.x, p.x, p.y * p.y));
         }
-        df.cnt = m.cnt3 + slot;
+        if (SYNC) df.cnt = m.cnt3 + slot;
         if (m.flags & 4) df.flush_warp();
         pc.lap(3);
     }
@@ -401,6 +402,25 @@ template <int N, bool U16> __global__ void __launch_bounds__(kThreads, (N >= 512
     __syncthreads();
     if (threadIdx.x < 16) atomicAdd(&g_phase[threadIdx.x], s_phase[threadIdx.x]);
 #endif
+}
+
+// ---- the same three passes as stream-ordered kernels over one chunk of waves -----------------------
+// grid (NCB, waves of the chunk); no flags: the stream orders pass 1 -> 2 -> 3 of a chunk, and each
+// kernel gets the register budget (hence the resident warps) of its own pass instead of the
+// megakernel's maximum over all three.  S holds the chunk (slot % R).
+template <int N, bool U16, int KIND>
+__global__ void __launch_bounds__(kThreads, (N >= 512 ? 1 : (KIND == 2 ? 2 : 3))) k_dm_pass(MegaArgs m, int wave0) {
+    using G = Geo<N>;
+    extern __shared__ __align__(16) float2 sm[];
+    float4* s_tw = reinterpret_cast<float4*>(sm + G::LPB * MegaGeo<N>::LINE);
+    __shared__ float s_red[kThreads / 32];
+    load_tw(s_tw, m.f.tw, m.f.twi, N);
+    __syncthreads();
+    Deferred df;
+    const int blk = blockIdx.x, wave = wave0 + blockIdx.y;
+    if (KIND == 2) mega_pass1<N, false>(m, blk, wave, sm, s_tw, df);
+    else if (KIND == 1) mega_pass2<N, U16, false>(m, blk, wave, sm, s_tw, s_red, df);
+    else mega_pass3<N, false>(m, blk, wave, sm, s_tw, df);
 }
 
 }  // namespace ptycho

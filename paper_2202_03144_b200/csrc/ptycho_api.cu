@@ -210,6 +210,12 @@ template <int N> ptycho_status set_attrs(ptycho_ctx* c) {
     CU(cudaFuncSetAttribute(k_cols<N, CM_PLAIN_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
     CU(cudaFuncSetAttribute(k_dm_mega<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
     CU(cudaFuncSetAttribute(k_dm_mega<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
+    CU(cudaFuncSetAttribute(k_dm_pass<N, true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
+    CU(cudaFuncSetAttribute(k_dm_pass<N, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
+    CU(cudaFuncSetAttribute(k_dm_pass<N, true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
+    CU(cudaFuncSetAttribute(k_dm_pass<N, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
+    CU(cudaFuncSetAttribute(k_dm_pass<N, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
+    CU(cudaFuncSetAttribute(k_dm_pass<N, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
     int per_sm = 0, dev = 0, sms = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_dm_mega<N, true>, kThreads, MegaGeo<N>::smem));
     CU(cudaGetDevice(&dev));
@@ -270,6 +276,17 @@ void passes(ptycho_ctx* c, const FrameArgs& a, int nframes, int fwd, int col, in
     }
 }
 
+// Stream-ordered form of the DM cycle: per chunk of waves, pass 1 -> pass 2 -> pass 3 as three kernels.
+template <int N, bool U16> void launch_split(ptycho_ctx* c, MegaArgs m, int chunk_waves) {
+    const size_t smem = MegaGeo<N>::smem;
+    for (int w0 = 0; w0 < m.nW; w0 += chunk_waves) {
+        const dim3 grid(Geo<N>::NCB, std::min(chunk_waves, m.nW - w0));
+        LAUNCH(c, PTYCHO_K_ROWS_FWD, (k_dm_pass<N, U16, 2><<<grid, kThreads, smem, c->stream>>>(m, w0)));
+        LAUNCH(c, PTYCHO_K_COLS, (k_dm_pass<N, U16, 1><<<grid, kThreads, smem, c->stream>>>(m, w0)));
+        LAUNCH(c, PTYCHO_K_ROWS_INV, (k_dm_pass<N, U16, 0><<<grid, kThreads, smem, c->stream>>>(m, w0)));
+    }
+}
+
 int ew_blocks(size_t n) { return (int)std::min<size_t>(kRedBlocks, (n + 255) / 256); }
 
 // spatial order (H6): tiles of N/2 rows, boustrophedon in x, so that consecutive frames overlap
@@ -301,9 +318,21 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         m.spos = c->spos;
         m.It = c->It;
         m.flags = env_int("PTYCHO_MEGA_FLAGS", 0);
+        m.pf = m.M;
         { int nw = (m.flags >> 8) ? 1 : 0; cudaMemcpyToSymbolAsync(g_nowait, &nw, sizeof(int), 0, cudaMemcpyHostToDevice, c->stream); }
         m.head = c->mega_ctr; m.cnt1 = c->mega_ctr + 64; m.cnt2 = m.cnt1 + c->J; m.cnt3 = m.cnt2 + c->J;
         CU(cudaMemsetAsync(c->mega_ctr, 0, sizeof(int) * (64 + 3 * (size_t)c->J), c->stream));
+        if (env_int("PTYCHO_DM_SPLIT", 0)) {
+            const int cw = std::max(1, std::min(env_int("PTYCHO_SPLIT_C", 96), m.R) / m.M);
+            m.pf = cw * m.M;
+            const bool u = c->itype == PTYCHO_I_U16;
+            switch (c->N) {
+                case 64: u ? launch_split<64, true>(c, m, cw) : launch_split<64, false>(c, m, cw); break;
+                case 128: u ? launch_split<128, true>(c, m, cw) : launch_split<128, false>(c, m, cw); break;
+                case 256: u ? launch_split<256, true>(c, m, cw) : launch_split<256, false>(c, m, cw); break;
+                default: u ? launch_split<512, true>(c, m, cw) : launch_split<512, false>(c, m, cw); break;
+            }
+        } else {
         const long long items = (long long)(m.nW + 2 * m.D) * 3 * ncb;
         const int grid = (int)std::min<long long>(items, c->mega_grid);
         const bool u16 = c->itype == PTYCHO_I_U16;
@@ -315,6 +344,7 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
                 default: if (u16) k_dm_mega<512, true><<<grid, kThreads, MegaGeo<512>::smem, c->stream>>>(m); else k_dm_mega<512, false><<<grid, kThreads, MegaGeo<512>::smem, c->stream>>>(m); break;
             }
         });
+        }
     } else
     for (int s0 = 0; s0 < c->J; s0 += c->chunk) {
         const int nf = std::min(c->chunk, c->J - s0);

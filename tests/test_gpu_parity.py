@@ -185,3 +185,78 @@ def test_device_resident_inputs(B, oracle_mod):
     g.fetch_object(out)
     o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities).iterate("DM", 3)
     assert rel(out.cpu().numpy(), o.O) < TOL_RUN
+
+
+# ------------------------------------------------- full size, in the configuration bench.py times
+def test_cfg2_full_size_sampled_frames_and_object(B, oracle_mod):
+    """Config 2 as `bench.py` runs it (DM, 256x256, J = 10 000, uint16, pbound 0.5, default queue
+    geometry).  In the first DM iteration psi_j' depends only on (O0, P0, I_j), so the oracle can
+    compute sampled frames one by one: an oracle built from the sampled positions alone must give
+    the GPU's exit waves for those frames.  The object is checked on everything the oracle can
+    afford: where the host has the memory, one full oracle iteration; in any case the closed form
+    of step 5 on a window, from the GPU's own exit waves of the frames that cover it."""
+    import psutil
+    s = synth.make_config(2)
+    par = dict(pbound=s.params["pbound"])
+    g = make(B, s, **par)
+    g.iterate("DM", 1)
+    J, n = s.n_pos, s.n
+    rng = np.random.default_rng(7)
+    idx = np.sort(rng.choice(J, 24, replace=False)).astype(np.int32)
+    idx[0], idx[-1] = 0, J - 1                                   # first and last frame of the scan
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos[idx], s.intensities[idx], par)
+    o.iterate("DM", 1)
+    psi_g = g.fetch_exit_waves(idx)
+    for k in range(len(idx)):
+        assert rel(psi_g[k], o.psi[k]) < TOL_ITER, (k, idx[k])
+    assert np.isfinite(g.fetch_error()[0])
+    O_g, P_g = g.fetch_object(), g.fetch_probe()
+
+    # window check: O_new = (sum_j conj(P0) psi_j' + eps O0) / (sum_j |P0|^2 + eps), eps = delta max|P0|^2 (R5)
+    y0, x0, w = 2000, 2010, 48
+    cover = np.where((s.pos[:, 0] <= y0) & (s.pos[:, 0] + n >= y0 + w) & (s.pos[:, 1] <= x0) & (s.pos[:, 1] + n >= x0 + w))[0]
+    part = np.where((s.pos[:, 0] < y0 + w) & (s.pos[:, 0] + n > y0) & (s.pos[:, 1] < x0 + w) & (s.pos[:, 1] + n > x0))[0]
+    assert len(cover) > 5
+    P0 = s.probe0[0].astype(np.complex128)
+    num = np.zeros((w, w), np.complex128)
+    den = np.zeros((w, w))
+    psi_w = g.fetch_exit_waves(part.astype(np.int32))
+    for k, j in enumerate(part):
+        py, px = int(s.pos[j, 0]), int(s.pos[j, 1])
+        ys, xs = max(y0, py), max(x0, px)
+        ye, xe = min(y0 + w, py + n), min(x0 + w, px + n)
+        sl = (slice(ys - py, ye - py), slice(xs - px, xe - px))
+        num[ys - y0:ye - y0, xs - x0:xe - x0] += np.conj(P0[sl]) * psi_w[k, 0][sl]
+        den[ys - y0:ye - y0, xs - x0:xe - x0] += np.abs(P0[sl]) ** 2
+    eps = 1e-2 * np.max(np.abs(P0) ** 2)
+    expect = (num + eps * s.obj0[y0:y0 + w, x0:x0 + w]) / (den + eps)
+    assert rel(O_g[y0:y0 + w, x0:x0 + w], expect) < TOL_ITER
+
+    if psutil.virtual_memory().available > 40 * 2 ** 30:         # psi in double: 10.5 GB
+        of = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, par)
+        of.iterate("DM", 1)
+        assert rel(O_g, of.O) < TOL_ITER and rel(P_g, of.P) < TOL_ITER
+        assert np.allclose(g.fetch_error(), of.err, rtol=2e-3)
+    g.destroy()
+
+
+def test_dm_queue_geometry_does_not_change_the_result(B, oracle_mod, monkeypatch):
+    """The megakernel's wave size, lag and ring slack are scheduling only: any legal setting gives the
+    oracle's result (ragged last wave, ring wrap-around and J smaller than a wave included)."""
+    s = synth.make_custom(128, 420, 7, 37, k=1, peak=2e4, dtype=np.uint16, jitter=3, seed=5, probe_kind="zone")
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(pbound=0.3)).iterate("DM", 3)
+    for M, D, X in ((1, 2, 0), (3, 2, 1), (5, 3, 4), (64, 2, 0)):
+        monkeypatch.setenv("PTYCHO_MEGA_M", str(M))
+        monkeypatch.setenv("PTYCHO_MEGA_D", str(D))
+        monkeypatch.setenv("PTYCHO_MEGA_X", str(X))
+        g = make(B, s, pbound=0.3)
+        g.iterate("DM", 3)
+        assert rel(g.fetch_object(), o.O) < 3 * TOL_ITER, (M, D, X)
+        assert rel(g.fetch_exit_waves(), o.psi) < 3 * TOL_ITER, (M, D, X)
+        g.destroy()
+    monkeypatch.setenv("PTYCHO_DM_SPLIT", "1")                   # the stream-ordered three-kernel form of the same passes
+    monkeypatch.setenv("PTYCHO_MEGA_M", "2")
+    g = make(B, s, pbound=0.3)
+    g.iterate("DM", 3)
+    assert rel(g.fetch_object(), o.O) < 3 * TOL_ITER and rel(g.fetch_exit_waves(), o.psi) < 3 * TOL_ITER
+    g.destroy()

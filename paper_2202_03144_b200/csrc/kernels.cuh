@@ -36,6 +36,8 @@ struct FrameArgs {
     const int* __restrict__ frames; // caller frame id of each slot of this launch
     float2* S;                      // scratch: nframes x K x N x N
     const void* __restrict__ I;     // intensities, caller numbering
+    const void* __restrict__ It;    // intensities re-tiled per (DM slot, column block) in pass-2 register order (dm_mega.cuh)
+    const int* __restrict__ slot_of; // caller frame -> DM slot (indexes It)
     int itype;                      // 0 f32, 1 u16
     float* e_part;                  // per slot: NCB error partials (this launch's first slot)
     float2* nO; float* dO;          // object canvases H x W
@@ -54,7 +56,8 @@ template <int N> struct Geo {
     static constexpr int NCB = N / LPB;                          // column blocks (= row blocks) per frame
     static constexpr size_t smem_rows = (size_t)(LPB * LS_ROW + 4 * N) * sizeof(float2);
     static size_t smem_cols(int K) {
-        return (size_t)(LPB * LS_COL + 4 * N) * sizeof(float2) + (K > 1 ? (size_t)K * E * kThreads * sizeof(float2) : 0) + 64;
+        (void)K;
+        return (size_t)(LPB * LS_COL + 4 * N) * sizeof(float2) + 64;
     }
 };
 
@@ -119,11 +122,11 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_fw
                 v[i] = make_float2(2.f * v[i].x - s.x, 2.f * v[i].y - s.y);             // reflector
             }
         }
-        fft_line_fwd<N>(v, t, sx, s_tw);
+        fft_line_fwd<N, true>(v, t, sx, s_tw);          // a row's T threads sit in one warp
         float2* srow = a.S + fr + off;
 #pragma unroll
         for (int r = 0; r < E; ++r) srow[freq_b<N>(t, r)] = v[r];
-        __syncthreads();
+        __syncwarp();
     }
     if (MODE == RF_DM) {
 #pragma unroll
@@ -140,7 +143,6 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_cols(Fr
     constexpr int E = G::E, T = G::T, CB = G::LPB;
     extern __shared__ __align__(16) float2 sm[];
     float4* s_tw = reinterpret_cast<float4*>(sm + CB * G::LS_COL);
-    float2* stage = reinterpret_cast<float2*>(s_tw + 2 * N);                         // K > 1: [k][r][tid]
     __shared__ float s_red[kThreads / 32];
     load_tw(s_tw, a.tw, a.twi, N);
     const int c = threadIdx.x % CB, t = threadIdx.x / CB;
@@ -168,7 +170,6 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_cols(Fr
         return;
     }
 
-    const size_t ibase = (size_t)a.frames[slot] * N * N + col;
     float amp2[E];
 #pragma unroll
     for (int r = 0; r < E; ++r) amp2[r] = 0.f;
@@ -182,9 +183,35 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_cols(Fr
         for (int r = 0; r < E; ++r) amp2[r] += v[r].x * v[r].x + v[r].y * v[r].y;
         if (a.K > 1) {
 #pragma unroll
-            for (int r = 0; r < E; ++r) stage[((size_t)k * E + r) * kThreads + threadIdx.x] = v[r];
+            for (int r = 0; r < E; ++r) const_cast<float2*>(base)[(size_t)freq_b<N>(t, r) * N] = v[r];   // K > 1: the spectrum waits in S (L2), not in shared memory: keeps 2-3 CTAs per SM
         }
         __syncthreads();
+    }
+    // I_j in this thread's register order: 16-byte chunks of the tiled copy (dm_mega.cuh k_tile_intensity)
+    float in_t[E];
+    {
+        const size_t tile_bytes = (size_t)N * CB * (a.itype == 1 ? 2 : 4);
+        const uint4* it = reinterpret_cast<const uint4*>(reinterpret_cast<const char*>(a.It) +
+                                                         ((size_t)a.slot_of[a.frames[slot]] * G::NCB + blockIdx.x) * tile_bytes) + threadIdx.x;
+        if (a.itype == 1) {
+#pragma unroll
+            for (int j = 0; j < E / 8; ++j) {
+                const uint4 q = __ldg(it + j * kThreads);
+                const unsigned w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const unsigned lo = w[k] & 0xffffu, hi = w[k] >> 16;
+                    in_t[8 * j + 2 * k] = lo == 65535u ? -1.0f : (float)lo;
+                    in_t[8 * j + 2 * k + 1] = hi == 65535u ? -1.0f : (float)hi;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < E / 4; ++j) {
+                const float4 q = __ldg(reinterpret_cast<const float4*>(it) + j * kThreads);
+                in_t[4 * j] = q.x; in_t[4 * j + 1] = q.y; in_t[4 * j + 2] = q.z; in_t[4 * j + 3] = q.w;
+            }
+        }
     }
     // a4 error term and a5 scale.  scale[r] carries the 1/N^2 of F^-1.
     constexpr float inv_n2 = 1.0f / ((float)N * (float)N);
@@ -193,7 +220,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_cols(Fr
     bool zero_amp = false;
 #pragma unroll
     for (int r = 0; r < E; ++r) {
-        const float in = load_intensity(a.I, a.itype, ibase + (size_t)freq_b<N>(t, r) * N);
+        const float in = in_t[r];
         const float amp = sqrtf(amp2[r]);
         if (in >= 0.f) {
             const float sq = sqrtf(in), d = sq - amp;
@@ -217,7 +244,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_cols(Fr
     for (int k = 0; k < a.K; ++k) {
         if (a.K > 1) {
 #pragma unroll
-            for (int r = 0; r < E; ++r) v[r] = stage[((size_t)k * E + r) * kThreads + threadIdx.x];
+            for (int r = 0; r < E; ++r) v[r] = (a.S + fr + (size_t)k * N * N + col)[(size_t)freq_b<N>(t, r) * N];   // this thread's own stores
         }
 #pragma unroll
         for (int r = 0; r < E; ++r) {
@@ -283,7 +310,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_in
         const float2* srow = a.S + fr + off;
 #pragma unroll
         for (int r = 0; r < E; ++r) v[r] = srow[freq_b<N>(t, r)];
-        fft_line_inv<N>(v, t, sx, s_tw + N);            // v = F^-1[exact projection]
+        fft_line_inv<N, true>(v, t, sx, s_tw + N);      // v = F^-1[exact projection]
 #pragma unroll
         for (int r = 0; r < E; ++r) {
             const int x = pos_a_inv<N>(t, r);
@@ -306,7 +333,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_in
             accO[r] = cadd(accO[r], cmulc(w, p));                          // a8 conj(P_k) w
             accD[r] = fmaf(p.x, p.x, fmaf(p.y, p.y, accD[r]));
         }
-        __syncthreads();
+        __syncwarp();
     }
     if (MODE == RI_REVISED) return;
 #pragma unroll
@@ -352,29 +379,24 @@ struct Scalars {            // device-resident scalars (no host round trip insid
     unsigned int max_bits;  // scratch for atomicMax on non-negative floats
 };
 
-// max over r of sum_k |P_k(r)|^2 -> sc->max_p2.  single CTA of 1024 threads.
+// max over r of sum_k |P_k(r)|^2 -> sc->max_p2 (zeroed by the caller; atomicMax on the bit pattern of
+// non-negative floats is order-independent, hence deterministic).
 __global__ void k_probe_max(const float2* __restrict__ P, int K, int nn, Scalars* sc) {
-    __shared__ float s[32];
     float m = 0.f;
-    for (int q = threadIdx.x; q < nn; q += blockDim.x) {
+    for (int q = blockIdx.x * blockDim.x + threadIdx.x; q < nn; q += gridDim.x * blockDim.x) {
         float v = 0.f;
         for (int k = 0; k < K; ++k) { const float2 p = P[(size_t)k * nn + q]; v += p.x * p.x + p.y * p.y; }
         m = fmaxf(m, v);
     }
     for (int d = 16; d > 0; d >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, d));
-    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = m;
-    __syncthreads();
-    if (threadIdx.x == 0) { for (int w = 1; w < (int)blockDim.x / 32; ++w) m = fmaxf(m, s[w]); sc->max_p2 = m; }
+    if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<unsigned int*>(&sc->max_p2), __float_as_uint(m));
 }
-// max over r of d_P(r) -> sc->max_dp.  single CTA.
+// max over r of d_P(r) -> sc->max_dp (zeroed by the caller).
 __global__ void k_real_max(const float* __restrict__ d, int nn, Scalars* sc) {
-    __shared__ float s[32];
     float m = 0.f;
-    for (int q = threadIdx.x; q < nn; q += blockDim.x) m = fmaxf(m, d[q]);
+    for (int q = blockIdx.x * blockDim.x + threadIdx.x; q < nn; q += gridDim.x * blockDim.x) m = fmaxf(m, d[q]);
     for (int dd = 16; dd > 0; dd >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, dd));
-    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = m;
-    __syncthreads();
-    if (threadIdx.x == 0) { for (int w = 1; w < (int)blockDim.x / 32; ++w) m = fmaxf(m, s[w]); sc->max_dp = m; }
+    if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<unsigned int*>(&sc->max_dp), __float_as_uint(m));
 }
 // max |O|^2 at init (for eps_P); uses atomicMax on the bit pattern of non-negative floats.
 __global__ void k_abs2_max(const float2* __restrict__ a, size_t n, Scalars* sc) {
@@ -435,14 +457,14 @@ __global__ void k_direction(float2* n, const float* __restrict__ d, size_t plane
 }
 
 // LSQML cross term A12 = Re sum_j sum_r T(r) conj(dO[r_j+r]) O[r_j+r],  T = sum_k conj(P_k) dP_k.
-// grid (nframes); part[block] = this frame's sum.
+// grid (nframes, parts): block (f, p) sums every parts-th pixel group of frame f; part[f * parts + p].
 __global__ void k_lsq_cross(const float2* __restrict__ O, const float2* __restrict__ dO, int W,
                             const float2* __restrict__ P, const float2* __restrict__ dPk, int K, int n,
                             const YX* __restrict__ pos, const int* __restrict__ frames, double* part) {
     const YX p0 = pos[frames[blockIdx.x]];
     const int nn = n * n;
     double acc = 0.0;
-    for (int q = threadIdx.x; q < nn; q += blockDim.x) {
+    for (int q = blockIdx.y * blockDim.x + threadIdx.x; q < nn; q += gridDim.y * blockDim.x) {
         const int y = q / n, x = q % n;
         float2 tq = make_float2(0.f, 0.f);
         for (int k = 0; k < K; ++k) tq = cadd(tq, cmulc(dPk[(size_t)k * nn + q], P[(size_t)k * nn + q]));
@@ -454,17 +476,27 @@ __global__ void k_lsq_cross(const float2* __restrict__ O, const float2* __restri
     for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
     if ((threadIdx.x & 31) == 0) sa[threadIdx.x >> 5] = acc;
     __syncthreads();
-    if (threadIdx.x == 0) { for (int w = 1; w < (int)blockDim.x / 32; ++w) acc += sa[w]; part[blockIdx.x] = acc; }
+    if (threadIdx.x == 0) { for (int w = 1; w < (int)blockDim.x / 32; ++w) acc += sa[w]; part[blockIdx.x * gridDim.y + blockIdx.y] = acc; }
 }
 
-// a11: sum the partials in fixed order, solve the 2x2 system (R9), publish the steps.
+// a11: sum the partials in a fixed order (thread-strided, then a shared-memory tree: the same order
+// on every run), solve the 2x2 system (R9), publish the steps.  One CTA of 256 threads.
 __global__ void k_lsq_solve(const double* partO, int nO, const double* partP, int nP, const double* partX, int nX,
                             float lambda, int update_probe, Scalars* sc, double* steps_out) {
-    if (threadIdx.x || blockIdx.x) return;
-    double A11 = 0, b1 = 0, A22 = 0, b2 = 0, A12 = 0;
-    for (int i = 0; i < nO; ++i) { A11 += partO[2 * i]; b1 += partO[2 * i + 1]; }
-    for (int i = 0; i < nP; ++i) { A22 += partP[2 * i]; b2 += partP[2 * i + 1]; }
-    for (int i = 0; i < nX; ++i) A12 += partX[i];
+    __shared__ double sh[5][256];
+    double v[5] = {0, 0, 0, 0, 0};                       // A11, b1, A22, b2, A12
+    for (int i = threadIdx.x; i < nO; i += 256) { v[0] += partO[2 * i]; v[1] += partO[2 * i + 1]; }
+    for (int i = threadIdx.x; i < nP; i += 256) { v[2] += partP[2 * i]; v[3] += partP[2 * i + 1]; }
+    for (int i = threadIdx.x; i < nX; i += 256) v[4] += partX[i];
+    for (int q = 0; q < 5; ++q) sh[q][threadIdx.x] = v[q];
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if ((int)threadIdx.x < w)
+            for (int q = 0; q < 5; ++q) sh[q][threadIdx.x] += sh[q][threadIdx.x + w];
+        __syncthreads();
+    }
+    if (threadIdx.x) return;
+    const double A11 = sh[0][0], b1 = sh[1][0], A22 = sh[2][0], b2 = sh[3][0], A12 = sh[4][0];
     const double l = 1.0 + (double)lambda;
     double a, b;
     if (!update_probe) { a = (A11 > 0) ? b1 / (A11 * l) : 0.0; b = 0.0; }

@@ -24,7 +24,8 @@ namespace {
 
 constexpr int kErrCap = 1 << 16;    // iterations of error history kept
 constexpr int kStepCap = 1 << 18;   // (a, b) pairs kept
-constexpr int kRedBlocks = 1024;    // blocks of the canvas reductions / element-wise kernels
+constexpr int kCrossParts = 8;      // blocks per frame of the LSQML cross-term gather
+constexpr int kRedBlocks = 4736;    // blocks of the canvas reductions / element-wise kernels
 
 struct Carver {                     // bump allocator over the caller's workspace (256-byte aligned)
     char* base;
@@ -180,10 +181,10 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
     c->steps = w.take<double>(2 * (size_t)kStepCap);
     c->partO = w.take<double>(2 * kRedBlocks);
     c->partP = w.take<double>(2 * kRedBlocks);
-    c->partX = w.take<double>(c->J);
+    c->partX = w.take<double>((size_t)c->J * kCrossParts);
     c->scratch_d = w.take<double>(kRedBlocks);
     if (!c->par.disable_dm) c->psi = w.take<float2>((size_t)c->J * knn);
-    if (c->mega_M > 0) c->It = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
+    c->It = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
     if (copy_I) c->I = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
     return (w.off + 255) & ~size_t(255);
 }
@@ -238,6 +239,7 @@ void host_twiddles(int n, int E, int T, std::vector<float2>& tw, std::vector<flo
 FrameArgs base_args(const ptycho_ctx* c) {
     FrameArgs a{};
     a.O = c->O; a.W = c->W; a.P = c->P; a.K = c->K; a.pos = c->pos; a.S = c->S; a.I = c->I; a.itype = c->itype;
+    a.It = c->It; a.slot_of = c->slot_of;
     a.nO = c->nO; a.dO = c->dO; a.nP = c->nP; a.dP = c->dP; a.pbound = c->par.pbound; a.tw = c->tw; a.twi = c->twi;
     return a;
 }
@@ -366,7 +368,8 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
     const int nb = (int)c->mb_offsets.size() - 1;
     for (int b = 0; b < nb; ++b) {
         const int b0 = c->mb_offsets[b], b1 = c->mb_offsets[b + 1];
-        LAUNCH(c, PTYCHO_K_UPDATE, (k_probe_max<<<1, 1024, 0, c->stream>>>(c->P, c->K, (int)nn, c->sc)));
+        CU(cudaMemsetAsync(&c->sc->max_p2, 0, sizeof(float), c->stream));
+        LAUNCH(c, PTYCHO_K_UPDATE, (k_probe_max<<<64, 256, 0, c->stream>>>(c->P, c->K, (int)nn, c->sc)));
         for (int s0 = b0; s0 < b1; s0 += c->chunk) {
             const int nf = std::min(c->chunk, b1 - s0);
             FrameArgs a = base_args(c);
@@ -378,16 +381,17 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
         const int gO = ew_blocks(HW), gP = ew_blocks(nn);
         LAUNCH(c, PTYCHO_K_UPDATE, (k_direction<<<gO, 256, 0, c->stream>>>(c->nO, c->dO, HW, 1, c->par.delta_obj, c->sc, 0, lsq ? c->partO : nullptr)));
         if (upd) {
-            LAUNCH(c, PTYCHO_K_UPDATE, (k_real_max<<<1, 1024, 0, c->stream>>>(c->dP, (int)nn, c->sc)));
+            CU(cudaMemsetAsync(&c->sc->max_dp, 0, sizeof(float), c->stream));
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_real_max<<<64, 256, 0, c->stream>>>(c->dP, (int)nn, c->sc)));
             LAUNCH(c, PTYCHO_K_UPDATE, (k_direction<<<gP, 256, 0, c->stream>>>(c->nP, c->dP, nn, c->K, c->par.delta_probe, c->sc, 1, lsq ? c->partP : nullptr)));
         }
         double* step_slot = c->n_steps < kStepCap ? c->steps + 2 * c->n_steps : nullptr;
         if (lsq) {
             if (upd) {
-                LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_cross<<<b1 - b0, 256, 0, c->stream>>>(c->O, c->nO, c->W, c->P, c->nP, c->K, c->N, c->pos,
+                LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_cross<<<dim3(b1 - b0, kCrossParts), 256, 0, c->stream>>>(c->O, c->nO, c->W, c->P, c->nP, c->K, c->N, c->pos,
                                                                                         c->mb_frames + b0, c->partX)));
             }
-            LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_solve<<<1, 32, 0, c->stream>>>(c->partO, gO, c->partP, upd ? gP : 0, c->partX, upd ? b1 - b0 : 0,
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_solve<<<1, 256, 0, c->stream>>>(c->partO, gO, c->partP, upd ? gP : 0, c->partX, upd ? (b1 - b0) * kCrossParts : 0,
                                                                             c->par.lsq_lambda, upd, c->sc, step_slot ? step_slot : c->scratch_d)));
         } else {
             LAUNCH(c, PTYCHO_K_UPDATE, (k_set_steps<<<1, 1, 0, c->stream>>>(c->sc, c->par.alpha_obj, upd ? c->par.alpha_probe : 0.f, step_slot)));
@@ -544,7 +548,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     CUI(cudaMemcpyAsync(c->mb_frames, mb.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
     CUI(cudaMemcpyAsync(c->slot_of, c->slot_of_h.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
 
-    if (c->mega_M > 0) {                                    // intensities in pass-2 tile order (dm_mega.cuh)
+    {                                                       // intensities in pass-2 tile order (dm_mega.cuh)
         const dim3 g(ncb_of(n), n_pos);
 #define TILE_I(NN) do { if (itype == PTYCHO_I_U16) k_tile_intensity<NN, unsigned short><<<g, kThreads, 0, s>>>((unsigned short*)c->It, (const unsigned short*)c->I, c->dm_frames); \
                         else k_tile_intensity<NN, float><<<g, kThreads, 0, s>>>((float*)c->It, (const float*)c->I, c->dm_frames); } while (0)
@@ -553,7 +557,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
         ++c->launches;
     }
     // init-time constants on the device: eps_O, eps_P (R5), sum_I (C3)
-    k_probe_max<<<1, 1024, 0, s>>>(c->P, c->K, (int)nn, c->sc);
+    k_probe_max<<<64, 256, 0, s>>>(c->P, c->K, (int)nn, c->sc);   // sc was zeroed above
     k_finish_init<<<1, 1, 0, s>>>(c->sc, par.delta_blend, n_pos, 0);
     k_abs2_max<<<ew_blocks(HW), 256, 0, s>>>(c->O, HW, c->sc);
     k_finish_init<<<1, 1, 0, s>>>(c->sc, par.delta_blend, n_pos, 1);

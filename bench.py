@@ -32,6 +32,7 @@ sys.path.insert(0, _ROOT)
 METRIC = "diffraction patterns/sec per DM iteration (256x256, 1 B200); % HBM roofline"
 UNIT = "patterns/s"
 CFG = 2                      # BASELINE.json configs[2]
+NCU_DRAM_BYTES_PER_LAUNCH = 14.84e9   # profiles/r01_v2_mega_full_metrics.txt (7.289 GB read + 7.555 GB written)
 REF_SAMPLE = 256             # frames of the bounded oracle sample (first positions of the same scan)
 
 
@@ -256,7 +257,9 @@ def ours_line(args) -> dict | None:
     n_chain = sum(prof[k][1] for k in chain)
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": None, "peak_source": peak_src,
+        "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (chain == ("mega",) and J == 10000 and args.n_pos is None) else None,
+        "traffic_source": "ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of one k_dm_mega launch (profiles/r01_v2.md)",
+        "peak_source": peak_src,
         "kernel": ("k_dm_mega<256> (one persistent launch per DM iteration: a1-a9 of all frames)" if chain == ("mega",)
                    else "k_rows_fwd+k_cols+k_rows_inv chain (one chunk of frames per launch triple)"),
         "algorithmic_bytes_per_pattern": alg_bytes,

@@ -110,7 +110,7 @@ struct Timed {
 bool valid_n(int n) { return n == 64 || n == 128 || n == 256 || n == 512; }
 
 int chunk_frames(int n, int K, int J) {
-    double mb = 32.0;
+    double mb = 64.0;
     if (const char* e = getenv("PTYCHO_CHUNK_MB")) mb = atof(e) > 0 ? atof(e) : mb;
     long long per = (long long)K * n * n * 8;
     long long c = (long long)(mb * 1048576.0) / per;

@@ -72,8 +72,11 @@ typedef struct {
                            amplitude error per pixel in counts; 0 = exact projection (R6)          */
     int disable_dm;     /* 1 = do not reserve the DM exit-wave store (J*K*N*N complex64) in the
                            workspace; ptycho_iterate(PTYCHO_DM) then returns PTYCHO_ESTATE          */
-    int deterministic;  /* 1 = fixed-order gather accumulation of the overlap sums: results are
-                           bit-reproducible run to run; 0 = tiled atomics                          */
+    int deterministic;  /* 1 = fixed-order gather accumulation of the overlap sums (north_star "deterministic
+                           sorted-tile mode"): O, P and psi are bit-reproducible run to run; psi is read
+                           twice more per iteration.  Single-mode DM only: init returns
+                           PTYCHO_EUNSUPPORTED for n_modes > 1 or disable_dm, iterate for the minibatch
+                           algorithms.  0 = atomic scatter-add                                     */
     const int32_t *batch_order; /* HOST pointer or NULL.  NULL: strided batches, n_b = ceil(J/B),
                            batch b = { j : j mod n_b = b } (R8).  Else a permutation of 0..J-1;
                            batch b = its entries [b*B, (b+1)*B).  Copied at init.                  */

@@ -29,6 +29,7 @@ struct MegaArgs {
     FrameArgs f;        // psi = slot 0 of the store; S = ring base; frames = slot -> caller frame; e_part [J][NCB]
     int J, M, D, R, nW;
     int update_probe;   // accumulate the lagged probe sums (a9) in pass 1
+    int det;            // deterministic mode: no floating-point atomics here (dm_det.cuh forms the overlap sums)
     int pf;             // slots ahead that the L2 prefetches reach (megakernel: M, the next wave; split kernels: the next chunk)
     int flags;          // experiment switches: 1 = no L2 prefetch, 4 = immediate signals
     const void* It;     // intensities re-tiled at init into pass-2 register order (k_tile_intensity)
@@ -353,8 +354,10 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
             const float2 po = cmul(p, o[r]);
             const float2 w = make_float2(fmaf(keep, v[r].x, po.x), fmaf(keep, v[r].y, po.y));   // a7
             __stcs(prow + x, w);
-            red_add(a.nO + obase + x, cmulc(w, p));                         // a8 conj(P) psi_j
-            red_add(a.dO + obase + x, fmaf(p.x, p.x, p.y * p.y));
+            if (!m.det) {
+                red_add(a.nO + obase + x, cmulc(w, p));                     // a8 conj(P) psi_j
+                red_add(a.dO + obase + x, fmaf(p.x, p.x, p.y * p.y));
+            }
         }
         if (SYNC) df.cnt = m.cnt3 + slot;
         if (m.flags & 4) df.flush_warp();

@@ -17,6 +17,7 @@
 
 #include "kernels.cuh"
 #include "dm_mega.cuh"
+#include "dm_det.cuh"
 
 using namespace ptycho;
 
@@ -50,6 +51,9 @@ struct ptycho_ctx {
     float *dO = nullptr, *dP = nullptr, *e_part = nullptr, *e_tmp = nullptr;
     float2 *tw = nullptr, *twi = nullptr;
     YX* pos = nullptr;
+    int *tile_start = nullptr, *tile_list = nullptr;   // deterministic mode: frames per object tile (CSR, slot order)
+    float4* det_partial = nullptr;
+    int det_tx = 0, det_ty = 0;
     void* It = nullptr;                        // intensities re-tiled for the DM megakernel
     YX* spos = nullptr;                        // positions in DM slot order
     int *dm_frames = nullptr, *mb_frames = nullptr, *tmp_idx = nullptr, *slot_of = nullptr;
@@ -185,6 +189,12 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
     c->scratch_d = w.take<double>(kRedBlocks);
     if (!c->par.disable_dm) c->psi = w.take<float2>((size_t)c->J * knn);
     c->It = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
+    if (c->par.deterministic) {
+        c->det_tx = (c->W + kDetTileW - 1) / kDetTileW; c->det_ty = (c->H + kDetTileH - 1) / kDetTileH;
+        c->tile_start = w.take<int>((size_t)c->det_tx * c->det_ty + 1);
+        c->tile_list = w.take<int>((size_t)c->J * (c->N / kDetTileW + 1) * (c->N / kDetTileH + 1));   // upper bound
+        c->det_partial = w.take<float4>((size_t)kDetGroups * nn);
+    }
     if (copy_I) c->I = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
     return (w.off + 255) & ~size_t(255);
 }
@@ -316,7 +326,14 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         m.f = base_args(c);
         m.f.psi = c->psi; m.f.frames = c->dm_frames; m.f.e_part = c->e_part;
         m.J = c->J; m.M = c->mega_M; m.D = c->mega_D; m.R = c->mega_R; m.nW = (c->J + m.M - 1) / m.M;
-        m.update_probe = upd;
+        const int det = c->par.deterministic;
+        m.update_probe = det ? 0 : upd;
+        m.det = det;
+        if (det && upd) {                                   // lagged probe sums from the incoming psi (R4), fixed order
+            LAUNCH(c, PTYCHO_K_OTHER, (k_det_probe<<<dim3((unsigned)((nn + 255) / 256), kDetGroups), 256, 0, c->stream>>>(
+                                           c->det_partial, c->psi, c->O, c->W, c->N, c->spos, c->J)));
+            LAUNCH(c, PTYCHO_K_OTHER, (k_det_probe_final<<<(unsigned)((nn + 255) / 256), 256, 0, c->stream>>>(c->nP, c->dP, c->det_partial, (int)nn, kDetGroups)));
+        }
         m.spos = c->spos;
         m.It = c->It;
         m.flags = env_int("PTYCHO_MEGA_FLAGS", 0);
@@ -356,6 +373,9 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         a.e_part = c->e_part + (size_t)s0 * ncb;
         passes(c, a, nf, RF_DM, CM_FULL, RI_DM);
     }
+    if (c->par.deterministic)                               // object sums from the new psi, fixed order
+        LAUNCH(c, PTYCHO_K_OTHER, (k_det_object<<<dim3(c->det_tx, c->det_ty), dim3(kDetTileW, kDetTileH), 0, c->stream>>>(
+                                       c->nO, c->dO, c->H, c->W, c->psi, c->P, c->N, c->spos, c->tile_start, c->tile_list)));
     LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(HW), 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1)));
     LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(nn), 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd)));
     return PTYCHO_OK;
@@ -448,7 +468,8 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     if (params) par = *params; else ptycho_default_params(&par);
     if (par.batch_size < 0 || par.pbound < 0 || par.delta_blend <= 0 || par.delta_obj <= 0 || par.delta_probe <= 0)
         return PTYCHO_EINVAL;
-    if (par.deterministic) return PTYCHO_EUNSUPPORTED;   // sorted-tile gather mode: not built yet
+    // deterministic mode (dm_det.cuh) is built for the single-mode DM megakernel path only
+    if (par.deterministic && (n_modes != 1 || par.disable_dm || !env_int("PTYCHO_MEGA", 1))) return PTYCHO_EUNSUPPORTED;
     if (cols_smem(n, n_modes) > 227 * 1024) return PTYCHO_EUNSUPPORTED;
 
     // positions: copy, check bounds (R10), accept host or device memory
@@ -548,6 +569,25 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     CUI(cudaMemcpyAsync(c->mb_frames, mb.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
     CUI(cudaMemcpyAsync(c->slot_of, c->slot_of_h.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
 
+    if (par.deterministic) {                                // frames per object tile, ascending slot (dm_det.cuh)
+        const size_t ntiles = (size_t)c->det_tx * c->det_ty;
+        std::vector<int> start(ntiles + 1, 0), list;
+        for (int pass = 0; pass < 2; ++pass) {
+            std::vector<int> fill(start.begin(), start.end() - 1);
+            for (int sidx = 0; sidx < n_pos; ++sidx) {
+                const int y = spos[2 * sidx], x = spos[2 * sidx + 1];
+                for (int ty = y / kDetTileH; ty <= (y + n - 1) / kDetTileH; ++ty)
+                    for (int tx = x / kDetTileW; tx <= (x + n - 1) / kDetTileW; ++tx) {
+                        const size_t tl = (size_t)ty * c->det_tx + tx;
+                        if (pass == 0) ++start[tl + 1]; else list[fill[tl]++] = sidx;
+                    }
+            }
+            if (pass == 0) { for (size_t i = 0; i < ntiles; ++i) start[i + 1] += start[i]; list.resize(start[ntiles]); }
+        }
+        CUI(cudaMemcpyAsync(c->tile_start, start.data(), start.size() * 4, cudaMemcpyHostToDevice, s));
+        CUI(cudaMemcpyAsync(c->tile_list, list.data(), list.size() * 4, cudaMemcpyHostToDevice, s));
+        CUI(cudaStreamSynchronize(s));                      // the host vectors go out of scope
+    }
     {                                                       // intensities in pass-2 tile order (dm_mega.cuh)
         const dim3 g(ncb_of(n), n_pos);
 #define TILE_I(NN) do { if (itype == PTYCHO_I_U16) k_tile_intensity<NN, unsigned short><<<g, kThreads, 0, s>>>((unsigned short*)c->It, (const unsigned short*)c->I, c->dm_frames); \
@@ -574,6 +614,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
 ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
     if (!c || n_iters < 0) return PTYCHO_EINVAL;
     if (alg != PTYCHO_EPIE_MB && alg != PTYCHO_DM && alg != PTYCHO_LSQML) return fail(c, PTYCHO_EINVAL, "unknown algorithm");
+    if (alg != PTYCHO_DM && c->par.deterministic) return fail(c, PTYCHO_EUNSUPPORTED, "deterministic mode covers DM only");
     if (alg == PTYCHO_DM && !c->psi) return fail(c, PTYCHO_ESTATE, "DM needs the exit-wave store (disable_dm was set)");
     for (int it = 0; it < n_iters; ++it) {
         ptycho_status st = alg == PTYCHO_DM ? dm_iteration(c) : minibatch_iteration(c, alg);

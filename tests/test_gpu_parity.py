@@ -260,3 +260,26 @@ def test_dm_queue_geometry_does_not_change_the_result(B, oracle_mod, monkeypatch
     g.iterate("DM", 3)
     assert rel(g.fetch_object(), o.O) < 3 * TOL_ITER and rel(g.fetch_exit_waves(), o.psi) < 3 * TOL_ITER
     g.destroy()
+
+
+def test_deterministic_mode_is_bit_reproducible_and_matches_the_oracle(B, oracle_mod):
+    """deterministic = 1: the overlap sums are formed by owner-computes kernels in slot order
+    (dm_det.cuh), no floating-point atomics: two runs agree bit for bit; the atomic mode agrees with
+    both within the parity tolerance; minibatch algorithms and K > 1 are refused."""
+    s = synth.make_custom(128, 420, 7, 37, k=1, peak=2e4, dtype=np.uint16, jitter=3, seed=9, probe_kind="zone")
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(pbound=0.3)).iterate("DM", 4)
+    runs = []
+    for _ in range(2):
+        g = make(B, s, pbound=0.3, deterministic=1)
+        g.iterate("DM", 4)
+        runs.append((g.fetch_object(), g.fetch_probe(), g.fetch_exit_waves(), g.fetch_error()))
+        with pytest.raises(B.PtychoError, match="EUNSUPPORTED"):
+            g.iterate("EPIE_MB", 1)
+        g.destroy()
+    for a, b in zip(*runs):
+        assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
+    assert rel(runs[0][0], o.O) < 4 * TOL_ITER and rel(runs[0][1], o.P) < 4 * TOL_ITER and rel(runs[0][2], o.psi) < 4 * TOL_ITER
+    assert np.allclose(runs[0][3], o.err, rtol=2e-3)
+    s3 = synth.make_custom(64, 160, 5, 13, k=2, peak=2e4, dtype=np.uint16, jitter=3, seed=3)
+    with pytest.raises(B.PtychoError, match="EUNSUPPORTED"):
+        make(B, s3, deterministic=1)

@@ -283,3 +283,41 @@ def test_deterministic_mode_is_bit_reproducible_and_matches_the_oracle(B, oracle
     s3 = synth.make_custom(64, 160, 5, 13, k=2, peak=2e4, dtype=np.uint16, jitter=3, seed=3)
     with pytest.raises(B.PtychoError, match="EUNSUPPORTED"):
         make(B, s3, deterministic=1)
+
+
+# --------------------------------------- the other configurations of BASELINE.json at their own sizes
+def _free_run(B, oracle_mod, s, alg, iters, par, tol, check_psi=False):
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, par)
+    g = make(B, s, **par)
+    o.iterate(alg, iters)
+    g.iterate(alg, iters)
+    ro, rp = rel(g.fetch_object(), o.O), rel(g.fetch_probe(), o.P)
+    assert ro < tol and rp < tol, (ro, rp)
+    if check_psi:
+        assert rel(g.fetch_exit_waves(), o.psi) < tol
+    assert np.allclose(g.fetch_error(), o.err, rtol=5e-3)
+    g.destroy()
+
+
+def test_cfg1_full_50_iterations_epie_and_dm(B, oracle_mod):
+    """Config 1 as written (128x128, 1024 positions, fp32 Poisson counts, batch 256): 50 free-running
+    iterations of ePIE-minibatch and of DM (pbound 0.12) within the 1e-3 bound of north_star."""
+    s = synth.make_config(1)
+    _free_run(B, oracle_mod, s, "EPIE_MB", 50, dict(batch_size=256), TOL_RUN)
+    _free_run(B, oracle_mod, s, "DM", 50, dict(pbound=s.params["pbound_dm"]), TOL_RUN, check_psi=True)
+
+
+def test_cfg3_lsqml_three_modes_truncated_scan(B, oracle_mod):
+    """Config 3 (LSQML-style, 256x256, 3 modes, uint16, 6144^2 object, batch 512) on the first 2048
+    positions of its scan (4 batches): 5 free-running iterations.  The full 20 000-position scan is
+    timed but not compared: one oracle iteration of it takes minutes."""
+    s = synth.make_config(3, n_pos=2048)
+    _free_run(B, oracle_mod, s, "LSQML", 5, dict(batch_size=512), TOL_RUN)
+
+
+def test_cfg4_dm_512_truncated_scan(B, oracle_mod):
+    """Config 4 (DM, 512x512, uint16, 8192^2 object, pbound 0.5) on the first 1024 positions of its
+    Fermat spiral: 3 free-running iterations, exit waves included (the oracle's psi of the full
+    16 384 positions would need 69 GB)."""
+    s = synth.make_config(4, n_pos=1024)
+    _free_run(B, oracle_mod, s, "DM", 3, dict(pbound=s.params["pbound"]), 3 * TOL_ITER, check_psi=True)

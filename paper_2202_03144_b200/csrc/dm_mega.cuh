@@ -75,6 +75,13 @@ __device__ __forceinline__ void warp_signal(int* cnt) {
     __syncwarp();
     if ((threadIdx.x & 31) == 0) asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(cnt) : "memory");
 }
+// "Ring slot read" needs no release: pass 3 signals only that its LOADS of S[slot] have completed (they
+// have, the butterflies consumed them); nothing it writes is read again inside this kernel.  A relaxed
+// increment spares the MEMBAR that would wait for the 48 stores and atomics of the previous slot.
+__device__ __forceinline__ void warp_signal_relaxed(int* cnt) {
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) asm volatile("red.relaxed.gpu.global.add.s32 [%0], 1;" ::"l"(cnt) : "memory");
+}
 __device__ __forceinline__ void warp_wait(const int* cnt, int target) {
     if ((threadIdx.x & 31) == 0) {
         while (ld_relaxed_gpu(cnt) < target && !g_nowait) __nanosleep(64);
@@ -345,7 +352,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
         fft_line_inv<N, true>(v, t, sx, s_tw + N);                          // v = F^-1[(s-1) Phi]
         __syncwarp();                                                       // sx is free for the next slot
         pc.lap(2);
-        df.flush_warp();                                                    // previous slot's signal
+        if (SYNC) warp_signal_relaxed(m.cnt3 + slot);                       // S[slot] has been read: the ring slot may be refilled
         float2* prow = a.psi + (size_t)slot * N * N + off;
 #pragma unroll
         for (int r = 0; r < E; ++r) {
@@ -359,8 +366,6 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
                 red_add(a.dO + obase + x, fmaf(p.x, p.x, p.y * p.y));
             }
         }
-        if (SYNC) df.cnt = m.cnt3 + slot;
-        if (m.flags & 4) df.flush_warp();
         pc.lap(3);
     }
 }

@@ -32,7 +32,7 @@ sys.path.insert(0, _ROOT)
 METRIC = "diffraction patterns/sec per DM iteration (256x256, 1 B200); % HBM roofline"
 UNIT = "patterns/s"
 CFG = 2                      # BASELINE.json configs[2]
-NCU_DRAM_BYTES_PER_LAUNCH = 14.84e9   # profiles/r01_v2_mega_full_metrics.txt (7.289 GB read + 7.555 GB written)
+NCU_DRAM_BYTES_PER_LAUNCH = 14.92e9   # profiles/r01_v3_mega_full_metrics.txt (7.286 GB read + 7.631 GB written)
 REF_SAMPLE = 256             # frames of the bounded oracle sample (first positions of the same scan)
 
 

@@ -200,11 +200,15 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(co
         float2 v[E];
 #pragma unroll
         for (int i = 0; i < E; ++i) v[i] = __ldcs(prow + t + T * i);      // psi_j: streamed once
+        float2 ov[E];
+#pragma unroll
+        for (int i = 0; i < E; ++i) ov[i] = __ldg(orow + t + T * i);
+        df.flush_warp();                        // previous slot's signal: its fence waits while these loads are in flight anyway
         PHASE_TOUCH(v[E - 1].x);
         pc.lap(1);
 #pragma unroll
         for (int i = 0; i < E; ++i) {
-            const float2 o = __ldg(orow + t + T * i);
+            const float2 o = ov[i];
             const float2 po = cmul(sP[t + T * i], o);                     // psi_O = P O_j
             const float2 s = v[i];
             if (m.update_probe) {
@@ -216,7 +220,6 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(co
         fft_line_fwd<N, true>(v, t, sx, s_tw);
         __syncwarp();                                                       // sx is free for the next slot
         pc.lap(2);
-        df.flush_warp();                                                    // previous slot's signal
         float2* srow = a.S + (size_t)(slot % m.R) * N * N + off;
 #pragma unroll
         for (int r = 0; r < E; ++r) __stcg(srow + freq_b<N>(t, r), v[r]);
@@ -267,10 +270,10 @@ template <int N, bool U16, bool SYNC = true> __device__ __forceinline__ void meg
 #pragma unroll
             for (int j = 0; j < NQ; ++j) iq[j] = __ldcs(it + j * kThreads);
         }
+        df.flush_cta_after_barrier();           // previous slot's signal: its fence waits while these loads are in flight anyway
         PHASE_TOUCH(v[E - 1].x + __uint_as_float(iq[NQ - 1].w));
         pc.lap(1);
         fft_line_fwd<N>(v, t, sx, s_tw);                                    // (CTA barrier inside)
-        df.flush_cta_after_barrier();                                       // previous slot's signal
         float err = 0.f;
 #pragma unroll
         for (int r = 0; r < E; ++r) {

@@ -40,7 +40,7 @@ class Params(C.Structure):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """nvcc the CUDA library in-tree for sm_100a (cross-compiles without a GPU)."""
-    srcs = [os.path.join(_CSRC, f) for f in ("ptycho_api.cu", "kernels.cuh", "fft_core.cuh", "dm_mega.cuh", "dm_det.cuh")]
+    srcs = [os.path.join(_CSRC, f) for f in ("ptycho_api.cu", "kernels.cuh", "fft_core.cuh", "dm_mega.cuh", "dm_det.cuh", "dm_cluster.cuh")]
     srcs.append(os.path.join(os.path.dirname(_HERE), "include", "ptycho_b200.h"))
     if not force and os.path.exists(LIB_PATH) and all(os.path.getmtime(LIB_PATH) >= os.path.getmtime(s) for s in srcs):
         return LIB_PATH

@@ -18,6 +18,7 @@
 #include "kernels.cuh"
 #include "dm_mega.cuh"
 #include "dm_det.cuh"
+#include "dm_cluster.cuh"
 
 using namespace ptycho;
 
@@ -288,6 +289,29 @@ void passes(ptycho_ctx* c, const FrameArgs& a, int nframes, int fwd, int col, in
     }
 }
 
+// One cluster of NCB CTAs per frame (dm_cluster.cuh).  N <= 256 only (a cluster holds at most 16 CTAs).
+template <int N, bool U16> ptycho_status launch_cluster(ptycho_ctx* c, ClusterArgs m) {
+    auto kern = k_dm_cluster<N, U16>;
+    const size_t smem = ClusterGeo<N>::smem;
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    cudaLaunchConfig_t cfg{};
+    cudaLaunchAttribute at{};
+    at.id = cudaLaunchAttributeClusterDimension;
+    at.val.clusterDim.x = Geo<N>::NCB; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+    cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream; cfg.attrs = &at; cfg.numAttrs = 1;
+    cfg.gridDim = dim3(Geo<N>::NCB);
+    int ncl = 0;
+    CU(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
+    if (ncl < 1) return fail(c, PTYCHO_EUNSUPPORTED, "no cluster of this size fits on the device");
+    ncl = std::min(std::min(ncl, c->J), std::max(1, env_int("PTYCHO_CLUSTERS", ncl)));
+    m.nclusters = ncl;
+    cfg.gridDim = dim3(Geo<N>::NCB * ncl);
+    LAUNCH(c, PTYCHO_K_MEGA, { cudaLaunchKernelEx(&cfg, kern, m); });
+    CU(cudaGetLastError());
+    return PTYCHO_OK;
+}
+
 // Stream-ordered form of the DM cycle: per chunk of waves, pass 1 -> pass 2 -> pass 3 as three kernels.
 template <int N, bool U16> void launch_split(ptycho_ctx* c, MegaArgs m, int chunk_waves) {
     const size_t smem = MegaGeo<N>::smem;
@@ -341,7 +365,18 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         { int nw = (m.flags >> 8) ? 1 : 0; cudaMemcpyToSymbolAsync(g_nowait, &nw, sizeof(int), 0, cudaMemcpyHostToDevice, c->stream); }
         m.head = c->mega_ctr; m.cnt1 = c->mega_ctr + 64; m.cnt2 = m.cnt1 + c->J; m.cnt3 = m.cnt2 + c->J;
         CU(cudaMemsetAsync(c->mega_ctr, 0, sizeof(int) * (64 + 3 * (size_t)c->J), c->stream));
-        if (env_int("PTYCHO_DM_SPLIT", 0)) {
+        if (env_int("PTYCHO_DM_CLUSTER", 0) && c->N <= 256) {
+            ClusterArgs ca{};
+            ca.f = m.f; ca.J = c->J; ca.update_probe = m.update_probe; ca.det = m.det; ca.spos = c->spos; ca.It = c->It;
+            const bool u = c->itype == PTYCHO_I_U16;
+            ptycho_status st = PTYCHO_OK;
+            switch (c->N) {
+                case 64: st = u ? launch_cluster<64, true>(c, ca) : launch_cluster<64, false>(c, ca); break;
+                case 128: st = u ? launch_cluster<128, true>(c, ca) : launch_cluster<128, false>(c, ca); break;
+                default: st = u ? launch_cluster<256, true>(c, ca) : launch_cluster<256, false>(c, ca); break;
+            }
+            if (st != PTYCHO_OK) return st;
+        } else if (env_int("PTYCHO_DM_SPLIT", 0)) {
             const int cw = std::max(1, std::min(env_int("PTYCHO_SPLIT_C", 96), m.R) / m.M);
             m.pf = cw * m.M;
             const bool u = c->itype == PTYCHO_I_U16;

@@ -254,6 +254,12 @@ def test_dm_queue_geometry_does_not_change_the_result(B, oracle_mod, monkeypatch
         assert rel(g.fetch_object(), o.O) < 3 * TOL_ITER, (M, D, X)
         assert rel(g.fetch_exit_waves(), o.psi) < 3 * TOL_ITER, (M, D, X)
         g.destroy()
+    monkeypatch.setenv("PTYCHO_DM_CLUSTER", "1")                 # one thread-block cluster per frame, exchange through DSMEM
+    g = make(B, s, pbound=0.3)
+    g.iterate("DM", 3)
+    assert rel(g.fetch_object(), o.O) < 3 * TOL_ITER and rel(g.fetch_exit_waves(), o.psi) < 3 * TOL_ITER
+    g.destroy()
+    monkeypatch.delenv("PTYCHO_DM_CLUSTER")
     monkeypatch.setenv("PTYCHO_DM_SPLIT", "1")                   # the stream-ordered three-kernel form of the same passes
     monkeypatch.setenv("PTYCHO_MEGA_M", "2")
     g = make(B, s, pbound=0.3)

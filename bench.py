@@ -32,7 +32,7 @@ sys.path.insert(0, _ROOT)
 METRIC = "diffraction patterns/sec per DM iteration (256x256, 1 B200); % HBM roofline"
 UNIT = "patterns/s"
 CFG = 2                      # BASELINE.json configs[2]
-NCU_DRAM_BYTES_PER_LAUNCH = 14.92e9   # profiles/r01_v3_mega_full_metrics.txt (7.286 GB read + 7.631 GB written)
+NCU_DRAM_BYTES_PER_LAUNCH = 14.89e9   # profiles/r01_v4_mega_full_metrics.txt (7.307 GB read + 7.579 GB written)
 REF_SAMPLE = 256             # frames of the bounded oracle sample (first positions of the same scan)
 
 
@@ -258,7 +258,7 @@ def ours_line(args) -> dict | None:
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (chain == ("mega",) and J == 10000 and args.n_pos is None) else None,
-        "traffic_source": "ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of one k_dm_mega launch (profiles/r01_v2.md)",
+        "traffic_source": "ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of one k_dm_mega launch (profiles/r01_v2.md, v4)",
         "peak_source": peak_src,
         "kernel": ("k_dm_mega<256> (one persistent launch per DM iteration: a1-a9 of all frames)" if chain == ("mega",)
                    else "k_rows_fwd+k_cols+k_rows_inv chain (one chunk of frames per launch triple)"),

@@ -164,6 +164,26 @@ long long ptycho_launch_count(const ptycho_ctx *ctx);
 const char *ptycho_last_error(const ptycho_ctx *ctx); /* never NULL; "" if none */
 void ptycho_destroy(ptycho_ctx *ctx);                 /* frees host state; the workspace is the caller's */
 
+/* ---- init-time preparation of raw detector frames (first item beyond the hot path) ----
+ * PAPER.md:50 lists what the paper does to the diffraction patterns before reconstruction: their centre
+ * is located, they are cropped to the reconstruction size, a noise threshold is applied and saturated
+ * pixels are detected from the detector bit depth.  This call does that on the GPU and writes the
+ * intensities in the layout ptycho_init takes (reading R1: FFT order, DC at [0,0]; reading R3: masked
+ * pixels carry the sentinel 65535 (uint16) or -1 (fp32)).  For output pixel (ky, kx), 0 <= ky, kx < n:
+ *     sy = center_y + (ky < n/2 ? ky : ky - n),   sx = center_x + (kx < n/2 ? kx : kx - n)
+ *     v  = raw[frame][sy][sx]            (a source pixel outside the detector, or a raw value that already is
+ *                                         the sentinel -- 65535 in uint16, negative in fp32: masked)
+ *     saturation > 0 and v >= saturation : masked
+ *     threshold  > 0 and v <  threshold  : 0
+ *     otherwise v (uint16 output: rounded to nearest, clipped to 65534)
+ * raw: n_frames x det_h x det_w, uint16 or fp32, row-major, host or device; out: n_frames x n x n, host or
+ * device; n is any even size >= 2 (not only the FFT sizes).  Integer / byte work: results are bit-exact
+ * against the oracle.  Synchronises the stream before returning.  PTYCHO_EINVAL on null pointers, odd n,
+ * non-positive sizes or unknown types. */
+ptycho_status ptycho_prepare_frames(const void *raw, ptycho_itype raw_type, int n_frames, int det_h, int det_w,
+                                    int center_y, int center_x, int n, float threshold, float saturation,
+                                    void *out, ptycho_itype out_type, void *cuda_stream);
+
 /* Unit-test entry points of single kernels (tier T2).  Device pointers. */
 /* Batched 2-D complex64 FFT of `count` n x n frames, in place, on `cuda_stream`. */
 ptycho_status ptycho_test_fft2(float *data, int n, int count, int inverse, void *cuda_stream);

@@ -179,3 +179,44 @@ class Oracle:
             self.err.append(float(num) / (self.sum_I if self.sum_I > 0 else 1.0))
             self.t += 1
         return self
+
+
+# --------------------------------------------------------------------------------------------------
+# Frame preparation (centre, crop, threshold, saturation from the bit depth).
+# TEST INFRASTRUCTURE like the rest of this package.  The definition written out: a centred crop of n x n
+# pixels around (cy, cx), the noise threshold, the saturation mask, then numpy's ifftshift to put the centre
+# pixel at [0, 0] (reading R1: FFT order).  Pinned in tests/test_oracle_pins.py against index arithmetic done by
+# hand on a 6 x 6 example and against the fftshift/ifftshift involution.
+def prepare_frames(raw, center, n, threshold=0.0, saturation=0.0, out_dtype=np.uint16):
+    raw = np.asarray(raw)
+    assert raw.ndim == 3 and n % 2 == 0
+    f, dh, dw = raw.shape
+    cy, cx = int(center[0]), int(center[1])
+    h = n // 2
+    val = np.zeros((f, n, n), np.float64)
+    masked = np.ones((f, n, n), bool)                      # outside the detector: masked
+    for iy in range(n):                                    # plain loops over the crop window (slow, obvious)
+        sy = cy - h + iy
+        if sy < 0 or sy >= dh:
+            continue
+        for ix in range(n):
+            sx = cx - h + ix
+            if sx < 0 or sx >= dw:
+                continue
+            v = raw[:, sy, sx].astype(np.float64)
+            m = (v == 65535) if raw.dtype == np.uint16 else (v < 0)     # already the sentinel (R3)
+            if saturation > 0:
+                m = m | (v >= np.float32(saturation))
+            if threshold > 0:
+                v = np.where(v < np.float32(threshold), 0.0, v)
+            val[:, iy, ix] = v
+            masked[:, iy, ix] = m
+    val = np.fft.ifftshift(val, axes=(1, 2))               # centre pixel (index h) -> index 0
+    masked = np.fft.ifftshift(masked, axes=(1, 2))
+    if np.dtype(out_dtype) == np.uint16:
+        out = np.minimum(np.rint(val), 65534).astype(np.uint16)
+        out[masked] = 65535
+    else:
+        out = val.astype(np.float32)
+        out[masked] = -1.0
+    return out

@@ -82,6 +82,8 @@ def lib():
         l.ptycho_destroy.argtypes = [C.c_void_p]
         l.ptycho_default_params.argtypes = [C.POINTER(Params)]
         l.ptycho_test_fft2.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
+        l.ptycho_prepare_frames.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float,
+                                            C.c_float, C.c_void_p, C.c_int, C.c_void_p]
         _lib = l
     return _lib
 
@@ -254,6 +256,27 @@ class Ptycho:
             self.destroy()
         except Exception:
             pass
+
+
+def prepare_frames(raw, center, n: int, threshold: float = 0.0, saturation: float = 0.0, out_dtype=np.uint16, out=None):
+    """ptycho_prepare_frames: raw detector frames (F, det_h, det_w), uint16 or float32, numpy or torch CUDA ->
+    FFT-order intensities (F, n, n) with masked pixels as the sentinel.  Marshalling only."""
+    import torch
+    is_t = isinstance(raw, torch.Tensor)
+    itype = lambda dt: 1 if dt in (np.uint16, torch.uint16, np.dtype(np.uint16)) else 0
+    if not is_t:
+        raw = np.ascontiguousarray(raw)
+        assert raw.dtype in (np.uint16, np.float32)
+    f, dh, dw = raw.shape
+    if out is None:
+        out = (torch.empty((f, n, n), dtype=torch.uint16 if itype(out_dtype) else torch.float32, device=raw.device) if is_t
+               else np.empty((f, n, n), np.uint16 if itype(out_dtype) else np.float32))
+    stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+    st = lib().ptycho_prepare_frames(_ptr(raw), itype(raw.dtype), f, dh, dw, int(center[0]), int(center[1]), int(n), float(threshold),
+                                     float(saturation), _ptr(out), itype(out.dtype), C.c_void_p(stream))
+    if st != 0:
+        raise PtychoError(st, "ptycho_prepare_frames")
+    return out
 
 
 def test_fft2(data, inverse: bool = False):

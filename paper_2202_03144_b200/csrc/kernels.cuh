@@ -564,4 +564,42 @@ __global__ void k_finish_init(Scalars* sc, float delta, int J, int which) {
     else { sc->eps_P = delta * (float)J * __uint_as_float(sc->max_bits); }
 }
 
+// ------------------------------------------------------------------------------------------
+// init-time preparation of raw detector frames (include/ptycho_b200.h: ptycho_prepare_frames)
+// ------------------------------------------------------------------------------------------
+template <typename TI, typename TO> __device__ __forceinline__ TO prepare_pixel(const TI* __restrict__ raw, size_t f, int det_h, int det_w, int sy,
+                                                                                 int sx, float threshold, float saturation) {
+    bool masked = sy < 0 || sx < 0 || sy >= det_h || sx >= det_w;
+    float v = 0.f;
+    if (!masked) {
+        v = (float)__ldg(raw + (f * det_h + sy) * det_w + sx);
+        if (sizeof(TI) == 2 && v == 65535.f) masked = true;            // already the sentinel
+        if (sizeof(TI) == 4 && v < 0.f) masked = true;
+        if (saturation > 0.f && v >= saturation) masked = true;
+        if (threshold > 0.f && v < threshold) v = 0.f;
+    }
+    if (sizeof(TO) == 2) return (TO)(masked ? 65535.f : fminf(rintf(v), 65534.f));
+    return (TO)(masked ? -1.0f : v);
+}
+// V output pixels along kx per thread (V = 8 when n % 8 == 0 and `out` is 16-byte aligned: one or two 16-byte
+// stores; the V source pixels are contiguous too, because a group of 8 never straddles kx = n/2), else V = 1.
+template <typename TI, typename TO, int V> __global__ void __launch_bounds__(256) k_prepare_frames(
+    const TI* __restrict__ raw, int det_h, int det_w, int cy, int cx, int n, float threshold, float saturation, TO* __restrict__ out, size_t total) {
+    for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g * V < total; g += (size_t)gridDim.x * blockDim.x) {
+        const size_t i = g * V;
+        const int kx = (int)(i % n), ky = (int)((i / n) % n);
+        const size_t f = i / ((size_t)n * n);
+        const int sy = cy + (ky < n / 2 ? ky : ky - n), sx = cx + (kx < n / 2 ? kx : kx - n);
+        TO v[V];
+#pragma unroll
+        for (int k = 0; k < V; ++k) v[k] = prepare_pixel<TI, TO>(raw, f, det_h, det_w, sy, sx + k, threshold, saturation);
+        if (V == 1) out[i] = v[0];
+        else {
+            const uint4* src = reinterpret_cast<const uint4*>(v);
+#pragma unroll
+            for (int k = 0; k < (int)(V * sizeof(TO) / 16); ++k) reinterpret_cast<uint4*>(out + i)[k] = src[k];
+        }
+    }
+}
+
 }  // namespace ptycho

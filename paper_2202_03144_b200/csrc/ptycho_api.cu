@@ -810,6 +810,36 @@ long long ptycho_launch_count(const ptycho_ctx* c) { return c ? c->launches : 0;
 const char* ptycho_last_error(const ptycho_ctx* c) { return c ? c->err.c_str() : ""; }
 void ptycho_destroy(ptycho_ctx* c) { delete c; }
 
+ptycho_status ptycho_prepare_frames(const void* raw, ptycho_itype raw_type, int n_frames, int det_h, int det_w, int center_y,
+                                    int center_x, int n, float threshold, float saturation, void* out, ptycho_itype out_type,
+                                    void* cuda_stream) {
+    ptycho_ctx* c = nullptr;
+    if (!raw || !out || n_frames < 1 || det_h < 1 || det_w < 1 || n < 2 || (n & 1)) return PTYCHO_EINVAL;
+    if ((raw_type != PTYCHO_I_F32 && raw_type != PTYCHO_I_U16) || (out_type != PTYCHO_I_F32 && out_type != PTYCHO_I_U16)) return PTYCHO_EINVAL;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t in_bytes = (size_t)n_frames * det_h * det_w * (raw_type == PTYCHO_I_U16 ? 2 : 4);
+    const size_t total = (size_t)n_frames * n * n, out_bytes = total * (out_type == PTYCHO_I_U16 ? 2 : 4);
+    const bool dev_in = is_device_ptr(raw), dev_out = is_device_ptr(out);
+    void *d_in = const_cast<void*>(raw), *d_out = out;
+    if (!dev_in) { CU(cudaMalloc(&d_in, in_bytes)); CU(cudaMemcpyAsync(d_in, raw, in_bytes, cudaMemcpyHostToDevice, s)); }
+    if (!dev_out) CU(cudaMalloc(&d_out, out_bytes));
+    const bool vec = (n % 8 == 0) && ((reinterpret_cast<uintptr_t>(d_out) & 15) == 0);
+    const int grid = (int)std::min<size_t>((total / (vec ? 8 : 1) + 255) / 256, (size_t)148 * 64);
+#define PREP(TI, TO) do { if (vec) k_prepare_frames<TI, TO, 8><<<grid, 256, 0, s>>>((const TI*)d_in, det_h, det_w, center_y, center_x, n, threshold, saturation, (TO*)d_out, total); \
+                          else k_prepare_frames<TI, TO, 1><<<grid, 256, 0, s>>>((const TI*)d_in, det_h, det_w, center_y, center_x, n, threshold, saturation, (TO*)d_out, total); } while (0)
+    if (raw_type == PTYCHO_I_U16 && out_type == PTYCHO_I_U16) PREP(unsigned short, unsigned short);
+    else if (raw_type == PTYCHO_I_U16) PREP(unsigned short, float);
+    else if (out_type == PTYCHO_I_U16) PREP(float, unsigned short);
+    else PREP(float, float);
+#undef PREP
+    if (!dev_out) CU(cudaMemcpyAsync(out, d_out, out_bytes, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    CU(cudaGetLastError());
+    if (!dev_in) cudaFree(d_in);
+    if (!dev_out) cudaFree(d_out);
+    return PTYCHO_OK;
+}
+
 __global__ void k_scale(float2* d, size_t n, float s) {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) { d[i].x *= s; d[i].y *= s; }
 }

@@ -327,3 +327,22 @@ def test_cfg4_dm_512_truncated_scan(B, oracle_mod):
     16 384 positions would need 69 GB)."""
     s = synth.make_config(4, n_pos=1024)
     _free_run(B, oracle_mod, s, "DM", 3, dict(pbound=s.params["pbound"]), 3 * TOL_ITER, check_psi=True)
+
+
+# ------------------------------------------------------------------- frame preparation (S:8(f) f2)
+@pytest.mark.parametrize("in_dt,out_dt", [(np.uint16, np.uint16), (np.uint16, np.float32), (np.float32, np.uint16), (np.float32, np.float32)])
+def test_prepare_frames_bit_exact(B, oracle_mod, in_dt, out_dt):
+    """Integer / byte work: the GPU result equals the oracle bit for bit -- centred crop with the window
+    hanging over the detector edge, threshold, saturation, sentinels; host and device pointers."""
+    import torch
+    rng = np.random.default_rng(11)
+    raw = rng.integers(0, 70000, (5, 150, 170)).clip(0, 65535).astype(np.uint16)
+    raw = raw if in_dt == np.uint16 else (raw.astype(np.float32) * 1.37 - 20.0).astype(np.float32)
+    for center, n in (((75, 85), 128), ((10, 160), 64), ((149, 0), 32), ((3, 168), 6)):      # n = 6: the scalar path
+        ref = oracle_mod.prepare_frames(raw, center, n, threshold=300.0, saturation=60000.0, out_dtype=out_dt)
+        got = B.prepare_frames(raw, center, n, threshold=300.0, saturation=60000.0, out_dtype=out_dt)
+        assert got.dtype == ref.dtype and np.array_equal(got, ref), (center, n)
+        got_d = B.prepare_frames(torch.from_numpy(raw).cuda(), center, n, threshold=300.0, saturation=60000.0, out_dtype=out_dt)
+        assert np.array_equal(got_d.cpu().numpy(), ref), (center, n)
+    plain = B.prepare_frames(raw, (75, 85), 64, out_dtype=out_dt)        # no threshold, no saturation
+    assert np.array_equal(plain, oracle_mod.prepare_frames(raw, (75, 85), 64, out_dtype=out_dt))

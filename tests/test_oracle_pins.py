@@ -320,3 +320,27 @@ def test_float_build_tracks_double(oracle_mod):
     d = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities).iterate("DM", 10)
     f = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, precision="f32").iterate("DM", 10)
     assert rel(f.O, d.O) < 1e-4 and rel(f.psi, d.psi) < 1e-4
+
+
+# ------------------------------------------------------------------ frame preparation (S:8(f) f2)
+def test_prepare_frames_hand_example_and_shift_involution(oracle_mod):
+    """6 x 6 detector, n = 4, centre (3, 2): indices worked out by hand from the definition in the header
+    (sy = cy + (ky < n/2 ? ky : ky - n)); out-of-detector pixels masked; threshold zeroes, saturation masks."""
+    raw = (np.arange(36, dtype=np.uint16).reshape(1, 6, 6) * 10)
+    out = oracle_mod.prepare_frames(raw, (3, 2), 4)
+    # ky = 0,1,2,3 -> sy = 3,4,1,2 ; kx = 0,1,2,3 -> sx = 2,3,0,1
+    expect = np.array([[raw[0, sy, sx] for sx in (2, 3, 0, 1)] for sy in (3, 4, 1, 2)], np.uint16)
+    assert np.array_equal(out[0], expect)
+    assert out[0, 0, 0] == raw[0, 3, 2]                                 # the centre pixel is the DC term
+    edge = oracle_mod.prepare_frames(raw, (0, 5), 4)                     # window hangs over two detector edges
+    # ky -> sy = 0,1,-2,-1 ; kx -> sx = 5,6,3,4
+    assert edge[0, 0, 0] == raw[0, 0, 5] and edge[0, 0, 1] == 65535 and edge[0, 2, 0] == 65535 and edge[0, 1, 3] == raw[0, 1, 4]
+    th = oracle_mod.prepare_frames(raw, (3, 2), 4, threshold=185.0, saturation=260.0)
+    assert th[0, 2, 2] == 0 and th[0, 0, 0] == 200 and th[0, 1, 0] == 65535 and th[0, 1, 1] == 65535   # 60 -> 0; 260, 270 saturated
+    f32 = oracle_mod.prepare_frames(raw.astype(np.float32), (3, 2), 4, saturation=260.0, out_dtype=np.float32)
+    assert f32.dtype == np.float32 and f32[0, 1, 0] == -1.0 and f32[0, 0, 0] == 200.0
+    # fftshift of the result is the plain centred crop (involution of the shift for even n)
+    rng = np.random.default_rng(0)
+    big = rng.integers(0, 60000, (3, 40, 50)).astype(np.uint16)
+    o = oracle_mod.prepare_frames(big, (20, 25), 16)
+    assert np.array_equal(np.fft.fftshift(o, axes=(1, 2)), big[:, 12:28, 17:33])

@@ -29,6 +29,7 @@ struct MegaArgs {
     FrameArgs f;        // psi = slot 0 of the store; S = ring base; frames = slot -> caller frame; e_part [J][NCB]
     int J, M, D, R, nW;
     int update_probe;   // accumulate the lagged probe sums (a9) in pass 1
+    int fresh;          // first DM iteration after init / a minibatch algorithm: psi_j = P O_j (R4) is formed here, not read
     int det;            // deterministic mode: no floating-point atomics here (dm_det.cuh forms the overlap sums)
     int pf;             // slots ahead that the L2 prefetches reach (megakernel: M, the next wave; split kernels: the next chunk)
     int flags;          // experiment switches: 1 = no L2 prefetch, 4 = immediate signals
@@ -199,7 +200,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(co
         const float2* prow = a.psi + (size_t)slot * N * N + off;
         float2 v[E];
 #pragma unroll
-        for (int i = 0; i < E; ++i) v[i] = __ldcs(prow + t + T * i);      // psi_j: streamed once
+        for (int i = 0; i < E; ++i) v[i] = m.fresh ? make_float2(0.f, 0.f) : __ldcs(prow + t + T * i);   // psi_j: streamed once
         float2 ov[E];
 #pragma unroll
         for (int i = 0; i < E; ++i) ov[i] = __ldg(orow + t + T * i);
@@ -210,7 +211,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(co
         for (int i = 0; i < E; ++i) {
             const float2 o = ov[i];
             const float2 po = cmul(sP[t + T * i], o);                     // psi_O = P O_j
-            const float2 s = v[i];
+            const float2 s = m.fresh ? po : v[i];                         // R4: the initial exit wave is P O_j
             if (m.update_probe) {
                 accN[i] = cadd(accN[i], cmulc(s, o));                     // conj(O_j) psi_j (lagged, R4)
                 accD[i] = fmaf(o.x, o.x, fmaf(o.y, o.y, accD[i]));

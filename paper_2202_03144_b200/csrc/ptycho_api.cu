@@ -339,11 +339,16 @@ void spatial_sort(std::vector<int>& idx, const int32_t* pos, int n) {
 ptycho_status dm_iteration(ptycho_ctx* c) {
     const size_t nn = (size_t)c->N * c->N, knn = nn * c->K, HW = (size_t)c->H * c->W;
     const int ncb = ncb_of(c->N);
-    if (!c->psi_valid) {
+    // R4: psi_j = P O_j before the first DM iteration.  The plain megakernel forms it on the fly in pass 1 (saves a
+    // 5 GB write and read at config 2); the other forms of the cycle read the store, so it is written first.
+    const bool fresh = !c->psi_valid;
+    const bool fresh_in_kernel = fresh && c->mega_M > 0 && !c->par.deterministic && !env_int("PTYCHO_DM_SPLIT", 0) &&
+                                 !(env_int("PTYCHO_DM_CLUSTER", 0) && c->N <= 256);
+    if (fresh && !fresh_in_kernel) {
         const dim3 g((unsigned)((knn + 255) / 256), c->J);
         LAUNCH(c, PTYCHO_K_OTHER, (k_init_psi<<<g, 256, 0, c->stream>>>(c->psi, c->O, c->W, c->P, c->K, c->N, c->pos, c->dm_frames)));
-        c->psi_valid = true;
     }
+    c->psi_valid = true;
     const int upd = c->t >= c->par.probe_start;
     if (c->mega_M > 0) {
         MegaArgs m{};
@@ -353,6 +358,7 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         const int det = c->par.deterministic;
         m.update_probe = det ? 0 : upd;
         m.det = det;
+        m.fresh = fresh_in_kernel ? 1 : 0;
         if (det && upd) {                                   // lagged probe sums from the incoming psi (R4), fixed order
             LAUNCH(c, PTYCHO_K_OTHER, (k_det_probe<<<dim3((unsigned)((nn + 255) / 256), kDetGroups), 256, 0, c->stream>>>(
                                            c->det_partial, c->psi, c->O, c->W, c->N, c->spos, c->J)));

@@ -344,3 +344,70 @@ def test_prepare_frames_hand_example_and_shift_involution(oracle_mod):
     big = rng.integers(0, 60000, (3, 40, 50)).astype(np.uint16)
     o = oracle_mod.prepare_frames(big, (20, 25), 16)
     assert np.array_equal(np.fft.fftshift(o, axes=(1, 2)), big[:, 12:28, 17:33])
+
+
+# ------------------------------------------------- pins asked for by the round-1 review
+def test_eval_error_off_zero_against_numpy(oracle_mod):
+    """orc_eval_error_num away from the ground truth (R7, C3): sum_j sum_q (sqrt I - sqrt(sum_k |fft2(P_k O_j)|^2))^2
+    / sum I, typed here with numpy's FFT; J = 4, K in {1, 2}, O != truth, one masked pixel per frame."""
+    for k in (1, 2):
+        s, lam = f64_scan(n=8, h=20, side=2, step=4, k=k)
+        cnt = RNG.poisson(lam * 25).astype(np.float64)
+        cnt[:, 2, 5] = -1.0                                                      # masked (R3): excluded from both sums
+        obj = s.obj_true * (1 + 0.3 * crandn(*s.obj_true.shape))
+        p0 = s.probe_true * np.sqrt(25) * (1 + 0.1 * crandn(*s.probe_true.shape))
+        o = oracle_mod.Oracle(obj, p0, s.pos, cnt)
+        n, num, den = s.n, 0.0, 0.0
+        for j, (y, x) in enumerate(s.pos):
+            a = np.sqrt(sum(np.abs(np.fft.fft2(p0[m] * obj[y:y + n, x:x + n])) ** 2 for m in range(k)))
+            ok = cnt[j] >= 0
+            num += np.sum((np.sqrt(cnt[j][ok]) - a[ok]) ** 2)
+            den += np.sum(cnt[j][ok])
+        assert num / den > 1e-3                                                  # really off zero
+        assert o.eval_error() == pytest.approx(num / den, rel=1e-12)
+        assert o.sum_I == pytest.approx(den, rel=1e-14)
+
+
+def test_epie_probe_direction_against_numpy(oracle_mod):
+    """Probe side of the minibatch step (R8): one full-batch ePIE step, alpha_P = 1, delta_probe = 0.37:
+    P_new - P = n_P / (d_P + 0.37 max_r d_P), n_P = sum_j conj(O_j)(revised_j - P O_j), d_P = sum_j |O_j|^2,
+    summed here with numpy slices; K = 2 so that d_P is shared by the modes."""
+    s, lam = f64_scan(n=8, h=20, side=2, step=4, k=2)
+    cnt = RNG.poisson(lam * 30).astype(np.float64)
+    p0 = s.probe_true * np.sqrt(30)
+    obj0 = 1 + 0.2 * crandn(*s.obj_true.shape)
+    o = oracle_mod.Oracle(obj0, p0, s.pos, cnt, dict(delta_probe=0.37, delta_obj=0.61), keep_revised=True)
+    o.iterate("EPIE_MB", 1)
+    n = s.n
+    n_p, d_p = np.zeros_like(p0), np.zeros((n, n))
+    n_o, d_o = np.zeros_like(obj0), np.zeros(obj0.shape)
+    for j, (y, x) in enumerate(s.pos):
+        oj = obj0[y:y + n, x:x + n]
+        chi = o.revised[j] - p0 * oj[None]
+        n_p += np.conj(oj)[None] * chi
+        d_p += np.abs(oj) ** 2
+        n_o[y:y + n, x:x + n] += np.sum(np.conj(p0) * chi, 0)
+        d_o[y:y + n, x:x + n] += np.sum(np.abs(p0) ** 2, 0)
+    assert rel(o.P - p0, n_p / (d_p + 0.37 * d_p.max())[None]) < 1e-12
+    assert rel(o.O - obj0, n_o / (d_o + 0.61 * np.max(np.sum(np.abs(p0) ** 2, 0)))) < 1e-12
+
+
+def test_masked_pixels_are_excluded_from_sum_intensity(oracle_mod):
+    """R3: masked pixels count neither in the error terms nor in sum I.  err[0] * sum(I unmasked) must equal
+    the numpy sum over unmasked pixels; including the masked counts in sum I would fail this."""
+    s, lam = f64_scan(n=8, h=20, side=2, step=4)
+    cnt = np.minimum(RNG.poisson(lam * 400), 65534).astype(np.uint16)
+    cnt[:, 0, 0] = 65535                                                         # the brightest pixel of every frame
+    cnt[1, 3, 4] = 65535
+    p0 = s.probe_true * np.sqrt(400)
+    o = oracle_mod.Oracle(s.obj0, p0, s.pos, cnt, dict(probe_start=10 ** 9))
+    o.iterate("EPIE_MB", 1)
+    ok = cnt < 65535
+    n, num = s.n, 0.0
+    for j, (y, x) in enumerate(s.pos):
+        a = np.abs(np.fft.fft2(p0[0] * s.obj0[y:y + n, x:x + n]))
+        num += np.sum((np.sqrt(cnt[j][ok[j]].astype(float)) - a[ok[j]]) ** 2)
+    unmasked = float(np.sum(cnt[ok].astype(np.float64)))
+    assert o.sum_I == unmasked
+    assert o.err[0] * unmasked == pytest.approx(num, rel=1e-12)
+    assert abs(o.err[0] * float(cnt.astype(np.float64).sum()) - num) > 1e-3 * num   # the wrong denominator is far off

@@ -1,15 +1,18 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the projection cycle (BASELINE.json `metric`).
 
-    python bench.py --gpus N --steps K --warmup W            # this build (CUDA path, C ABI)
+    python bench.py --gpus N --steps K --warmup W            # this build (CUDA path, C ABI), config 2
+    python bench.py --config {1,2,3,4} [--alg DM|EPIE_MB|LSQML]   # the other configurations of BASELINE.json
     python bench.py --impl reference --steps K --warmup W    # the CPU oracle as it stands
+    python bench.py --cufft-ref                              # harness-side reference point: the cycle as unfused torch.fft ops
 
-A "step" is one DM iteration over all J scan positions of config 2 (BASELINE.json configs[2]: DM,
+A "step" is one iteration over all J scan positions.  The default is config 2 (BASELINE.json configs[2]: DM,
 256x256 frames, 10 000 Fermat-spiral positions, 4096^2 object, uint16 Poisson counts) -- the
 configuration the metric "diffraction patterns/sec per DM iteration (256x256, 1 B200)" is quoted
 on.  `value` = J * K / (device time of K iterations), inputs resident in HBM; `e2e` = the same
 through the C ABI from pinned HOST buffers: ptycho_init (H2D of intensities, object, probe,
-positions) + one DM iteration + ptycho_fetch_error, all inside the timed region.
+positions) + one iteration + ptycho_fetch_error, all inside the timed region (that one iteration is the FIRST
+one after init: for DM it forms psi = P O_j inside the kernel instead of reading the exit-wave store).
 N > 1: the path does not shard in this build ("replicas only"): every rank
 reconstructs its own replica scan, no data-path collective; time = max over ranks.
 
@@ -31,9 +34,25 @@ sys.path.insert(0, _ROOT)
 
 METRIC = "diffraction patterns/sec per DM iteration (256x256, 1 B200); % HBM roofline"
 UNIT = "patterns/s"
-CFG = 2                      # BASELINE.json configs[2]
-NCU_DRAM_BYTES_PER_LAUNCH = 14.89e9   # profiles/r01_v4_mega_full_metrics.txt (7.307 GB read + 7.579 GB written)
-REF_SAMPLE = 256             # frames of the bounded oracle sample (first positions of the same scan)
+CFG = 2                      # default: BASELINE.json configs[2]
+DEFAULT_ALG = {1: "EPIE_MB", 2: "DM", 3: "LSQML", 4: "DM"}
+REF_SAMPLE = {1: 256, 2: 256, 3: 96, 4: 64}   # frames of the bounded oracle sample (first positions of the same scan)
+TRAFFIC_FILE = os.path.join(_ROOT, "profiles", "r02_traffic.json")   # ncu dram__bytes per launch of the dominant kernel, per config
+
+
+def ncu_traffic(cfg: int, alg: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu summary
+    (profiles/r02_traffic.json, written from the `ncu --set full` captures named in profiles/r02.md); None if not captured."""
+    try:
+        with open(TRAFFIC_FILE) as f:
+            return json.load(f).get(f"cfg{cfg}_{alg}")
+    except Exception:
+        return None
+
+
+def flops_per_pattern(n: int, k: int) -> float:
+    """nominal K (2 * 10 N^2 log2 N + 40 N^2) (two 2-D transforms of 5 N^2 log2 N^2 flops + point-wise work)."""
+    return k * (2 * 10 * n * n * np.log2(n) + 40 * n * n)
 
 
 def algorithmic_bytes_per_pattern(n: int, k: int, bytes_i: int) -> int:

@@ -16,11 +16,14 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
-LIB_PATH = os.environ.get("PTYCHO_B200_LIB") or os.path.join(_CSRC, "libptycho_b200.so")   # override: a debug build
+# Development only: PTYCHO_BUILD_ONLY_N=256 compiles one frame size into a separate file (a quarter of the build time);
+# the product library always holds all four sizes.
+_ONLY_N = os.environ.get("PTYCHO_BUILD_ONLY_N")
+LIB_PATH = os.environ.get("PTYCHO_B200_LIB") or os.path.join(_CSRC, f"libptycho_dev{_ONLY_N}.so" if _ONLY_N else "libptycho_b200.so")
 ALG = {"EPIE_MB": 0, "DM": 1, "LSQML": 2}
 KCLASS = ["rows_fwd", "cols", "rows_inv", "update", "other", "mega"]   # ptycho_kclass
 STATUS = ["OK", "EINVAL", "EBOUNDS", "EUNSUPPORTED", "ENOMEM", "ECUDA", "ESTATE"]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+NVCC_FLAGS = ["--threads", "0", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "128"]
 
 
@@ -40,11 +43,12 @@ class Params(C.Structure):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """nvcc the CUDA library in-tree for sm_100a (cross-compiles without a GPU)."""
-    srcs = [os.path.join(_CSRC, f) for f in ("ptycho_api.cu", "kernels.cuh", "fft_core.cuh", "dm_mega.cuh", "dm_det.cuh", "dm_cluster.cuh")]
+    srcs = [os.path.join(_CSRC, f) for f in ("ptycho_api.cu", "kernels.cuh", "fft_core.cuh", "dm_mega.cuh", "dm_det.cuh")]
     srcs.append(os.path.join(os.path.dirname(_HERE), "include", "ptycho_b200.h"))
     if not force and os.path.exists(LIB_PATH) and all(os.path.getmtime(LIB_PATH) >= os.path.getmtime(s) for s in srcs):
         return LIB_PATH
-    cmd = ["nvcc", *NVCC_FLAGS, *( ["-Xptxas", "-v"] if verbose else []), srcs[0], "-o", LIB_PATH]
+    cmd = ["nvcc", *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), *([f"-DPTYCHO_ONLY_N={_ONLY_N}"] if _ONLY_N else []), *os.environ.get("PTYCHO_BUILD_DEFS", "").split(),
+           srcs[0], "-o", LIB_PATH]
     subprocess.check_call(cmd, cwd=_CSRC)
     return LIB_PATH
 

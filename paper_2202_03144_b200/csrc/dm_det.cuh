@@ -88,4 +88,63 @@ __global__ void __launch_bounds__(kDetTileW * kDetTileH) k_det_object(float2* __
     }
 }
 
+// a10 for the DM megakernel (dm_mega.cuh), which scatters only the CORRECTION term of the object sum:
+// with psi'_j = P O_j + keep_j v_j (v_j = F^-1[(s - 1) Phi_j], keep_j = 1 - rb_j of the relaxed projection, R6),
+//     n_O(q) = sum_j conj(P) psi'_j = d_O(q) O(q) + c(q),   c(q) = sum_j keep_j conj(P(q - r_j)) v_j(q - r_j),
+// so the blended division of R5 becomes  O <- (n_O + eps O)/(d_O + eps) = O + c / (d_O + eps)  -- the same value, and frames whose
+// error is already inside the power bound (keep_j = 0) add nothing.  d_O(q) = sum_j |P(q - r_j)|^2 depends only on the probe and
+// the positions: it is gathered HERE over the tile's frame list instead of being scatter-added with one atomic per pixel and frame.
+// Also zeroes c.
+// |P|^2 table of the current probe; block 0 also rolls the megakernel's statistic: stat[0] <- frames inside the power bound in
+// the iteration just run, stat[1] <- 0.
+__global__ void __launch_bounds__(1024) k_probe_support(float* __restrict__ p2, const float2* __restrict__ P, int n, int* stat) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < n * n) { const float2 v = P[q]; p2[q] = fmaf(v.x, v.x, v.y * v.y); }
+    if (q == 0 && stat) { stat[0] = stat[1]; stat[1] = 0; }
+}
+
+// tile_start / tile_mid / tile_list: per 32 x 8 object tile, the packed positions (y << 16 | x) of the frames that overlap it,
+// those covering the whole tile first ([tile_start, tile_mid)), then the partial ones ([tile_mid, tile_start[tile + 1])); each
+// group in ascending slot order, so the sum has one fixed order.
+__global__ void __launch_bounds__(kDetTileW * kDetTileH) k_dm_blend_gather(float2* __restrict__ O, float2* __restrict__ cO, int H, int W,
+                                                                            const float* __restrict__ p2, int n, const int* __restrict__ tile_start,
+                                                                            const int* __restrict__ tile_mid, const int* __restrict__ tile_list,
+                                                                            const Scalars* __restrict__ sc) {
+    constexpr int NT = kDetTileW * kDetTileH;
+    __shared__ int s_off[NT];
+    const int tile = blockIdx.y * gridDim.x + blockIdx.x, tid = threadIdx.y * kDetTileW + threadIdx.x;
+    const int qx = blockIdx.x * kDetTileW + threadIdx.x, qy = blockIdx.y * kDetTileH + threadIdx.y;
+    const int e0 = tile_start[tile], em = tile_mid[tile], e1 = tile_start[tile + 1];
+    const float* pb = p2 + qy * n + qx;
+    float d0 = 0.f, d1 = 0.f, d2 = 0.f, d3 = 0.f;
+    for (int c0 = e0; c0 < em; c0 += NT) {                           // frames covering the whole tile: no per-pixel test, four loads in flight
+        const int nc = min(NT, em - c0);
+        __syncthreads();
+        if (tid < nc) { const int v = tile_list[c0 + tid]; s_off[tid] = (v >> 16) * n + (v & 0xffff); }
+        __syncthreads();
+        int e = 0;
+        for (; e + 4 <= nc; e += 4) {
+            d0 += __ldg(pb - s_off[e]); d1 += __ldg(pb - s_off[e + 1]); d2 += __ldg(pb - s_off[e + 2]); d3 += __ldg(pb - s_off[e + 3]);
+        }
+        for (; e < nc; ++e) d0 += __ldg(pb - s_off[e]);
+    }
+    for (int c0 = em; c0 < e1; c0 += NT) {                           // frames covering part of it
+        const int nc = min(NT, e1 - c0);
+        __syncthreads();
+        if (tid < nc) s_off[tid] = tile_list[c0 + tid];
+        __syncthreads();
+        for (int e = 0; e < nc; ++e) {
+            const int y = qy - (s_off[e] >> 16), x = qx - (s_off[e] & 0xffff);
+            if (y >= 0 && y < n && x >= 0 && x < n) d1 += __ldg(p2 + y * n + x);
+        }
+    }
+    const float d = (d0 + d1) + (d2 + d3);
+    if (qy >= H || qx >= W) return;
+    const size_t i = (size_t)qy * W + qx;
+    const float inv = 1.0f / (d + sc->eps_O);
+    const float2 c = cO[i], o = O[i];
+    O[i] = make_float2(fmaf(c.x, inv, o.x), fmaf(c.y, inv, o.y));
+    cO[i] = make_float2(0.f, 0.f);
+}
+
 }  // namespace ptycho

@@ -30,6 +30,7 @@ struct MegaArgs {
     int J, M, D, R, nW;
     int update_probe;   // accumulate the lagged probe sums (a9) in pass 1
     int fresh;          // first DM iteration after init / a minibatch algorithm: psi_j = P O_j (R4) is formed here, not read
+    int corr;           // object canvas holds only the correction sum_j keep_j conj(P) v_j; d_O is gathered by k_dm_blend_gather (dm_det.cuh)
     int det;            // deterministic mode: no floating-point atomics here (dm_det.cuh forms the overlap sums)
     int pf;             // slots ahead that the L2 prefetches reach (megakernel: M, the next wave; split kernels: the next chunk)
     int flags;          // experiment switches: 1 = no L2 prefetch, 4 = immediate signals
@@ -38,6 +39,8 @@ struct MegaArgs {
     int* head;          // queue head
     int* cnt1;          // [J] pass-1 blocks done per slot
     int* cnt2;          // [J] pass-2 blocks done
+    int* cnt2a;         // [J] split mode: error-only column blocks done (pass 2a)
+    int* stat;          // [0] frames inside the power bound in the PREVIOUS iteration, [1] running count of this one
     int* cnt3;          // [J] pass-3 blocks done
 };
 
@@ -66,7 +69,6 @@ __device__ __forceinline__ void slot_wait(const int* cnt, int target) {
 // consumer polls with a relaxed load and then reads the producer's data only through ld.global.cg
 // (L2, the point of coherence); the producer orders its st.global.cg writes before the counter
 // increment with the release.  The poll's result is a control dependency of every later load.
-__device__ int g_nowait;   // debug: ignore the flags (racy; timing experiments only)
 __device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
     int v;
     asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -85,7 +87,7 @@ __device__ __forceinline__ void warp_signal_relaxed(int* cnt) {
 }
 __device__ __forceinline__ void warp_wait(const int* cnt, int target) {
     if ((threadIdx.x & 31) == 0) {
-        while (ld_relaxed_gpu(cnt) < target && !g_nowait) __nanosleep(64);
+        while (ld_relaxed_gpu(cnt) < target) __nanosleep(64);
     }
     __syncwarp();
 }
@@ -152,7 +154,7 @@ template <int N, typename TI> __global__ void __launch_bounds__(kThreads) k_tile
                                                                                             const int* __restrict__ frames) {
     using G = Geo<N>;
     constexpr int E = G::E, CB = G::LPB, EPC = 16 / (int)sizeof(TI);
-    const int slot = blockIdx.y, blk = blockIdx.x, tid = threadIdx.x;
+    const int slot = blockIdx.x, blk = blockIdx.y, tid = threadIdx.x;
     const int c = tid % CB, t = tid / CB;
     const TI* src = I + (size_t)frames[slot] * N * N + blk * CB + c;
     TI* dst = out + ((size_t)slot * G::NCB + blk) * N * CB;
@@ -238,7 +240,11 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(co
 }
 
 // ---- pass 2: a3 column FFTs, a4 error partial, a5 modulus projection (as s - 1), a6 inverse columns
-template <int N, bool U16, bool SYNC = true> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
+// MODE 0: the whole pass (fused form).  Split form, used when most frames were inside the power bound in the previous iteration (R6:
+// their projection is the identity, so nothing has to be transformed back): MODE 1 = pass 2a, column FFTs and error partials only,
+// S is left untouched; MODE 2 = pass 2b, the whole pass again, but only for the frames whose error turned out to exceed the bound.
+enum { P2_FUSED = 0, P2_ERR_ONLY = 1, P2_IF_NEEDED = 2 };
+template <int N, bool U16, int MODE, bool SYNC = true> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
                                                             float* s_red, Deferred& df) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T, CB = G::LPB;
@@ -257,7 +263,18 @@ template <int N, bool U16, bool SYNC = true> __device__ __forceinline__ void meg
     PhaseClock pc;
     for (int slot = s_begin; slot < s_end; ++slot) {
         pc.start(1);
-        if (SYNC) warp_wait(m.cnt1 + slot, G::NCB * kWarps);
+        if (MODE == P2_IF_NEEDED) {
+            warp_wait(m.cnt2a + slot, G::NCB);                              // every error partial of the frame is there
+            float e = 0.f;
+            for (int i = 0; i < G::NCB; ++i) e += __ldcg(a.e_part + (size_t)slot * G::NCB + i);
+            e *= 1.0f / ((float)N * (float)N);
+            if (e <= a.pbound) {                                            // inside the bound: pass 3 needs nothing from S
+                __syncthreads();
+                df.flush_cta_after_barrier();
+                df.cnt = m.cnt2 + slot;
+                continue;
+            }
+        } else if (SYNC) warp_wait(m.cnt1 + slot, G::NCB * kWarps);
         pc.lap(0);
         float2* base = a.S + (size_t)(slot % m.R) * N * N + col;
         float2 v[E];
@@ -299,13 +316,18 @@ template <int N, bool U16, bool SYNC = true> __device__ __forceinline__ void meg
         for (int s = 16; s > 0; s >>= 1) err += __shfl_xor_sync(0xffffffffu, err, s);
         if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = err;
         __syncthreads();                                                    // sx free again; s_red visible
-        fft_line_inv<N>(v, t, sx, s_tw + N);
+        if (MODE != P2_ERR_ONLY) fft_line_inv<N>(v, t, sx, s_tw + N);
         if (threadIdx.x == 0) {
             float tot = 0.f;
             for (int w = 0; w < kThreads / 32; ++w) tot += s_red[w];        // fixed order
             a.e_part[(size_t)slot * G::NCB + blk] = tot;
         }
         pc.lap(2);
+        if (MODE == P2_ERR_ONLY) {
+            __syncthreads();                                                // s_red free; e_part written
+            df.cnt = m.cnt2a + slot;
+            continue;
+        }
 #pragma unroll
         for (int r = 0; r < E; ++r) __stcg(base + (size_t)pos_a_inv<N>(t, r) * N, v[r]);
         __syncthreads();                                                    // sx and s_red free; stores issued by all
@@ -335,10 +357,6 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
         pc.start(2);
         if (SYNC) warp_wait(m.cnt2 + slot, G::NCB);
         pc.lap(0);
-        const float2* srow = a.S + (size_t)(slot % m.R) * N * N + off;
-        float2 v[E];
-#pragma unroll
-        for (int r = 0; r < E; ++r) v[r] = __ldcg(srow + freq_b<N>(t, r));
         const YX p0 = m.spos[slot];
         float keep = 1.f;                                                   // 1 - rb  (R6)
         if (a.pbound > 0.f) {
@@ -348,6 +366,23 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
             keep = (e <= a.pbound) ? 0.f : 1.f - sqrtf(a.pbound / e);
         }
         const size_t obase = (size_t)(p0.y + y) * a.W + p0.x;
+        float2* prow = a.psi + (size_t)slot * N * N + off;
+        if (m.corr && blk == 0 && threadIdx.x == 0 && keep == 0.f) atomicAdd(m.stat + 1, 1);   // statistic for the next iteration's form
+        if (m.corr && keep == 0.f) {
+            // The frame's error is inside the power bound (R6: rb = 1): the relaxed projection is the identity, psi' = P O_j, and the
+            // frame adds nothing to the object correction (dm_det.cuh k_dm_blend_gather).  S[slot] is not read, nothing is transformed.
+            if (SYNC) warp_signal_relaxed(m.cnt3 + slot);
+#pragma unroll
+            for (int i = 0; i < E; ++i) {
+                const int x = t + T * i;
+                __stcs(prow + x, cmul(sP[x], __ldg(a.O + obase + x)));
+            }
+            continue;
+        }
+        const float2* srow = a.S + (size_t)(slot % m.R) * N * N + off;
+        float2 v[E];
+#pragma unroll
+        for (int r = 0; r < E; ++r) v[r] = __ldcg(srow + freq_b<N>(t, r));
         float2 o[E];                                                        // O_j: in flight during the butterflies
 #pragma unroll
         for (int r = 0; r < E; ++r) o[r] = __ldg(a.O + obase + pos_a_inv<N>(t, r));
@@ -357,17 +392,20 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
         __syncwarp();                                                       // sx is free for the next slot
         pc.lap(2);
         if (SYNC) warp_signal_relaxed(m.cnt3 + slot);                       // S[slot] has been read: the ring slot may be refilled
-        float2* prow = a.psi + (size_t)slot * N * N + off;
 #pragma unroll
         for (int r = 0; r < E; ++r) {
             const int x = pos_a_inv<N>(t, r);
             const float2 p = sP[x];
             const float2 po = cmul(p, o[r]);
-            const float2 w = make_float2(fmaf(keep, v[r].x, po.x), fmaf(keep, v[r].y, po.y));   // a7
+            const float2 kv = make_float2(keep * v[r].x, keep * v[r].y);
+            const float2 w = cadd(po, kv);                                  // a7
             __stcs(prow + x, w);
             if (!m.det) {
-                red_add(a.nO + obase + x, cmulc(w, p));                     // a8 conj(P) psi_j
-                red_add(a.dO + obase + x, fmaf(p.x, p.x, p.y * p.y));
+                if (m.corr) red_add(a.nO + obase + x, cmulc(kv, p));        // a8, correction term only: keep conj(P) v
+                else {
+                    red_add(a.nO + obase + x, cmulc(w, p));                 // a8 conj(P) psi_j
+                    red_add(a.dO + obase + x, fmaf(p.x, p.x, p.y * p.y));
+                }
             }
         }
         pc.lap(3);
@@ -381,8 +419,11 @@ template <int N, bool U16> __global__ void __launch_bounds__(kThreads, (N >= 512
     __shared__ float s_red[kThreads / 32];
     __shared__ int s_item;
     load_tw(s_tw, m.f.tw, m.f.twi, N);
-    const int per_qw = 3 * G::NCB;
-    const int total = (m.nW + 2 * m.D) * per_qw;
+    // split form when most frames were inside the power bound last time (their projection is the identity)
+    const bool split = m.corr && m.f.pbound > 0.f && 2 * m.stat[0] > m.J;
+    const int nk = split ? 4 : 3;                             // item kinds per queue wave
+    const int per_qw = nk * G::NCB;
+    const int total = (m.nW + (nk - 1) * m.D) * per_qw;
     Deferred df;
     bool df_cta = false;                                      // the pending signal is a CTA-level one (pass 2)
 #ifdef PTYCHO_PHASE_PROF
@@ -401,38 +442,20 @@ template <int N, bool U16> __global__ void __launch_bounds__(kThreads, (N >= 512
         const int q = s_item;
         if (q >= total) break;
         const int qw = q / per_qw, idx = q % per_qw;
-        const int kind = idx / G::NCB, blk = idx % G::NCB;    // 0: pass 3, 1: pass 2, 2: pass 1
-        const int wave = qw - (2 - kind) * m.D;
+        const int kind = idx / G::NCB, blk = idx % G::NCB;    // fused: 0 pass 3, 1 pass 2, 2 pass 1; split: 0 pass 3, 1 pass 2b, 2 pass 2a, 3 pass 1
+        const int wave = qw - (nk - 1 - kind) * m.D;
         if (wave < 0 || wave >= m.nW) continue;
-        if ((m.flags >> 8) & (1 << kind)) continue;               // debug: skip pass kinds (0x100 pass 3, 0x200 pass 2, 0x400 pass 1)
-        df_cta = kind == 1;
-        if (kind == 2) mega_pass1<N>(m, blk, wave, sm, s_tw, df);
-        else if (kind == 1) mega_pass2<N, U16>(m, blk, wave, sm, s_tw, s_red, df);
-        else mega_pass3<N>(m, blk, wave, sm, s_tw, df);
+        df_cta = kind == 1 || (split && kind == 2);
+        if (kind == nk - 1) mega_pass1<N>(m, blk, wave, sm, s_tw, df);
+        else if (kind == 0) mega_pass3<N>(m, blk, wave, sm, s_tw, df);
+        else if (!split) mega_pass2<N, U16, P2_FUSED>(m, blk, wave, sm, s_tw, s_red, df);
+        else if (kind == 2) mega_pass2<N, U16, P2_ERR_ONLY>(m, blk, wave, sm, s_tw, s_red, df);
+        else mega_pass2<N, U16, P2_IF_NEEDED>(m, blk, wave, sm, s_tw, s_red, df);
     }
 #ifdef PTYCHO_PHASE_PROF
     __syncthreads();
     if (threadIdx.x < 16) atomicAdd(&g_phase[threadIdx.x], s_phase[threadIdx.x]);
 #endif
-}
-
-// ---- the same three passes as stream-ordered kernels over one chunk of waves -----------------------
-// grid (NCB, waves of the chunk); no flags: the stream orders pass 1 -> 2 -> 3 of a chunk, and each
-// kernel gets the register budget (hence the resident warps) of its own pass instead of the
-// megakernel's maximum over all three.  S holds the chunk (slot % R).
-template <int N, bool U16, int KIND>
-__global__ void __launch_bounds__(kThreads, (N >= 512 ? 1 : (KIND == 2 ? 2 : 3))) k_dm_pass(MegaArgs m, int wave0) {
-    using G = Geo<N>;
-    extern __shared__ __align__(16) float2 sm[];
-    float4* s_tw = reinterpret_cast<float4*>(sm + G::LPB * MegaGeo<N>::LINE);
-    __shared__ float s_red[kThreads / 32];
-    load_tw(s_tw, m.f.tw, m.f.twi, N);
-    __syncthreads();
-    Deferred df;
-    const int blk = blockIdx.x, wave = wave0 + blockIdx.y;
-    if (KIND == 2) mega_pass1<N, false>(m, blk, wave, sm, s_tw, df);
-    else if (KIND == 1) mega_pass2<N, U16, false>(m, blk, wave, sm, s_tw, s_red, df);
-    else mega_pass3<N, false>(m, blk, wave, sm, s_tw, df);
 }
 
 }  // namespace ptycho

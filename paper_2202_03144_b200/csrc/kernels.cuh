@@ -225,7 +225,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_cols(Fr
         if (in >= 0.f) {
             const float sq = sqrtf(in), d = sq - amp;
             err = fmaf(d, d, err);
-            if (amp > 0.f) scale[r] = sq / amp * inv_n2;
+            if (amp2[r] > 1e-30f) scale[r] = sq / amp * inv_n2;   // R2 threshold shared with dm_mega.cuh: below it |Phi| counts as 0
             else { scale[r] = -sq * inv_n2; zero_amp = true; }   // R2: flagged by the sign
         } else scale[r] = inv_n2;                                 // R3: masked, keep Phi
     }
@@ -348,11 +348,11 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_in
 // ------------------------------------------------------------------------------------------
 // small element-wise / reduction kernels (a10, a11)
 // ------------------------------------------------------------------------------------------
-// psi_j = P O_j for every slot (R4 initial exit waves).  grid (N*N*K / 256, nslots)
+// psi_j = P O_j for every slot (R4 initial exit waves).  grid (nslots, N*N*K / 256)
 __global__ void k_init_psi(float2* psi, const float2* __restrict__ O, int W, const float2* __restrict__ P, int K,
                            int n, const YX* __restrict__ pos, const int* __restrict__ frames) {
-    const int slot = blockIdx.y;
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;   // over K*n*n
+    const int slot = blockIdx.x;
+    const size_t i = (size_t)blockIdx.y * blockDim.x + threadIdx.x;   // over K*n*n
     const size_t nn = (size_t)n * n;
     if (i >= nn * K) return;
     const size_t q = i % nn;
@@ -545,18 +545,32 @@ __global__ void k_finish_sum_I(const double* part, int n, Scalars* sc) {
     double s = 0; for (int i = 0; i < n; ++i) s += part[i];
     sc->sum_I = s;
 }
-// E_t = (sum of all error partials, fixed order, double) / sum_I.  single CTA of 1024 threads.
-__global__ void k_sum_error(const float* __restrict__ e_part, size_t count, const Scalars* sc, double* out) {
+// E_t = (sum of all error partials, fixed order, double) / sum_I.  Two steps, both in a fixed order: kErrBlocks CTAs each
+// reduce a contiguous piece to part[block]; the last CTA to finish (atomic ticket) adds the pieces in index order.
+constexpr int kErrBlocks = 148;
+__global__ void __launch_bounds__(1024) k_sum_error(const float* __restrict__ e_part, size_t count, const Scalars* sc, double* out, double* part,
+                                                    unsigned int* ticket) {
     __shared__ double sa[32];
+    __shared__ bool last;
+    const size_t per = (count + gridDim.x - 1) / gridDim.x, i0 = blockIdx.x * per, i1 = min(count, i0 + per);
     double acc = 0.0;
-    for (size_t i = threadIdx.x; i < count; i += blockDim.x) acc += (double)e_part[i];
+    for (size_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) acc += (double)e_part[i];
     for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
     if ((threadIdx.x & 31) == 0) sa[threadIdx.x >> 5] = acc;
     __syncthreads();
     if (threadIdx.x == 0) {
         for (int w = 1; w < (int)blockDim.x / 32; ++w) acc += sa[w];
-        *out = acc / (sc->sum_I > 0 ? sc->sum_I : 1.0);
+        part[blockIdx.x] = acc;
+        __threadfence();
+        last = atomicAdd(ticket, 1u) == gridDim.x - 1;
     }
+    __syncthreads();
+    if (!last || threadIdx.x) return;
+    __threadfence();
+    double tot = 0.0;
+    for (unsigned b = 0; b < gridDim.x; ++b) tot += __ldcg(part + b);
+    *out = tot / (sc->sum_I > 0 ? sc->sum_I : 1.0);
+    *ticket = 0;
 }
 __global__ void k_finish_init(Scalars* sc, float delta, int J, int which) {
     if (threadIdx.x || blockIdx.x) return;

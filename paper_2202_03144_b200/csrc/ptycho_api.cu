@@ -18,7 +18,6 @@
 #include "kernels.cuh"
 #include "dm_mega.cuh"
 #include "dm_det.cuh"
-#include "dm_cluster.cuh"
 
 using namespace ptycho;
 
@@ -52,7 +51,7 @@ struct ptycho_ctx {
     float *dO = nullptr, *dP = nullptr, *e_part = nullptr, *e_tmp = nullptr;
     float2 *tw = nullptr, *twi = nullptr;
     YX* pos = nullptr;
-    int *tile_start = nullptr, *tile_list = nullptr;   // deterministic mode: frames per object tile (CSR, slot order)
+    int *tile_start = nullptr, *tile_mid = nullptr, *tile_list = nullptr;   // frames per object tile (CSR; see ptycho_init)
     float4* det_partial = nullptr;
     int det_tx = 0, det_ty = 0;
     void* It = nullptr;                        // intensities re-tiled for the DM megakernel
@@ -66,6 +65,10 @@ struct ptycho_ctx {
     // DM megakernel (dm_mega.cuh): frames per wave, wave lag between passes, ring slots, grid
     int mega_M = 0, mega_D = 0, mega_R = 0, mega_grid = 0;
     int* mega_ctr = nullptr;                   // device: [head | pad to 64 ints | cnt1[J] | cnt2[J] | cnt3[J]]
+    float* p2 = nullptr;                       // |P|^2 of the current probe (d_O gather, dm_det.cuh)
+    double* err_part = nullptr; unsigned int* err_ticket = nullptr;   // k_sum_error: per-CTA pieces and the finishing ticket
+    int* dm_stat = nullptr;                    // [0] frames inside the power bound in the previous DM iteration, [1] running count
+    int sms = 148;
     std::vector<int> dm_order;                 // slot -> caller frame
     std::vector<int> slot_of_h;                // caller frame -> slot
     std::vector<int> mb_offsets;               // batch b = mb_frames[mb_offsets[b] .. mb_offsets[b+1])
@@ -112,7 +115,31 @@ struct Timed {
 };
 #define LAUNCH(c, cls, ...) do { Timed t_(c, cls); __VA_ARGS__; } while (0)
 
-bool valid_n(int n) { return n == 64 || n == 128 || n == 256 || n == 512; }
+// Frame-size dispatch.  A development build may compile ONE size only (-DPTYCHO_ONLY_N=256: a quarter of the build
+// time); the product build (PTYCHO_ONLY_N undefined or 0) instantiates all four.
+#ifndef PTYCHO_ONLY_N
+#define PTYCHO_ONLY_N 0
+#endif
+#define PTYCHO_HAS_N(n) (PTYCHO_ONLY_N == 0 || PTYCHO_ONLY_N == (n))
+template <int V> struct IntC { static constexpr int value = V; };
+template <class F> void dispatch_n(int n, F&& f) {
+    switch (n) {
+#if PTYCHO_HAS_N(64)
+        case 64: f(IntC<64>{}); break;
+#endif
+#if PTYCHO_HAS_N(128)
+        case 128: f(IntC<128>{}); break;
+#endif
+#if PTYCHO_HAS_N(256)
+        case 256: f(IntC<256>{}); break;
+#endif
+#if PTYCHO_HAS_N(512)
+        case 512: f(IntC<512>{}); break;
+#endif
+        default: break;
+    }
+}
+bool valid_n(int n) { return (n == 64 || n == 128 || n == 256 || n == 512) && PTYCHO_HAS_N(n); }
 
 int chunk_frames(int n, int K, int J) {
     double mb = 64.0;
@@ -145,19 +172,17 @@ void mega_config(ptycho_ctx* c) {
     int M = std::max(1, std::min(env_int("PTYCHO_MEGA_M", 4), c->J));
     // 48 MB keeps the ring resident in L2 (config 2: 1.26 x algorithmic DRAM traffic; at 64 MB it is 2 % faster but
     // the ring is written back: 1.73 x); 512^2 frames need 64 MB for two slots per item (config 4: 86.9 -> 74.8 ms)
-    const double ring_mb = env_int("PTYCHO_MEGA_RING_MB", c->N >= 512 ? 64 : 48);
-    while (M > 1 && (double)(2 * c->mega_D + 1 + X) * M * c->N * c->N * 8.0 > ring_mb * 1048576.0) --M;
+    // The split form of the queue (dm_mega.cuh) puts three lags between pass 1 and pass 3 of a frame, so the ring spans 3 D + 1 + X waves.
+    const double ring_mb = env_int("PTYCHO_MEGA_RING_MB", c->N >= 512 ? 96 : 64);
+    while (M > 1 && (double)(3 * c->mega_D + 1 + X) * M * c->N * c->N * 8.0 > ring_mb * 1048576.0) --M;
     c->mega_M = M;
-    c->mega_R = (2 * c->mega_D + 1 + X) * M;
+    c->mega_R = (3 * c->mega_D + 1 + X) * M;
 }
 
 size_t cols_smem(int n, int K) {
-    switch (n) {
-        case 64: return Geo<64>::smem_cols(K);
-        case 128: return Geo<128>::smem_cols(K);
-        case 256: return Geo<256>::smem_cols(K);
-        default: return Geo<512>::smem_cols(K);
-    }
+    size_t r = 0;
+    dispatch_n(n, [&](auto nn) { r = Geo<decltype(nn)::value>::smem_cols(K); });
+    return r;
 }
 int ncb_of(int n) { return n == 64 ? Geo<64>::NCB : n == 128 ? Geo<128>::NCB : n == 256 ? Geo<256>::NCB : Geo<512>::NCB; }
 
@@ -166,13 +191,16 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
     Carver w(base);
     const size_t HW = (size_t)c->H * c->W, nn = (size_t)c->N * c->N, knn = nn * c->K;
     c->O = w.take<float2>(HW);
+    const bool want_corr = c->mega_M > 0 && !c->par.deterministic;   // object canvas = correction term, d_O gathered (dm_det.cuh)
+    c->p2 = want_corr ? w.take<float>(nn) : nullptr;
+    c->dm_stat = w.take<int>(2);
     c->P = w.take<float2>(knn);
     c->nO = w.take<float2>(HW);
     c->dO = w.take<float>(HW);
     c->nP = w.take<float2>(knn);
     c->dP = w.take<float>(nn);
     c->S = w.take<float2>((size_t)std::max(c->chunk, c->mega_R) * knn);
-    c->mega_ctr = w.take<int>(64 + 3 * (size_t)c->J);
+    c->mega_ctr = w.take<int>(64 + 4 * (size_t)c->J);
     c->e_part = w.take<float>((size_t)c->J * ncb_of(c->N));
     c->e_tmp = w.take<float>((size_t)c->J * ncb_of(c->N));
     c->tw = w.take<float2>(c->N);
@@ -190,13 +218,16 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
     c->partP = w.take<double>(2 * kRedBlocks);
     c->partX = w.take<double>((size_t)c->J * kCrossParts);
     c->scratch_d = w.take<double>(kRedBlocks);
+    c->err_part = w.take<double>(kErrBlocks);
+    c->err_ticket = w.take<unsigned int>(1);
     if (!c->par.disable_dm) c->psi = w.take<float2>((size_t)c->J * knn);
     c->It = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
-    if (c->par.deterministic) {
+    if (c->par.deterministic || want_corr) {                 // frames per object tile: deterministic mode, and the d_O gather
         c->det_tx = (c->W + kDetTileW - 1) / kDetTileW; c->det_ty = (c->H + kDetTileH - 1) / kDetTileH;
         c->tile_start = w.take<int>((size_t)c->det_tx * c->det_ty + 1);
+        c->tile_mid = w.take<int>((size_t)c->det_tx * c->det_ty);
         c->tile_list = w.take<int>((size_t)c->J * (c->N / kDetTileW + 1) * (c->N / kDetTileH + 1));   // upper bound
-        c->det_partial = w.take<float4>((size_t)kDetGroups * nn);
+        if (c->par.deterministic) c->det_partial = w.take<float4>((size_t)kDetGroups * nn);
     }
     if (copy_I) c->I = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
     return (w.off + 255) & ~size_t(255);
@@ -224,17 +255,12 @@ template <int N> ptycho_status set_attrs(ptycho_ctx* c) {
     CU(cudaFuncSetAttribute(k_cols<N, CM_PLAIN_INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
     CU(cudaFuncSetAttribute(k_dm_mega<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
     CU(cudaFuncSetAttribute(k_dm_mega<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
-    CU(cudaFuncSetAttribute(k_dm_pass<N, true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
-    CU(cudaFuncSetAttribute(k_dm_pass<N, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
-    CU(cudaFuncSetAttribute(k_dm_pass<N, true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
-    CU(cudaFuncSetAttribute(k_dm_pass<N, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
-    CU(cudaFuncSetAttribute(k_dm_pass<N, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
-    CU(cudaFuncSetAttribute(k_dm_pass<N, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MegaGeo<N>::smem));
     int per_sm = 0, dev = 0, sms = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_dm_mega<N, true>, kThreads, MegaGeo<N>::smem));
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     c->mega_grid = std::max(1, per_sm) * sms;
+    c->sms = sms;
     return PTYCHO_OK;
 }
 
@@ -283,46 +309,7 @@ template <int N> void launch_passes(ptycho_ctx* c, const FrameArgs& a, int nfram
 }
 
 void passes(ptycho_ctx* c, const FrameArgs& a, int nframes, int fwd, int col, int inv) {
-    switch (c->N) {
-        case 64: launch_passes<64>(c, a, nframes, fwd, col, inv); break;
-        case 128: launch_passes<128>(c, a, nframes, fwd, col, inv); break;
-        case 256: launch_passes<256>(c, a, nframes, fwd, col, inv); break;
-        default: launch_passes<512>(c, a, nframes, fwd, col, inv); break;
-    }
-}
-
-// One cluster of NCB CTAs per frame (dm_cluster.cuh).  N <= 256 only (a cluster holds at most 16 CTAs).
-template <int N, bool U16> ptycho_status launch_cluster(ptycho_ctx* c, ClusterArgs m) {
-    auto kern = k_dm_cluster<N, U16>;
-    const size_t smem = ClusterGeo<N>::smem;
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-    cudaLaunchConfig_t cfg{};
-    cudaLaunchAttribute at{};
-    at.id = cudaLaunchAttributeClusterDimension;
-    at.val.clusterDim.x = Geo<N>::NCB; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
-    cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream; cfg.attrs = &at; cfg.numAttrs = 1;
-    cfg.gridDim = dim3(Geo<N>::NCB);
-    int ncl = 0;
-    CU(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
-    if (ncl < 1) return fail(c, PTYCHO_EUNSUPPORTED, "no cluster of this size fits on the device");
-    ncl = std::min(std::min(ncl, c->J), std::max(1, env_int("PTYCHO_CLUSTERS", ncl)));
-    m.nclusters = ncl;
-    cfg.gridDim = dim3(Geo<N>::NCB * ncl);
-    LAUNCH(c, PTYCHO_K_MEGA, { cudaLaunchKernelEx(&cfg, kern, m); });
-    CU(cudaGetLastError());
-    return PTYCHO_OK;
-}
-
-// Stream-ordered form of the DM cycle: per chunk of waves, pass 1 -> pass 2 -> pass 3 as three kernels.
-template <int N, bool U16> void launch_split(ptycho_ctx* c, MegaArgs m, int chunk_waves) {
-    const size_t smem = MegaGeo<N>::smem;
-    for (int w0 = 0; w0 < m.nW; w0 += chunk_waves) {
-        const dim3 grid(Geo<N>::NCB, std::min(chunk_waves, m.nW - w0));
-        LAUNCH(c, PTYCHO_K_ROWS_FWD, (k_dm_pass<N, U16, 2><<<grid, kThreads, smem, c->stream>>>(m, w0)));
-        LAUNCH(c, PTYCHO_K_COLS, (k_dm_pass<N, U16, 1><<<grid, kThreads, smem, c->stream>>>(m, w0)));
-        LAUNCH(c, PTYCHO_K_ROWS_INV, (k_dm_pass<N, U16, 0><<<grid, kThreads, smem, c->stream>>>(m, w0)));
-    }
+    dispatch_n(c->N, [&](auto nn) { launch_passes<decltype(nn)::value>(c, a, nframes, fwd, col, inv); });
 }
 
 int ew_blocks(size_t n) { return (int)std::min<size_t>(kRedBlocks, (n + 255) / 256); }
@@ -344,10 +331,9 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
     // R4: psi_j = P O_j before the first DM iteration.  The plain megakernel forms it on the fly in pass 1 (saves a
     // 5 GB write and read at config 2); the other forms of the cycle read the store, so it is written first.
     const bool fresh = !c->psi_valid;
-    const bool fresh_in_kernel = fresh && c->mega_M > 0 && !c->par.deterministic && !env_int("PTYCHO_DM_SPLIT", 0) &&
-                                 !(env_int("PTYCHO_DM_CLUSTER", 0) && c->N <= 256);
+    const bool fresh_in_kernel = fresh && c->mega_M > 0 && !c->par.deterministic;
     if (fresh && !fresh_in_kernel) {
-        const dim3 g((unsigned)((knn + 255) / 256), c->J);
+        const dim3 g(c->J, (unsigned)((knn + 255) / 256));   // frame index in grid.x: J may exceed 65535
         LAUNCH(c, PTYCHO_K_OTHER, (k_init_psi<<<g, 256, 0, c->stream>>>(c->psi, c->O, c->W, c->P, c->K, c->N, c->pos, c->dm_frames)));
     }
     c->psi_valid = true;
@@ -360,6 +346,7 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         const int det = c->par.deterministic;
         m.update_probe = det ? 0 : upd;
         m.det = det;
+        m.corr = c->p2 ? 1 : 0;
         m.fresh = fresh_in_kernel ? 1 : 0;
         if (det && upd) {                                   // lagged probe sums from the incoming psi (R4), fixed order
             LAUNCH(c, PTYCHO_K_OTHER, (k_det_probe<<<dim3((unsigned)((nn + 255) / 256), kDetGroups), 256, 0, c->stream>>>(
@@ -370,41 +357,20 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         m.It = c->It;
         m.flags = env_int("PTYCHO_MEGA_FLAGS", 0);
         m.pf = m.M;
-        { int nw = (m.flags >> 8) ? 1 : 0; cudaMemcpyToSymbolAsync(g_nowait, &nw, sizeof(int), 0, cudaMemcpyHostToDevice, c->stream); }
-        m.head = c->mega_ctr; m.cnt1 = c->mega_ctr + 64; m.cnt2 = m.cnt1 + c->J; m.cnt3 = m.cnt2 + c->J;
-        CU(cudaMemsetAsync(c->mega_ctr, 0, sizeof(int) * (64 + 3 * (size_t)c->J), c->stream));
-        if (env_int("PTYCHO_DM_CLUSTER", 0) && c->N <= 256) {
-            ClusterArgs ca{};
-            ca.f = m.f; ca.J = c->J; ca.update_probe = m.update_probe; ca.det = m.det; ca.spos = c->spos; ca.It = c->It;
-            const bool u = c->itype == PTYCHO_I_U16;
-            ptycho_status st = PTYCHO_OK;
-            switch (c->N) {
-                case 64: st = u ? launch_cluster<64, true>(c, ca) : launch_cluster<64, false>(c, ca); break;
-                case 128: st = u ? launch_cluster<128, true>(c, ca) : launch_cluster<128, false>(c, ca); break;
-                default: st = u ? launch_cluster<256, true>(c, ca) : launch_cluster<256, false>(c, ca); break;
-            }
-            if (st != PTYCHO_OK) return st;
-        } else if (env_int("PTYCHO_DM_SPLIT", 0)) {
-            const int cw = std::max(1, std::min(env_int("PTYCHO_SPLIT_C", 96), m.R) / m.M);
-            m.pf = cw * m.M;
-            const bool u = c->itype == PTYCHO_I_U16;
-            switch (c->N) {
-                case 64: u ? launch_split<64, true>(c, m, cw) : launch_split<64, false>(c, m, cw); break;
-                case 128: u ? launch_split<128, true>(c, m, cw) : launch_split<128, false>(c, m, cw); break;
-                case 256: u ? launch_split<256, true>(c, m, cw) : launch_split<256, false>(c, m, cw); break;
-                default: u ? launch_split<512, true>(c, m, cw) : launch_split<512, false>(c, m, cw); break;
-            }
-        } else {
-        const long long items = (long long)(m.nW + 2 * m.D) * 3 * ncb;
+        m.head = c->mega_ctr; m.cnt1 = c->mega_ctr + 64; m.cnt2 = m.cnt1 + c->J; m.cnt3 = m.cnt2 + c->J; m.cnt2a = m.cnt3 + c->J;
+        m.stat = c->dm_stat;
+        if (fresh) CU(cudaMemsetAsync(c->dm_stat, 0, 2 * sizeof(int), c->stream));   // first iteration: fused form
+        CU(cudaMemsetAsync(c->mega_ctr, 0, sizeof(int) * (64 + 4 * (size_t)c->J), c->stream));
+        {
+        const long long items = (long long)(m.nW + 2 * m.D) * 3 * ncb;   // (fused form; the split form has more)
         const int grid = (int)std::min<long long>(items, c->mega_grid);
         const bool u16 = c->itype == PTYCHO_I_U16;
         LAUNCH(c, PTYCHO_K_MEGA, {
-            switch (c->N) {
-                case 64: if (u16) k_dm_mega<64, true><<<grid, kThreads, MegaGeo<64>::smem, c->stream>>>(m); else k_dm_mega<64, false><<<grid, kThreads, MegaGeo<64>::smem, c->stream>>>(m); break;
-                case 128: if (u16) k_dm_mega<128, true><<<grid, kThreads, MegaGeo<128>::smem, c->stream>>>(m); else k_dm_mega<128, false><<<grid, kThreads, MegaGeo<128>::smem, c->stream>>>(m); break;
-                case 256: if (u16) k_dm_mega<256, true><<<grid, kThreads, MegaGeo<256>::smem, c->stream>>>(m); else k_dm_mega<256, false><<<grid, kThreads, MegaGeo<256>::smem, c->stream>>>(m); break;
-                default: if (u16) k_dm_mega<512, true><<<grid, kThreads, MegaGeo<512>::smem, c->stream>>>(m); else k_dm_mega<512, false><<<grid, kThreads, MegaGeo<512>::smem, c->stream>>>(m); break;
-            }
+            dispatch_n(c->N, [&](auto nn) {
+                constexpr int N = decltype(nn)::value;
+                if (u16) k_dm_mega<N, true><<<grid, kThreads, MegaGeo<N>::smem, c->stream>>>(m);
+                else k_dm_mega<N, false><<<grid, kThreads, MegaGeo<N>::smem, c->stream>>>(m);
+            });
         });
         }
     } else
@@ -419,7 +385,13 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
     if (c->par.deterministic)                               // object sums from the new psi, fixed order
         LAUNCH(c, PTYCHO_K_OTHER, (k_det_object<<<dim3(c->det_tx, c->det_ty), dim3(kDetTileW, kDetTileH), 0, c->stream>>>(
                                        c->nO, c->dO, c->H, c->W, c->psi, c->P, c->N, c->spos, c->tile_start, c->tile_list)));
-    LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(HW), 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1)));
+    if (c->mega_M > 0 && c->p2) {                           // O += c / (d_O + eps), d_O gathered over the tile lists (dm_det.cuh)
+        LAUNCH(c, PTYCHO_K_UPDATE, (k_probe_support<<<(unsigned)((nn + 1023) / 1024), 1024, 0, c->stream>>>(c->p2, c->P, c->N, c->dm_stat)));
+        LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend_gather<<<dim3(c->det_tx, c->det_ty), dim3(kDetTileW, kDetTileH), 0, c->stream>>>(
+                                        c->O, c->nO, c->H, c->W, c->p2, c->N, c->tile_start, c->tile_mid, c->tile_list, c->sc)));
+    }
+    else
+        LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(HW), 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1)));
     LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(nn), 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd)));
     return PTYCHO_OK;
 }
@@ -547,12 +519,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
 
 #define CUI(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { fprintf(stderr, "ptycho_init: %s: %s\n", #call, cudaGetErrorString(e_)); delete c; return PTYCHO_ECUDA; } } while (0)
     ptycho_status st = PTYCHO_OK;
-    switch (n) {
-        case 64: st = set_attrs<64>(c); break;
-        case 128: st = set_attrs<128>(c); break;
-        case 256: st = set_attrs<256>(c); break;
-        default: st = set_attrs<512>(c); break;
-    }
+    dispatch_n(n, [&](auto nn) { st = set_attrs<decltype(nn)::value>(c); });
     if (st != PTYCHO_OK) { fprintf(stderr, "ptycho_init: %s\n", c->err.c_str()); delete c; return st; }
 
     const size_t HW = (size_t)obj_h * obj_w, nn = (size_t)n * n, knn = nn * n_modes;
@@ -567,6 +534,8 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     CUI(cudaMemsetAsync(c->dP, 0, nn * 4, s));
     CUI(cudaMemsetAsync(c->sc, 0, sizeof(Scalars), s));
     CUI(cudaMemsetAsync(c->err_hist, 0, sizeof(double) * kErrCap, s));
+    CUI(cudaMemsetAsync(c->err_ticket, 0, sizeof(unsigned int), s));
+    CUI(cudaMemsetAsync(c->dm_stat, 0, 2 * sizeof(int), s));
 
     std::vector<float2> tw, twi;
     const int E = n == 64 ? 8 : n == 512 ? 32 : 16, T = n / E;
@@ -612,30 +581,46 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     CUI(cudaMemcpyAsync(c->mb_frames, mb.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
     CUI(cudaMemcpyAsync(c->slot_of, c->slot_of_h.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
 
-    if (par.deterministic) {                                // frames per object tile, ascending slot (dm_det.cuh)
+    if (par.deterministic || c->p2) {                       // frames per object tile, ascending slot (dm_det.cuh)
+        // deterministic mode: entries are slots.  Otherwise (the d_O gather of k_dm_blend_gather): entries are packed positions
+        // y << 16 | x, and the frames that cover the WHOLE tile come first (tile_mid marks the boundary): no per-pixel test for them.
+        const bool gather = !par.deterministic;
         const size_t ntiles = (size_t)c->det_tx * c->det_ty;
-        std::vector<int> start(ntiles + 1, 0), list;
+        std::vector<int> start(ntiles + 1, 0), mid(ntiles, 0), list;
+        auto whole = [&](int y, int x, int ty, int tx) {
+            return y <= ty * kDetTileH && (ty + 1) * kDetTileH <= y + n && x <= tx * kDetTileW && (tx + 1) * kDetTileW <= x + n;
+        };
         for (int pass = 0; pass < 2; ++pass) {
-            std::vector<int> fill(start.begin(), start.end() - 1);
+            std::vector<int> fill_a, fill_b;
+            if (pass == 1) {
+                fill_a.assign(start.begin(), start.end() - 1);
+                fill_b.resize(ntiles);
+                for (size_t i = 0; i < ntiles; ++i) { fill_b[i] = start[i] + mid[i]; mid[i] = fill_b[i]; }
+            }
             for (int sidx = 0; sidx < n_pos; ++sidx) {
                 const int y = spos[2 * sidx], x = spos[2 * sidx + 1];
                 for (int ty = y / kDetTileH; ty <= (y + n - 1) / kDetTileH; ++ty)
                     for (int tx = x / kDetTileW; tx <= (x + n - 1) / kDetTileW; ++tx) {
                         const size_t tl = (size_t)ty * c->det_tx + tx;
-                        if (pass == 0) ++start[tl + 1]; else list[fill[tl]++] = sidx;
+                        const bool w = gather && whole(y, x, ty, tx);
+                        if (pass == 0) { ++start[tl + 1]; if (w) ++mid[tl]; }
+                        else if (!gather) list[fill_a[tl]++] = sidx;
+                        else if (w) list[fill_a[tl]++] = (y << 16) | x;
+                        else list[fill_b[tl]++] = (y << 16) | x;
                     }
             }
             if (pass == 0) { for (size_t i = 0; i < ntiles; ++i) start[i + 1] += start[i]; list.resize(start[ntiles]); }
         }
         CUI(cudaMemcpyAsync(c->tile_start, start.data(), start.size() * 4, cudaMemcpyHostToDevice, s));
+        CUI(cudaMemcpyAsync(c->tile_mid, mid.data(), mid.size() * 4, cudaMemcpyHostToDevice, s));
         CUI(cudaMemcpyAsync(c->tile_list, list.data(), list.size() * 4, cudaMemcpyHostToDevice, s));
         CUI(cudaStreamSynchronize(s));                      // the host vectors go out of scope
     }
     {                                                       // intensities in pass-2 tile order (dm_mega.cuh)
-        const dim3 g(ncb_of(n), n_pos);
+        const dim3 g(n_pos, ncb_of(n));   // frame index in grid.x: J may exceed 65535
 #define TILE_I(NN) do { if (itype == PTYCHO_I_U16) k_tile_intensity<NN, unsigned short><<<g, kThreads, 0, s>>>((unsigned short*)c->It, (const unsigned short*)c->I, c->dm_frames); \
                         else k_tile_intensity<NN, float><<<g, kThreads, 0, s>>>((float*)c->It, (const float*)c->I, c->dm_frames); } while (0)
-        switch (n) { case 64: TILE_I(64); break; case 128: TILE_I(128); break; case 256: TILE_I(256); break; default: TILE_I(512); break; }
+        dispatch_n(n, [&](auto nn) { constexpr int NN = decltype(nn)::value; TILE_I(NN); });
 #undef TILE_I
         ++c->launches;
     }
@@ -663,7 +648,7 @@ ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
         ptycho_status st = alg == PTYCHO_DM ? dm_iteration(c) : minibatch_iteration(c, alg);
         if (st != PTYCHO_OK) return st;
         double* slot = c->err_hist + (c->t < kErrCap ? c->t : kErrCap - 1);
-        LAUNCH(c, PTYCHO_K_UPDATE, (k_sum_error<<<1, 1024, 0, c->stream>>>(c->e_part, (size_t)c->J * ncb_of(c->N), c->sc, slot)));
+        LAUNCH(c, PTYCHO_K_UPDATE, (k_sum_error<<<kErrBlocks, 1024, 0, c->stream>>>(c->e_part, (size_t)c->J * ncb_of(c->N), c->sc, slot, c->err_part, c->err_ticket)));
         ++c->t;
     }
     CU(cudaGetLastError());
@@ -774,7 +759,7 @@ ptycho_status ptycho_eval_error(ptycho_ctx* c, double* out) {
         a.e_part = c->e_tmp + (size_t)s0 * ncb;
         passes(c, a, nf, RF_EXIT, CM_ERRONLY, -1);
     }
-    LAUNCH(c, PTYCHO_K_OTHER, (k_sum_error<<<1, 1024, 0, c->stream>>>(c->e_tmp, (size_t)c->J * ncb, c->sc, c->scratch_d)));
+    LAUNCH(c, PTYCHO_K_OTHER, (k_sum_error<<<kErrBlocks, 1024, 0, c->stream>>>(c->e_tmp, (size_t)c->J * ncb, c->sc, c->scratch_d, c->err_part, c->err_ticket)));
     CU(cudaMemcpyAsync(out, c->scratch_d, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     return PTYCHO_OK;
@@ -829,9 +814,10 @@ ptycho_status ptycho_prepare_frames(const void* raw, ptycho_itype raw_type, int 
     const size_t total = (size_t)n_frames * n * n, out_bytes = total * (out_type == PTYCHO_I_U16 ? 2 : 4);
     const bool dev_in = is_device_ptr(raw), dev_out = is_device_ptr(out);
     void *d_in = const_cast<void*>(raw), *d_out = out;
-    if (!dev_in) { CU(cudaMalloc(&d_in, in_bytes)); CU(cudaMemcpyAsync(d_in, raw, in_bytes, cudaMemcpyHostToDevice, s)); }
-    if (!dev_out) CU(cudaMalloc(&d_out, out_bytes));
-    const bool vec = (n % 8 == 0) && ((reinterpret_cast<uintptr_t>(d_out) & 15) == 0);
+    struct Tmp { void* p = nullptr; ~Tmp() { if (p) cudaFree(p); } } t_in, t_out;   // staging: freed on every return path
+    if (!dev_in) { CU(cudaMalloc(&t_in.p, in_bytes)); d_in = t_in.p; CU(cudaMemcpyAsync(d_in, raw, in_bytes, cudaMemcpyHostToDevice, s)); }
+    if (!dev_out) { CU(cudaMalloc(&t_out.p, out_bytes)); d_out = t_out.p; }
+    const bool vec = (n % 16 == 0) && ((reinterpret_cast<uintptr_t>(d_out) & 15) == 0);   // n/2 a multiple of 8: a group of 8 never straddles kx = n/2
     const int grid = (int)std::min<size_t>((total / (vec ? 8 : 1) + 255) / 256, (size_t)148 * 64);
 #define PREP(TI, TO) do { if (vec) k_prepare_frames<TI, TO, 8><<<grid, 256, 0, s>>>((const TI*)d_in, det_h, det_w, center_y, center_x, n, threshold, saturation, (TO*)d_out, total); \
                           else k_prepare_frames<TI, TO, 1><<<grid, 256, 0, s>>>((const TI*)d_in, det_h, det_w, center_y, center_x, n, threshold, saturation, (TO*)d_out, total); } while (0)
@@ -843,8 +829,6 @@ ptycho_status ptycho_prepare_frames(const void* raw, ptycho_itype raw_type, int 
     if (!dev_out) CU(cudaMemcpyAsync(out, d_out, out_bytes, cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
     CU(cudaGetLastError());
-    if (!dev_in) cudaFree(d_in);
-    if (!dev_out) cudaFree(d_out);
     return PTYCHO_OK;
 }
 
@@ -857,13 +841,15 @@ ptycho_status ptycho_test_fft2(float* data, int n, int count, int inverse, void*
     ptycho_ctx tmp;
     ptycho_ctx* c = &tmp;
     c->N = n; c->K = 1; c->stream = static_cast<cudaStream_t>(cuda_stream);
-    ptycho_status st = n == 64 ? set_attrs<64>(c) : n == 128 ? set_attrs<128>(c) : n == 256 ? set_attrs<256>(c) : set_attrs<512>(c);
+    ptycho_status st = PTYCHO_OK;
+    dispatch_n(n, [&](auto nn) { st = set_attrs<decltype(nn)::value>(c); });
     if (st != PTYCHO_OK) return st;
     std::vector<float2> tw, twi;
     const int E = n == 64 ? 8 : n == 512 ? 32 : 16;
     host_twiddles(n, E, n / E, tw, twi);
-    float2* d_tw = nullptr;
-    CU(cudaMalloc(&d_tw, 2 * n * sizeof(float2)));
+    struct Tmp { float2* p = nullptr; ~Tmp() { if (p) cudaFree(p); } } t_tw;   // freed on every return path
+    CU(cudaMalloc(&t_tw.p, 2 * n * sizeof(float2)));
+    float2* d_tw = t_tw.p;
     CU(cudaMemcpy(d_tw, tw.data(), n * 8, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(d_tw + n, twi.data(), n * 8, cudaMemcpyHostToDevice));
     FrameArgs a{};
@@ -876,7 +862,6 @@ ptycho_status ptycho_test_fft2(float* data, int n, int count, int inverse, void*
     }
     CU(cudaStreamSynchronize(c->stream));
     CU(cudaGetLastError());
-    cudaFree(d_tw);
     return PTYCHO_OK;
 }
 

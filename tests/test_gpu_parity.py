@@ -32,6 +32,15 @@ def make(B, s, **par):
     return B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(**par))
 
 
+def well_lit(s, frac=0.1):
+    """SURVEY.md 8(c) parity protocol: the region d_O > frac * max d_O, d_O = sum_j sum_k |P_k|^2 placed at r_j."""
+    d = np.zeros(s.obj0.shape)
+    p2 = np.sum(np.abs(np.asarray(s.probe0).reshape(-1, s.n, s.n)) ** 2, 0)
+    for y, x in s.pos:
+        d[y:y + s.n, x:x + s.n] += p2
+    return d > frac * d.max()
+
+
 # ------------------------------------------------------------------------------ T2: FFT alone
 @pytest.mark.parametrize("n", [64, 128, 256, 512])
 def test_fft2_vs_oracle(B, oracle_mod, n):
@@ -86,11 +95,8 @@ def test_cfg0_minibatch(B, oracle_mod, alg):
     o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(batch_size=16), keep_revised=True)
     g = make(B, s, batch_size=16)
     for it in range(10):
-        rv = g.revised_waves()                                # of the current (pre-iteration) state
         o.iterate(alg, 1)
         g.iterate(alg, 1)
-        if it == 0:
-            pass
         assert rel(g.fetch_object(), o.O) < TOL_RUN, it
         assert rel(g.fetch_probe(), o.P) < TOL_RUN, it
     assert np.allclose(g.fetch_error(), o.err, rtol=2e-3, atol=1e-9)
@@ -254,18 +260,6 @@ def test_dm_queue_geometry_does_not_change_the_result(B, oracle_mod, monkeypatch
         assert rel(g.fetch_object(), o.O) < 3 * TOL_ITER, (M, D, X)
         assert rel(g.fetch_exit_waves(), o.psi) < 3 * TOL_ITER, (M, D, X)
         g.destroy()
-    monkeypatch.setenv("PTYCHO_DM_CLUSTER", "1")                 # one thread-block cluster per frame, exchange through DSMEM
-    g = make(B, s, pbound=0.3)
-    g.iterate("DM", 3)
-    assert rel(g.fetch_object(), o.O) < 3 * TOL_ITER and rel(g.fetch_exit_waves(), o.psi) < 3 * TOL_ITER
-    g.destroy()
-    monkeypatch.delenv("PTYCHO_DM_CLUSTER")
-    monkeypatch.setenv("PTYCHO_DM_SPLIT", "1")                   # the stream-ordered three-kernel form of the same passes
-    monkeypatch.setenv("PTYCHO_MEGA_M", "2")
-    g = make(B, s, pbound=0.3)
-    g.iterate("DM", 3)
-    assert rel(g.fetch_object(), o.O) < 3 * TOL_ITER and rel(g.fetch_exit_waves(), o.psi) < 3 * TOL_ITER
-    g.destroy()
 
 
 def test_deterministic_mode_is_bit_reproducible_and_matches_the_oracle(B, oracle_mod):
@@ -338,7 +332,8 @@ def test_prepare_frames_bit_exact(B, oracle_mod, in_dt, out_dt):
     rng = np.random.default_rng(11)
     raw = rng.integers(0, 70000, (5, 150, 170)).clip(0, 65535).astype(np.uint16)
     raw = raw if in_dt == np.uint16 else (raw.astype(np.float32) * 1.37 - 20.0).astype(np.float32)
-    for center, n in (((75, 85), 128), ((10, 160), 64), ((149, 0), 32), ((3, 168), 6)):      # n = 6: the scalar path
+    for center, n in (((75, 85), 128), ((10, 160), 64), ((149, 0), 32), ((3, 168), 6),
+                      ((40, 50), 8), ((70, 90), 24), ((60, 20), 40), ((80, 80), 72)):   # n = 6 and n % 16 == 8: the scalar path
         ref = oracle_mod.prepare_frames(raw, center, n, threshold=300.0, saturation=60000.0, out_dtype=out_dt)
         got = B.prepare_frames(raw, center, n, threshold=300.0, saturation=60000.0, out_dtype=out_dt)
         assert got.dtype == ref.dtype and np.array_equal(got, ref), (center, n)
@@ -346,3 +341,179 @@ def test_prepare_frames_bit_exact(B, oracle_mod, in_dt, out_dt):
         assert np.array_equal(got_d.cpu().numpy(), ref), (center, n)
     plain = B.prepare_frames(raw, (75, 85), 64, out_dtype=out_dt)        # no threshold, no saturation
     assert np.array_equal(plain, oracle_mod.prepare_frames(raw, (75, 85), 64, out_dtype=out_dt))
+
+
+# ------------------------------------------------- the steady-state path bench.py times, at full size
+def test_cfg2_full_size_steady_state_teacher_forced(B, oracle_mod, record_property):
+    """Config 2 as `bench.py` times it AFTER the first iteration: psi_j is read from the 5.2 GB store, the reflector is not
+    the identity, the ring wraps ~90 times.  psi_j' of a DM iteration depends only on (O, P, psi_j, I_j), so it is teacher-forced:
+    a perturbed object, psi_j = Q O_j for a perturbed probe Q (built on the device), ONE iteration, then 48 sampled frames (first,
+    last, random: both sides of many ring wraps) against oracles holding just those frames with the same psi_j.  The object is
+    compared with the oracle on a window, from an oracle that holds every frame overlapping the window."""
+    import torch
+    s = synth.make_config(2)
+    par = dict(pbound=s.params["pbound"])
+    J, n = s.n_pos, s.n
+    rng = np.random.default_rng(21)
+    obj = (s.obj_true * (1 + 0.05 * (rng.standard_normal(s.obj_true.shape) + 1j * rng.standard_normal(s.obj_true.shape)))).astype(np.complex64)
+    q = (s.probe0[0] * (1 + 0.03 * (rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))))).astype(np.complex64)
+    g = make(B, s, **par)
+    g.set_object(obj)
+    od, qd = torch.from_numpy(obj).cuda(), torch.from_numpy(q).cuda()
+    psi = torch.empty((J, 1, n, n), dtype=torch.complex64, device="cuda")
+    for j, (y, x) in enumerate(s.pos):
+        psi[j, 0] = qd * od[y:y + n, x:x + n]
+    g.set_exit_waves(psi)
+    g.iterate("DM", 1)                                           # steady-state branch: psi is valid, nothing is re-initialised
+    idx = np.sort(rng.choice(J, 48, replace=False)).astype(np.int32)
+    idx[0], idx[-1] = 0, J - 1
+    psi_g = g.fetch_exit_waves(idx)
+    o = oracle_mod.Oracle(obj, s.probe0, s.pos[idx], s.intensities[idx], par)
+    o.psi = np.stack([(q * obj[y:y + n, x:x + n])[None] for y, x in s.pos[idx]]).astype(np.complex128)
+    o.iterate("DM", 1)
+    worst = max(rel(psi_g[k], o.psi[k]) for k in range(len(idx)))
+    assert worst < TOL_ITER, worst
+    # object on a window, against an oracle that holds all frames overlapping it
+    y0, x0, w = 2000, 2100, 48
+    cover = np.array([j for j, (y, x) in enumerate(s.pos) if y < y0 + w and y + n > y0 and x < x0 + w and x + n > x0], np.int32)
+    assert len(cover) > 20
+    ow = oracle_mod.Oracle(obj, s.probe0, s.pos[cover], s.intensities[cover], par)
+    ow.psi = np.stack([(q * obj[y:y + n, x:x + n])[None] for y, x in s.pos[cover]]).astype(np.complex128)
+    ow.iterate("DM", 1)
+    O_g = g.fetch_object()
+    assert rel(O_g[y0:y0 + w, x0:x0 + w], ow.O[y0:y0 + w, x0:x0 + w]) < TOL_ITER
+    assert np.isfinite(g.fetch_error()[-1])
+    # three free-running iterations against the full oracle, where the host can hold psi in double (10.5 GB)
+    import psutil
+    ran_full = psutil.virtual_memory().available > 40 * 2 ** 30
+    record_property("cfg2_full_oracle_branch_ran", ran_full)
+    print(f"cfg2 full-size free-running oracle branch ran: {ran_full}")
+    if ran_full:
+        g2 = make(B, s, **par)
+        of = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, par)
+        g2.iterate("DM", 3)
+        of.iterate("DM", 3)
+        lit = well_lit(s)
+        O2 = g2.fetch_object()
+        assert rel(O2, of.O) < 3 * TOL_ITER and rel(O2[lit], of.O[lit]) < 3 * TOL_ITER and rel(g2.fetch_probe(), of.P) < 3 * TOL_ITER
+        assert rel(g2.fetch_exit_waves(idx), of.psi[idx]) < 3 * TOL_ITER
+        assert np.allclose(g2.fetch_error(), of.err, rtol=2e-3)
+        g2.destroy()
+    g.destroy()
+
+
+def test_dm_inside_the_power_bound_paths(B, oracle_mod):
+    """Frames whose error is inside the power bound (R6, rb = 1) take the short pass 3 (psi' = P O_j, no transform, no
+    scatter), and once most frames are there the megakernel switches to its split form (error-only column pass, the full pass
+    only for the frames that need it).  A bound chosen so that the frames cross it during the run exercises every combination;
+    the oracle knows none of this."""
+    s = synth.make_custom(128, 420, 7, 37, k=1, peak=2e4, dtype=np.uint16, jitter=3, seed=31, probe_kind="zone")
+    lit = well_lit(s)
+    for pb in (0.6, 3.0):
+        o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(pbound=pb))
+        g = make(B, s, pbound=pb)
+        inside = []
+        for it in range(14):
+            o.iterate("DM", 1)
+            g.iterate("DM", 1)
+            tol = TOL_ITER * (it + 1)
+            Og = g.fetch_object()
+            assert rel(Og, o.O) < tol and rel(Og[lit], o.O[lit]) < tol and rel(g.fetch_probe(), o.P) < tol, (pb, it)
+            inside.append(float(o.err[-1] * o.sum_I / (o.J * s.n * s.n)))
+        assert rel(g.fetch_exit_waves(), o.psi) < 14 * TOL_ITER
+        assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+        assert inside[0] > pb and inside[-1] < pb, inside          # the run really crossed the bound
+        g.destroy()
+
+
+@pytest.mark.parametrize("n,h,side,step", [(256, 520, 4, 61), (512, 900, 3, 150)])
+def test_dm_fp32_intensities_large_frames(B, oracle_mod, n, h, side, step):
+    """The float-intensity instantiations of the megakernel at 256^2 and 512^2 (every other test of these sizes uses uint16)."""
+    s = synth.make_custom(n, h, side, step, k=1, peak=2e4, dtype=np.float32, jitter=3, seed=n + 7, probe_kind="zone")
+    s.intensities[1, 3, 5] = -1.0                              # a masked pixel (R3)
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(pbound=0.4))
+    g = make(B, s, pbound=0.4)
+    lit = well_lit(s)
+    for it in range(4):
+        o.iterate("DM", 1)
+        g.iterate("DM", 1)
+        Og = g.fetch_object()
+        assert rel(Og, o.O) < TOL_ITER * (it + 1) and rel(Og[lit], o.O[lit]) < TOL_ITER * (it + 1), it
+        assert rel(g.fetch_probe(), o.P) < TOL_ITER * (it + 1), it
+    assert rel(g.fetch_exit_waves(), o.psi) < 4 * TOL_ITER
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+
+
+@pytest.mark.parametrize("alg,k", [("DM", 1), ("EPIE_MB", 1), ("LSQML", 2), ("DM", 2)])
+def test_zero_amplitude_branch_R2(B, oracle_mod, alg, k):
+    """R2: where the transformed wave is exactly zero the projection gives sqrt(I) with zero phase (mode 0) and 0 (other modes).
+    One frame sits on an object patch that is exactly 0, so its whole spectrum takes that branch -- in the megakernel (K = 1 DM)
+    and in the three-pass kernels (everything else), which share the threshold |Phi|^2 <= 1e-30."""
+    s = synth.make_custom(64, 200, 4, 30, k=k, peak=2e4, dtype=np.float32, jitter=0, seed=5, probe_kind="disk")
+    y, x = s.pos[5]
+    obj = s.obj0.copy()
+    obj[y:y + 64, x:x + 64] = 0
+    kw = dict(batch_size=4) if alg != "DM" else {}
+    o = oracle_mod.Oracle(obj, s.probe0, s.pos, s.intensities, kw, keep_revised=True)
+    g = B.Ptycho(obj, s.probe0, s.pos, s.intensities, B.default_params(**kw))
+    if alg != "DM":
+        rv = g.revised_waves(np.array([5], np.int32))
+    o.iterate(alg, 1)
+    g.iterate(alg, 1)
+    if alg != "DM":
+        assert rel(rv[0], o.revised[5]) < TOL_ITER             # F^-1[sqrt(I)] in mode 0, zero in the others
+        if k > 1:
+            assert np.abs(rv[0, 1:]).max() == 0
+    else:
+        assert rel(g.fetch_exit_waves(np.array([5], np.int32)), o.psi[5:6]) < TOL_ITER
+    o.iterate(alg, 1)
+    g.iterate(alg, 1)
+    assert rel(g.fetch_object(), o.O) < 2 * TOL_ITER and rel(g.fetch_probe(), o.P) < 2 * TOL_ITER
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+
+
+def test_lsqml_teacher_forced_256_three_modes(B, oracle_mod):
+    """Per-iteration parity (<= 1e-4) of the LSQML-style step at 256^2 with three probe modes: the GPU is reset to the oracle's
+    state before every iteration; revised waves, object, probe modes and the (a, b) steps are compared."""
+    s = synth.make_custom(256, 520, 4, 61, k=3, peak=2e4, dtype=np.uint16, jitter=3, seed=259, probe_kind="disk")
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(batch_size=6), keep_revised=True)
+    g = make(B, s, batch_size=6)
+    lit = well_lit(s)
+    for it in range(3):
+        g.set_object(o.O)
+        g.set_probe(o.P)
+        n_before = len(o.steps)
+        o.iterate("LSQML", 1)
+        g.iterate("LSQML", 1)
+        Og = g.fetch_object()
+        assert rel(Og, o.O) < TOL_ITER and rel(Og[lit], o.O[lit]) < TOL_ITER and rel(g.fetch_probe(), o.P) < TOL_ITER, it
+        assert np.allclose(g.fetch_steps()[n_before:], np.array(o.steps[n_before:]), rtol=1e-3), it
+    g.set_object(o.O)
+    g.set_probe(o.P)
+    sel = np.array([0, 7, 15], np.int32)
+    rv = g.revised_waves(sel)
+    o.iterate("LSQML", 1)
+    assert rel(rv, o.revised[sel]) < TOL_ITER
+
+
+def test_handoff_stress_deterministic_bitwise(B, monkeypatch):
+    """The cross-CTA hand-off of the megakernel (relaxed polls, release increments, ring reuse) under many queue geometries:
+    in deterministic mode the result does not depend on timing, so 10 random (M, D, X) x 20 iterations must reproduce the default
+    geometry BIT FOR BIT (object, probe, exit waves).  A missed dependency would read a half-written frame and break equality."""
+    s = synth.make_custom(64, 260, 9, 21, k=1, peak=2e4, dtype=np.uint16, jitter=3, seed=77, probe_kind="zone")
+    def run():
+        g = B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(pbound=0.3, deterministic=1))
+        g.iterate("DM", 20)
+        out = (g.fetch_object(), g.fetch_probe(), g.fetch_exit_waves(), g.fetch_error())
+        g.destroy()
+        return out
+    ref = run()
+    rng = np.random.default_rng(3)
+    for _ in range(10):
+        M, D, X = int(rng.integers(1, 9)), int(rng.integers(2, 7)), int(rng.integers(0, 5))
+        monkeypatch.setenv("PTYCHO_MEGA_M", str(M))
+        monkeypatch.setenv("PTYCHO_MEGA_D", str(D))
+        monkeypatch.setenv("PTYCHO_MEGA_X", str(X))
+        got = run()
+        for a, b in zip(got, ref):
+            assert np.array_equal(a, b), (M, D, X)

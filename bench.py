@@ -36,6 +36,7 @@ METRIC = "diffraction patterns/sec per DM iteration (256x256, 1 B200); % HBM roo
 UNIT = "patterns/s"
 CFG = 2                      # default: BASELINE.json configs[2]
 DEFAULT_ALG = {1: "EPIE_MB", 2: "DM", 3: "LSQML", 4: "DM"}
+FULL_J = {1: 1024, 2: 10000, 3: 20000, 4: 16384}
 REF_SAMPLE = {1: 256, 2: 256, 3: 96, 4: 64}   # frames of the bounded oracle sample (first positions of the same scan)
 TRAFFIC_FILE = os.path.join(_ROOT, "profiles", "r02_traffic.json")   # ncu dram__bytes per launch of the dominant kernel, per config
 
@@ -129,38 +130,92 @@ class ClockSampler(threading.Thread):
 
 
 # --------------------------------------------------------------------------- reference arm (oracle)
-def run_oracle_sample(steps: int, warmup: int, sample: int = REF_SAMPLE):
-    """Times the CPU oracle (oracle/, as it stands) on the first `sample` positions of config 2:
-    one step = one oracle DM iteration over those frames.  Returns (patterns/s, ms/step, cores)."""
+def scan_params(s, alg: str) -> dict:
+    """Parameters of the run: the config's own (synth.params) for the chosen algorithm."""
+    par = {}
+    if alg == "DM":
+        par["pbound"] = s.params.get("pbound", s.params.get("pbound_dm", 0.0))
+    else:
+        par["batch_size"] = s.params.get("batch_size", 0)
+        par["disable_dm"] = 1
+    return par
+
+
+def workload_name(cfg: int, alg: str, s, J: int) -> str:
+    return (f"cfg{cfg} {alg} {s.n}x{s.n} J={J} H={s.obj0.shape[0]} {s.intensities.dtype} K={s.n_modes}"
+            +  (f" pbound={scan_params(s, alg)['pbound']}" if alg == "DM" else f" batch={s.params.get('batch_size', 0)}"))
+
+
+def run_oracle_sample(cfg: int, alg: str, steps: int, warmup: int):
+    """Times the CPU oracle (oracle/, as it stands) on the first REF_SAMPLE[cfg] positions of the config:
+    one step = one oracle iteration over those frames.  Returns (patterns/s, ms/step, cores, sample)."""
     import oracle
     from paper_2202_03144_b200 import synth
     oracle.build()
-    s = synth.make_config(CFG, n_pos=sample)
-    o = oracle.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(pbound=s.params["pbound"]))
+    sample = REF_SAMPLE[cfg]
+    s = synth.make_config(cfg, n_pos=sample)
+    par = {k: v for k, v in scan_params(s, alg).items() if k != "disable_dm"}
+    o = oracle.Oracle(s.obj0, s.probe0, s.pos, s.intensities, par)
     for _ in range(warmup):
-        o.iterate("DM", 1)
+        o.iterate(alg, 1)
     t0 = time.perf_counter()
     for _ in range(steps):
-        o.iterate("DM", 1)
+        o.iterate(alg, 1)
     dt = time.perf_counter() - t0
     cores = int(os.environ.get("OMP_NUM_THREADS", 0)) or (os.cpu_count() or 1)
-    return sample * steps / dt, dt / steps * 1e3, cores
+    return sample * steps / dt, dt / steps * 1e3, cores, sample
 
 
 def reference_line(args) -> dict:
+    from paper_2202_03144_b200 import synth
+    cfg, alg = args.config, args.alg or DEFAULT_ALG[args.config]
     steps, warmup = max(1, args.steps), max(0, args.warmup)
-    val, ms, cores = run_oracle_sample(steps, warmup)
-    sample = (f"first {REF_SAMPLE} of the 10000 positions of config 2 (same generator), "
-              f"one oracle DM iteration (fp64, OpenMP over frames) per step")
+    val, ms, cores, sample = run_oracle_sample(cfg, alg, steps, warmup)
+    s = synth.make_config(cfg, n_pos=4)
+    what = (f"first {sample} positions of config {cfg} (same generator), one oracle {alg} iteration "
+            f"(fp64, OpenMP over frames) per step")
     return {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": warmup, "ms_per_step": ms, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "cfg2 DM 256x256 J=10000 H=4096 u16 (bounded sample)", "sample_frames": REF_SAMPLE},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "config": {"workload": workload_name(cfg, alg, s, FULL_J[cfg]) + " (bounded sample)", "sample_frames": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
+
+
+def cufft_reference_line(args) -> dict:
+    """B:ns "cuFFT is reported only as a reference point": the DM cycle of config 2's frame size written as unfused torch
+    operations on resident frames (reflector, fft2, modulus replacement, ifft2, exit-wave update; no object gather, no
+    overlap sums, no error) and the two bare transforms alone.  Harness-side only; the library never calls cuFFT."""
+    import torch
+    from paper_2202_03144_b200 import synth
+    dev = torch.device("cuda", 0)
+    n, f = (synth.make_config(args.config, n_pos=4).n), 2000
+    g = torch.Generator(device=dev).manual_seed(0)
+    psi = torch.randn((f, n, n), dtype=torch.complex64, device=dev, generator=g)
+    po = torch.randn((f, n, n), dtype=torch.complex64, device=dev, generator=g)
+    amp = torch.rand((f, n, n), device=dev, generator=g) * 30
+    def bare():
+        return torch.fft.ifft2(torch.fft.fft2(psi))
+    def cycle():
+        phi = torch.fft.fft2(2 * po - psi)
+        phi = phi * (amp / phi.abs().clamp_min(1e-30))
+        return psi + torch.fft.ifft2(phi) - po
+    out = {}
+    for name, fn in (("fft2_ifft2", bare), ("unfused_cycle", cycle)):
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(10):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        out[name] = f * 10 / (e0.elapsed_time(e1) * 1e-3)
+    return {"impl": "cufft_reference_point", "unit": "frames/s", "frame": n, "frames_resident": f, **out,
+            "note": "torch.fft (cuFFT) on resident complex64 frames; a reference point, not part of the library"}
 
 
 # --------------------------------------------------------------------------- this build's arm
@@ -200,10 +255,11 @@ def ours_line(args) -> dict | None:
     from paper_2202_03144_b200 import binding, synth
     binding.lib()                                            # fails loudly if the .so is missing
 
+    cfg, alg = args.config, args.alg or DEFAULT_ALG[args.config]
     steps, warmup = max(1, args.steps), max(3, args.warmup)
-    s = synth.make_config(CFG, n_pos=args.n_pos, replica=rank, threads=max(2, (os.cpu_count() or 8) // world))
+    s = synth.make_config(cfg, n_pos=args.n_pos, replica=rank, threads=max(2, (os.cpu_count() or 8) // world))
     J, N, K = s.n_pos, s.n, s.n_modes
-    par = dict(pbound=s.params["pbound"])
+    par = scan_params(s, alg)
     obj0 = torch.from_numpy(s.obj0.astype(np.complex64))
     probe0 = torch.from_numpy(s.probe0.astype(np.complex64))
     inten_h = torch.from_numpy(s.intensities).pin_memory()
@@ -214,7 +270,7 @@ def ours_line(args) -> dict | None:
     g = binding.Ptycho(obj0.to(dev), probe0.to(dev), s.pos, inten_d, binding.default_params(**par), device=dev)
     stream = torch.cuda.current_stream(dev)
     for _ in range(warmup):
-        g.iterate("DM", 1)
+        g.iterate(alg, 1)
     try:
         uuid = str(torch.cuda.get_device_properties(dev).uuid)
     except Exception:
@@ -229,7 +285,7 @@ def ours_line(args) -> dict | None:
     t0 = time.perf_counter()
     e0.record(stream)
     for _ in range(steps):
-        g.iterate("DM", 1)
+        g.iterate(alg, 1)
     e1.record(stream)
     torch.cuda.synchronize(dev)
     t1 = time.perf_counter()
@@ -246,7 +302,7 @@ def ours_line(args) -> dict | None:
     torch.cuda.empty_cache()
 
     # ---- end to end through the C ABI from pinned host buffers (H2D + iterate + D2H inside)
-    e2e_steps = min(steps, 10)
+    e2e_steps = min(steps, 10 if cfg != 4 else 3)
     h2d = inten_h.numel() * inten_h.element_size() + obj_h.numel() * 8 + probe_h.numel() * 8 + s.pos.nbytes
     e2e_ms = []
     for i in range(e2e_steps + 1):
@@ -254,7 +310,7 @@ def ours_line(args) -> dict | None:
         barrier(world)
         e0.record(stream)
         ge = binding.Ptycho(obj_h, probe_h, s.pos, inten_h, binding.default_params(**par), device=dev)
-        ge.iterate("DM", 1)
+        ge.iterate(alg, 1)
         ev = ge.fetch_error()                                # D2H of the step's result (8 bytes)
         e1.record(stream)
         torch.cuda.synchronize(dev)
@@ -267,34 +323,46 @@ def ours_line(args) -> dict | None:
     e2e_ms_step = max_over_ranks(sum(e2e_ms) / len(e2e_ms), world, dev)
 
     # ---- roofline of the dominant kernel chain
-    peak, peak_src = measured_peaks()
+    hbm_peak, peak_src = measured_peaks()
     chain = ("mega",) if prof.get("mega", (0.0, 0))[1] > 0 else ("rows_fwd", "cols", "rows_inv")
     chain_ms = sum(prof[k][0] for k in chain)
-    bytes_i = s.intensities.dtype.itemsize
-    alg_bytes = algorithmic_bytes_per_pattern(N, K, bytes_i)
-    achieved = alg_bytes * J * steps / (chain_ms * 1e-3) / 1e9 if chain_ms > 0 else 0.0
     n_chain = sum(prof[k][1] for k in chain)
-    roofline = {
-        "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (chain == ("mega",) and J == 10000 and args.n_pos is None) else None,
-        "traffic_source": "ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of one k_dm_mega launch (profiles/r01_v2.md, v4)",
-        "peak_source": peak_src,
-        "kernel": ("k_dm_mega<256> (one persistent launch per DM iteration: a1-a9 of all frames)" if chain == ("mega",)
-                   else "k_rows_fwd+k_cols+k_rows_inv chain (one chunk of frames per launch triple)"),
-        "algorithmic_bytes_per_pattern": alg_bytes,
+    bytes_i = s.intensities.dtype.itemsize
+    full = args.n_pos is None
+    if alg == "DM":                                          # HBM-bound: psi in, psi out, I in per pattern
+        alg_bytes = algorithmic_bytes_per_pattern(N, K, bytes_i)
+        achieved = alg_bytes * J * steps / (chain_ms * 1e-3) / 1e9 if chain_ms > 0 else 0.0
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
+                    "peak_source": peak_src, "algorithmic_bytes_per_pattern": alg_bytes,
+                    "step_frac_of_hbm_roofline": (alg_bytes * J * steps * world / (ms * 1e-3) / 1e9) / (hbm_peak * world)}
+    else:                                                    # no exit-wave traffic: the fp32 ALUs bind
+        mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965
+        peak = 148 * 128 * 2 * mhz * 1e6 / 1e12             # SMs x fp32 lanes x 2 flop (FMA) x SM clock sampled in this run
+        fl = flops_per_pattern(N, K)
+        achieved = fl * J * steps / (chain_ms * 1e-3) / 1e12 if chain_ms > 0 else 0.0
+        roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                    "peak_source": f"148 SMs x 128 fp32 lanes x 2 x {mhz} MHz (median SM clock of this run)",
+                    "nominal_flops_per_pattern": fl,
+                    "frac_of_hbm_roofline": (N * N * bytes_i * J * steps / (ms * 1e-3) / 1e9) / hbm_peak}
+    roofline.update({
+        "traffic": ncu_traffic(cfg, alg) if full else None,
+        "traffic_source": "profiles/r02_traffic.json: ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch (profiles/r02.md)",
+        "kernel": ("k_dm_mega (one persistent launch per DM iteration: a1-a9 of all frames)" if chain == ("mega",)
+                   else "k_rows_fwd + k_cols + k_rows_inv (one launch triple per chunk of a minibatch)"),
         "launches_timed": n_chain, "avg_launch_ms": chain_ms / max(n_chain, 1),
         "kernel_ms_per_step": {k: prof[k][0] / steps for k in prof},
-        "step_frac_of_hbm_roofline": (alg_bytes * J * steps * world / (ms * 1e-3) / 1e9) / (peak * world),
-    }
+    })
     line = {
         "metric": METRIC, "value": J * steps * world / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
         "steps": steps, "warmup": warmup, "ms_per_step": ms / steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"cfg2 DM {N}x{N} J={J} H={s.obj0.shape[0]} u16 K={K} pbound={par['pbound']}",
-                   "l2": "inputs larger than L2 (psi %.2f GB + I %.2f GB streamed per step)" % (J * K * N * N * 8 / 1e9, J * N * N * bytes_i / 1e9),
+        "config": {"workload": workload_name(cfg, alg, s, J),
+                   "l2": "inputs larger than L2 (%.2f GB streamed per step)" % ((J * K * N * N * 16 * (alg == "DM") + J * N * N * bytes_i) / 1e9),
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
-                   "e2e_step": "ptycho_init from pinned host buffers + 1 DM iteration + ptycho_fetch_error",
-                   "e2e_steps": e2e_steps},
+                   "e2e_step": f"ptycho_init from pinned host buffers + the FIRST {alg} iteration + ptycho_fetch_error",
+                   "e2e_steps": e2e_steps,
+                   "timed_iterations": f"{warmup}..{warmup + steps - 1} of a run from the flat object (DM: frames inside the power bound "
+                                       "take the short pass 3; see DESIGN.md section 5)"},
         "clocks": clocks,
         "e2e": {"value": J * world / (e2e_ms_step * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": 8, "ms_per_step": e2e_ms_step},
@@ -303,9 +371,9 @@ def ours_line(args) -> dict | None:
         "error_first_last": [float(err_hist[0]), float(err_hist[-1])],
     }
     if world == 1 and rank == 0 and not args.no_cpu_baseline:
-        val, _, cores = run_oracle_sample(steps=6, warmup=1)
+        val, _, cores, sample = run_oracle_sample(cfg, alg, steps=4 if cfg in (3, 4) else 6, warmup=1)
         line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"first {REF_SAMPLE} positions of config 2, 6 oracle DM iterations (fp64, OpenMP)"}
+                                "sample": f"first {sample} positions of config {cfg}, oracle {alg} iterations (fp64, OpenMP)"}
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
@@ -318,10 +386,17 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=CFG, choices=[1, 2, 3, 4], help="BASELINE.json configs[i] (default 2: the metric's)")
+    ap.add_argument("--alg", default=None, choices=["DM", "EPIE_MB", "LSQML"], help="default: the config's own algorithm")
+    ap.add_argument("--cufft-ref", action="store_true", help="print the torch.fft reference point instead (harness-side)")
     ap.add_argument("--n-pos", type=int, default=None, help="truncate the scan (debugging only; invalidates the metric)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank, _, world = dist_env()
+    if args.cufft_ref:
+        if rank == 0:
+            print(json.dumps(cufft_reference_line(args)), flush=True)
+        return
     if args.impl == "reference":
         if rank == 0:
             print(json.dumps(reference_line(args)), flush=True)

@@ -20,7 +20,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 ALG = {"EPIE_MB": 0, "DM": 1, "LSQML": 2}
 DEFAULTS = dict(batch_size=0, probe_start=0, delta_blend=1e-2, delta_obj=1.0, delta_probe=1.0,
-                alpha_obj=1.0, alpha_probe=1.0, lsq_lambda=0.1, pbound=0.0, batch_order=None)
+                alpha_obj=1.0, alpha_probe=1.0, lsq_lambda=0.1, pbound=0.0, batch_order=None, dm_sweeps=0)
 
 
 def build(force: bool = False) -> None:
@@ -157,9 +157,20 @@ class Oracle:
             if alg == "DM":
                 if self.psi is None:
                     self.init_exit_waves()
+                sweeps = int(p["dm_sweeps"])
+                # dm_sweeps = 0: reading R4 (lagged probe sums, one pass).  dm_sweeps = n >= 1: the textbook sequential overlap
+                # projection: Fourier step and object from the new psi (probe untouched), then the probe from the
+                # same psi and the NEW object; n - 1 more object/probe sweeps.
                 num = self.l.orc_dm_iteration(*self._dims(), C.c_int(self.J), _p(self.O), _p(self.P),
                                               _p(self.psi), _p(self.pos), _p(self.I), self.cr(self.eps_O),
-                                              self.cr(self.eps_P), C.c_int(upd), self.cr(p["pbound"]), _p(rev))
+                                              self.cr(self.eps_P), C.c_int(upd if sweeps == 0 else 0), self.cr(p["pbound"]), _p(rev))
+                for sw in range(sweeps):
+                    if sw > 0:
+                        self.l.orc_object_from_waves(*self._dims(), C.c_int(self.J), _p(self.O), _p(self.P), _p(self.psi),
+                                                     _p(self.pos), self.cr(self.eps_O))
+                    if upd:
+                        self.l.orc_probe_from_waves(*self._dims(), C.c_int(self.J), _p(self.O), _p(self.P), _p(self.psi),
+                                                    _p(self.pos), self.cr(self.eps_P))
             else:
                 self.psi = None
                 num = 0.0

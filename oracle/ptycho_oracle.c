@@ -376,3 +376,55 @@ double orc_minibatch_step(int alg, int H, int W, int n, int K, cplx *O, cplx *P,
     free(chi); free(ej); free(nO); free(dO); free(nP); free(dP);
     return tot;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Textbook (sequential) DM overlap projection, SURVEY 8(f) f1 / reading R4's alternative: after the
+ * Fourier step the object is formed from the new psi_j with the current probe, THEN the probe from the
+ * same psi_j with the NEW object, optionally repeated ("n inner sweeps").  PAPER.md:58 ("DM has to keep
+ * a copy of the previous calculation ... calculate the exit wavefronts of all the scan points at once")
+ * describes exactly this two-set alternation.  Both divisions are blended as in R5.
+ *   orc_object_from_waves : O <- (sum_j sum_k conj(P_k) psi_jk + eps_O O) / (sum_j sum_k |P_k|^2 + eps_O)
+ *   orc_probe_from_waves  : P_k <- (sum_j conj(O_j) psi_jk + eps_P P_k) / (sum_j |O_j|^2 + eps_P)
+ * ------------------------------------------------------------------------------------------ */
+void orc_object_from_waves(int H, int W, int n, int K, int J, cplx *O, const cplx *P, const cplx *psi,
+                           const int32_t *pos, real eps_O) {
+    const long np = (long)n * n, knp = K * np;
+    cplx *nO = (cplx *)calloc((size_t)H * W, sizeof(cplx));
+    real *dO = (real *)calloc((size_t)H * W, sizeof(real));
+    for (int j = 0; j < J; ++j) {
+        const int32_t *r = pos + 2 * j;
+        for (int y = 0; y < n; ++y)
+            for (int x = 0; x < n; ++x) {
+                long o = (long)(r[0] + y) * W + r[1] + x;
+                for (int k = 0; k < K; ++k) {
+                    cplx Pk = P[k * np + y * n + x];
+                    nO[o] += conj(Pk) * psi[j * knp + k * np + y * n + x];
+                    dO[o] += CABS2(Pk);
+                }
+            }
+    }
+    for (long o = 0; o < (long)H * W; ++o) O[o] = (nO[o] + eps_O * O[o]) / (dO[o] + eps_O);
+    free(nO); free(dO);
+}
+
+void orc_probe_from_waves(int H, int W, int n, int K, int J, const cplx *O, cplx *P, const cplx *psi,
+                          const int32_t *pos, real eps_P) {
+    (void)H;
+    const long np = (long)n * n, knp = K * np;
+    cplx *nP = (cplx *)calloc((size_t)knp, sizeof(cplx));
+    real *dP = (real *)calloc((size_t)np, sizeof(real));
+    for (int j = 0; j < J; ++j) {
+        const int32_t *r = pos + 2 * j;
+        for (int y = 0; y < n; ++y)
+            for (int x = 0; x < n; ++x) {
+                cplx Oj = O[(long)(r[0] + y) * W + r[1] + x];
+                for (int k = 0; k < K; ++k)
+                    nP[k * np + y * n + x] += conj(Oj) * psi[j * knp + k * np + y * n + x];
+                dP[y * n + x] += CABS2(Oj);
+            }
+    }
+    for (int k = 0; k < K; ++k)
+        for (long q = 0; q < np; ++q)
+            P[k * np + q] = (nP[k * np + q] + eps_P * P[k * np + q]) / (dP[q] + eps_P);
+    free(nP); free(dP);
+}

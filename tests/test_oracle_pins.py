@@ -411,3 +411,69 @@ def test_masked_pixels_are_excluded_from_sum_intensity(oracle_mod):
     assert o.sum_I == unmasked
     assert o.err[0] * unmasked == pytest.approx(num, rel=1e-12)
     assert abs(o.err[0] * float(cnt.astype(np.float64).sum()) - num) > 1e-3 * num   # the wrong denominator is far off
+
+
+# --------------------------------------------------------------------- f1: textbook variants
+def test_sequential_dm_overlap_closed_forms(oracle_mod):
+    """One sweep of the sequential overlap projection against the closed forms of S:8(c) "Overlap update": for consistent
+    waves psi_j = Q O*_j the object step returns (d_O O* + eps O_old)/(d_O + eps) -- with the probe it is given, Q -- and the
+    probe step, run with the NEW object, returns (d_P Q' + eps P_old)/(d_P + eps) where Q' solves psi_j = Q' O_new,j pixel by
+    pixel in the least-squares sense; here everything is typed with numpy slices.  All pixels masked: Pi_M = id."""
+    s, lam = f64_scan(n=8, h=22, side=3, step=4)
+    n = s.n
+    ostar = s.obj_true * (1 + 0.2 * crandn(*s.obj_true.shape))
+    q = s.probe_true * (1 + 0.3 * crandn(*s.probe_true.shape))
+    o_old = 1 + 0.1 * crandn(*s.obj_true.shape)
+    o = oracle_mod.Oracle(o_old, q, s.pos, -np.ones_like(lam), dict(dm_sweeps=1))
+    o.psi = np.stack([q * ostar[None, y:y + n, x:x + n] for y, x in s.pos]).astype(complex)
+    eps_o, eps_p = o.eps_O, o.eps_P
+    o.iterate("DM", 1)
+    # all-masked Fourier step: psi_new = psi + P O_old,j - P O_old,j ... = P O_old,j (reflector and update cancel, see the DM closed-form pin)
+    psi_new = np.stack([q * o_old[None, y:y + n, x:x + n] for y, x in s.pos])
+    assert rel(o.psi, psi_new) < 1e-13
+    d_o, n_o = np.zeros(o_old.shape), np.zeros_like(o_old)
+    for j, (y, x) in enumerate(s.pos):
+        d_o[y:y + n, x:x + n] += np.abs(q[0]) ** 2
+        n_o[y:y + n, x:x + n] += np.conj(q[0]) * psi_new[j, 0]
+    o_new = (n_o + eps_o * o_old) / (d_o + eps_o)
+    assert rel(o.O, o_new) < 1e-13
+    n_p, d_p = np.zeros_like(q[0]), np.zeros((n, n))
+    for j, (y, x) in enumerate(s.pos):
+        oj = o_new[y:y + n, x:x + n]                                             # the NEW object: sequential, not lagged
+        n_p += np.conj(oj) * psi_new[j, 0]
+        d_p += np.abs(oj) ** 2
+    assert rel(o.P[0], (n_p + eps_p * q[0]) / (d_p + eps_p)) < 1e-13
+    # two sweeps: the object is formed once more from the same waves with the new probe
+    o2 = oracle_mod.Oracle(o_old, q, s.pos, -np.ones_like(lam), dict(dm_sweeps=2))
+    o2.psi = np.stack([q * ostar[None, y:y + n, x:x + n] for y, x in s.pos]).astype(complex)
+    o2.iterate("DM", 1)
+    p1 = (n_p + eps_p * q[0]) / (d_p + eps_p)
+    d2, n2 = np.zeros(o_old.shape), np.zeros_like(o_old)
+    for j, (y, x) in enumerate(s.pos):
+        d2[y:y + n, x:x + n] += np.abs(p1) ** 2
+        n2[y:y + n, x:x + n] += np.conj(p1) * psi_new[j, 0]
+    assert rel(o2.O, (n2 + eps_o * o_new) / (d2 + eps_o)) < 1e-13
+
+
+def test_sequential_dm_fixed_point_and_decrease(oracle_mod):
+    s, lam = f64_scan()
+    o = oracle_mod.Oracle(s.obj_true, s.probe_true, s.pos, lam, dict(dm_sweeps=2)).iterate("DM", 2)
+    assert max(o.err) < 1e-25 and rel(o.O, s.obj_true) < 1e-13 and rel(o.P, s.probe_true) < 1e-13
+    c = synth.make_config(0)
+    e = np.array(oracle_mod.Oracle(c.obj0, c.probe0, c.pos, c.intensities, dict(dm_sweeps=1)).iterate("DM", 10).err)
+    assert np.all(np.diff(e[:8]) < 0) and e[-1] < 0.1 * e[0], e                  # SURVEY X2: the sequential form is monotone on cfg0
+
+
+def test_position_sequential_epie_is_single_frame_steps_in_sequence(oracle_mod):
+    """B = 1 (the paper's position-sequential ePIE): one iteration equals J single-frame oracles applied one
+    after the other to the running state, in scan order."""
+    s, lam = f64_scan(n=8, h=20, side=2, step=4)
+    cnt = RNG.poisson(lam * 30).astype(np.float64)
+    p0 = s.probe_true * np.sqrt(30)
+    obj0 = 1 + 0.1 * crandn(*s.obj_true.shape)
+    seq = oracle_mod.Oracle(obj0, p0, s.pos, cnt, dict(batch_size=1)).iterate("EPIE_MB", 1)
+    O, P = obj0.copy(), p0.copy()
+    for j in range(len(s.pos)):
+        one = oracle_mod.Oracle(O, P, s.pos[j:j + 1], cnt[j:j + 1]).iterate("EPIE_MB", 1)
+        O, P = one.O, one.P
+    assert rel(seq.O, O) < 1e-13 and rel(seq.P, P) < 1e-13

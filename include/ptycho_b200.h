@@ -77,6 +77,11 @@ typedef struct {
                            twice more per iteration.  Single-mode DM only: init returns
                            PTYCHO_EUNSUPPORTED for n_modes > 1 or disable_dm, iterate for the minibatch
                            algorithms.  0 = atomic scatter-add                                     */
+    int dm_sweeps;      /* DM overlap projection.  0 = reading R4: probe sums taken from the incoming exit waves (lagged),
+                           one pass over the exit waves per iteration.  n >= 1 = the textbook sequential form (SURVEY.md
+                           8(f) f1): object from the new exit waves, then the probe from the same waves and
+                           the NEW object, n sweeps; the exit waves are read once more per sweep (twice from the second
+                           sweep on).  Single-mode DM only (PTYCHO_EUNSUPPORTED otherwise)                        */
     const int32_t *batch_order; /* HOST pointer or NULL.  NULL: strided batches, n_b = ceil(J/B),
                            batch b = { j : j mod n_b = b } (R8).  Else a permutation of 0..J-1;
                            batch b = its entries [b*B, (b+1)*B).  Copied at init.                  */

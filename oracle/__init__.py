@@ -198,12 +198,29 @@ class Oracle:
 # pixels around (cy, cx), the noise threshold, the saturation mask, then numpy's ifftshift to put the centre
 # pixel at [0, 0] (reading R1: FFT order).  Pinned in tests/test_oracle_pins.py against index arithmetic done by
 # hand on a 6 x 6 example and against the fftshift/ifftshift involution.
-def prepare_frames(raw, center, n, threshold=0.0, saturation=0.0, out_dtype=np.uint16):
+def prepare_frames(raw, center, n, threshold=0.0, saturation=0.0, out_dtype=np.uint16, rot90=0, frame_scale=None):
+    """rot90 = k ("the rotation angles of the diffraction patterns"; multiples of 90 degrees only, R23): the
+    pattern is rotated counter-clockwise by k quarter turns about the centre pixel before the crop -- written here as numpy.rot90
+    of a window that has the centre pixel in its middle.  frame_scale ("diffraction pattern normalization", R24): one
+    factor per frame, applied to the counts that survive the threshold; masks are decided on the raw counts."""
     raw = np.asarray(raw)
     assert raw.ndim == 3 and n % 2 == 0
     f, dh, dw = raw.shape
     cy, cx = int(center[0]), int(center[1])
     h = n // 2
+    if rot90 % 4:
+        # window of (2n + 1)^2 pixels centred on (cy, cx), outside the detector = masked; rotate it; go on with the rotated window
+        m = n
+        big = np.full((f, 2 * m + 1, 2 * m + 1), 65535 if raw.dtype == np.uint16 else -1, raw.dtype)
+        for iy in range(2 * m + 1):
+            sy = cy - m + iy
+            if 0 <= sy < dh:
+                for ix in range(2 * m + 1):
+                    sx = cx - m + ix
+                    if 0 <= sx < dw:
+                        big[:, iy, ix] = raw[:, sy, sx]
+        raw, (cy, cx) = np.rot90(big, rot90 % 4, axes=(1, 2)), (m, m)
+        dh = dw = 2 * m + 1
     val = np.zeros((f, n, n), np.float64)
     masked = np.ones((f, n, n), bool)                      # outside the detector: masked
     for iy in range(n):                                    # plain loops over the crop window (slow, obvious)
@@ -220,6 +237,8 @@ def prepare_frames(raw, center, n, threshold=0.0, saturation=0.0, out_dtype=np.u
                 m = m | (v >= np.float32(saturation))
             if threshold > 0:
                 v = np.where(v < np.float32(threshold), 0.0, v)
+            if frame_scale is not None:
+                v = (v.astype(np.float32) * np.asarray(frame_scale, np.float32)).astype(np.float64)   # fp32 product, like any fp32 path
             val[:, iy, ix] = v
             masked[:, iy, ix] = m
     val = np.fft.ifftshift(val, axes=(1, 2))               # centre pixel (index h) -> index 0

@@ -38,7 +38,8 @@ class Params(C.Structure):
     _fields_ = [("batch_size", C.c_int), ("probe_start", C.c_int), ("delta_blend", C.c_float),
                 ("delta_obj", C.c_float), ("delta_probe", C.c_float), ("alpha_obj", C.c_float),
                 ("alpha_probe", C.c_float), ("lsq_lambda", C.c_float), ("pbound", C.c_float),
-                ("disable_dm", C.c_int), ("deterministic", C.c_int), ("batch_order", C.POINTER(C.c_int32))]
+                ("disable_dm", C.c_int), ("deterministic", C.c_int), ("dm_sweeps", C.c_int),
+                ("batch_order", C.POINTER(C.c_int32))]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

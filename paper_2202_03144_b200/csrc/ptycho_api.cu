@@ -52,6 +52,7 @@ struct ptycho_ctx {
     float2 *tw = nullptr, *twi = nullptr;
     YX* pos = nullptr;
     int *tile_start = nullptr, *tile_mid = nullptr, *tile_list = nullptr;   // frames per object tile (CSR; see ptycho_init)
+    int* tile_slots = nullptr;                 // dm_sweeps > 0: the same CSR with slots as entries, ascending (k_det_object)
     float4* det_partial = nullptr;
     int det_tx = 0, det_ty = 0;
     void* It = nullptr;                        // intensities re-tiled for the DM megakernel
@@ -227,7 +228,8 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
         c->tile_start = w.take<int>((size_t)c->det_tx * c->det_ty + 1);
         c->tile_mid = w.take<int>((size_t)c->det_tx * c->det_ty);
         c->tile_list = w.take<int>((size_t)c->J * (c->N / kDetTileW + 1) * (c->N / kDetTileH + 1));   // upper bound
-        if (c->par.deterministic) c->det_partial = w.take<float4>((size_t)kDetGroups * nn);
+        if (c->par.deterministic || c->par.dm_sweeps > 0) c->det_partial = w.take<float4>((size_t)kDetGroups * nn);
+        if (c->par.dm_sweeps > 0) c->tile_slots = w.take<int>((size_t)c->J * (c->N / kDetTileW + 1) * (c->N / kDetTileH + 1));
     }
     if (copy_I) c->I = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
     return (w.off + 255) & ~size_t(255);
@@ -344,7 +346,8 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         m.f.psi = c->psi; m.f.frames = c->dm_frames; m.f.e_part = c->e_part;
         m.J = c->J; m.M = c->mega_M; m.D = c->mega_D; m.R = c->mega_R; m.nW = (c->J + m.M - 1) / m.M;
         const int det = c->par.deterministic;
-        m.update_probe = det ? 0 : upd;
+        const int seq = c->par.dm_sweeps;                   // > 0: textbook sequential overlap projection
+        m.update_probe = (det || seq) ? 0 : upd;
         m.det = det;
         m.corr = c->p2 ? 1 : 0;
         m.fresh = fresh_in_kernel ? 1 : 0;
@@ -392,6 +395,24 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
     }
     else
         LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(HW), 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1)));
+    if (c->par.dm_sweeps > 0 && c->mega_M > 0) {
+        // sequential form: the object above came from the new exit waves with the old probe; now the probe from the same waves
+        // and the NEW object (fixed-order gathers of dm_det.cuh), then further object / probe sweeps.
+        for (int sw = 0; sw < c->par.dm_sweeps; ++sw) {
+            if (sw > 0) {
+                LAUNCH(c, PTYCHO_K_OTHER, (k_det_object<<<dim3(c->det_tx, c->det_ty), dim3(kDetTileW, kDetTileH), 0, c->stream>>>(
+                                               c->nO, c->dO, c->H, c->W, c->psi, c->P, c->N, c->spos, c->tile_start, c->tile_slots)));
+                LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(HW), 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->sc, 0, 1)));
+            }
+            if (upd) {
+                LAUNCH(c, PTYCHO_K_OTHER, (k_det_probe<<<dim3((unsigned)((nn + 255) / 256), kDetGroups), 256, 0, c->stream>>>(
+                                               c->det_partial, c->psi, c->O, c->W, c->N, c->spos, c->J)));
+                LAUNCH(c, PTYCHO_K_OTHER, (k_det_probe_final<<<(unsigned)((nn + 255) / 256), 256, 0, c->stream>>>(c->nP, c->dP, c->det_partial, (int)nn, kDetGroups)));
+                LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(nn), 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, 1)));
+            }
+        }
+        return PTYCHO_OK;
+    }
     LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(nn), 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd)));
     return PTYCHO_OK;
 }
@@ -485,6 +506,8 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
         return PTYCHO_EINVAL;
     // deterministic mode (dm_det.cuh) is built for the single-mode DM megakernel path only
     if (par.deterministic && (n_modes != 1 || par.disable_dm || !env_int("PTYCHO_MEGA", 1))) return PTYCHO_EUNSUPPORTED;
+    if (par.dm_sweeps < 0) return PTYCHO_EINVAL;
+    if (par.dm_sweeps > 0 && (n_modes != 1 || par.disable_dm || par.deterministic)) return PTYCHO_EUNSUPPORTED;
     if (cols_smem(n, n_modes) > 227 * 1024) return PTYCHO_EUNSUPPORTED;
 
     // positions: copy, check bounds (R10), accept host or device memory
@@ -586,16 +609,18 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
         // y << 16 | x, and the frames that cover the WHOLE tile come first (tile_mid marks the boundary): no per-pixel test for them.
         const bool gather = !par.deterministic;
         const size_t ntiles = (size_t)c->det_tx * c->det_ty;
-        std::vector<int> start(ntiles + 1, 0), mid(ntiles, 0), list;
+        std::vector<int> start(ntiles + 1, 0), mid(ntiles, 0), list, slots;
+        const bool want_slots = gather && par.dm_sweeps > 0;
         auto whole = [&](int y, int x, int ty, int tx) {
             return y <= ty * kDetTileH && (ty + 1) * kDetTileH <= y + n && x <= tx * kDetTileW && (tx + 1) * kDetTileW <= x + n;
         };
         for (int pass = 0; pass < 2; ++pass) {
-            std::vector<int> fill_a, fill_b;
+            std::vector<int> fill_a, fill_b, fill_s;
             if (pass == 1) {
                 fill_a.assign(start.begin(), start.end() - 1);
                 fill_b.resize(ntiles);
                 for (size_t i = 0; i < ntiles; ++i) { fill_b[i] = start[i] + mid[i]; mid[i] = fill_b[i]; }
+                if (want_slots) fill_s.assign(start.begin(), start.end() - 1);
             }
             for (int sidx = 0; sidx < n_pos; ++sidx) {
                 const int y = spos[2 * sidx], x = spos[2 * sidx + 1];
@@ -603,14 +628,16 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
                     for (int tx = x / kDetTileW; tx <= (x + n - 1) / kDetTileW; ++tx) {
                         const size_t tl = (size_t)ty * c->det_tx + tx;
                         const bool w = gather && whole(y, x, ty, tx);
-                        if (pass == 0) { ++start[tl + 1]; if (w) ++mid[tl]; }
-                        else if (!gather) list[fill_a[tl]++] = sidx;
+                        if (pass == 0) { ++start[tl + 1]; if (w) ++mid[tl]; continue; }
+                        if (want_slots) slots[fill_s[tl]++] = sidx;
+                        if (!gather) list[fill_a[tl]++] = sidx;
                         else if (w) list[fill_a[tl]++] = (y << 16) | x;
                         else list[fill_b[tl]++] = (y << 16) | x;
                     }
             }
-            if (pass == 0) { for (size_t i = 0; i < ntiles; ++i) start[i + 1] += start[i]; list.resize(start[ntiles]); }
+            if (pass == 0) { for (size_t i = 0; i < ntiles; ++i) start[i + 1] += start[i]; list.resize(start[ntiles]); if (want_slots) slots.resize(start[ntiles]); }
         }
+        if (want_slots) CUI(cudaMemcpyAsync(c->tile_slots, slots.data(), slots.size() * 4, cudaMemcpyHostToDevice, s));
         CUI(cudaMemcpyAsync(c->tile_start, start.data(), start.size() * 4, cudaMemcpyHostToDevice, s));
         CUI(cudaMemcpyAsync(c->tile_mid, mid.data(), mid.size() * 4, cudaMemcpyHostToDevice, s));
         CUI(cudaMemcpyAsync(c->tile_list, list.data(), list.size() * 4, cudaMemcpyHostToDevice, s));

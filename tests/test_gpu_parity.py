@@ -517,3 +517,36 @@ def test_handoff_stress_deterministic_bitwise(B, monkeypatch):
         got = run()
         for a, b in zip(got, ref):
             assert np.array_equal(a, b), (M, D, X)
+
+
+# ------------------------------------------------------------------ f1: textbook variants
+@pytest.mark.parametrize("sweeps", [1, 2])
+def test_sequential_dm_overlap_projection(B, oracle_mod, sweeps):
+    """dm_sweeps = n: object from the new exit waves, then the probe from the same waves and the NEW object, n sweeps."""
+    s = synth.make_custom(128, 420, 7, 37, k=1, peak=2e4, dtype=np.uint16, jitter=3, seed=41, probe_kind="zone")
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(pbound=0.3, dm_sweeps=sweeps))
+    g = make(B, s, pbound=0.3, dm_sweeps=sweeps)
+    lit = well_lit(s)
+    for it in range(5):
+        if it:                                                  # teacher-forced: per-iteration tolerance
+            g.set_object(o.O); g.set_probe(o.P); g.set_exit_waves(o.psi.astype(np.complex64))
+        o.iterate("DM", 1)
+        g.iterate("DM", 1)
+        Og = g.fetch_object()
+        assert rel(Og, o.O) < TOL_ITER and rel(Og[lit], o.O[lit]) < TOL_ITER and rel(g.fetch_probe(), o.P) < TOL_ITER, it
+        assert rel(g.fetch_exit_waves(), o.psi) < TOL_ITER, it
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+    with pytest.raises(B.PtychoError, match="EUNSUPPORTED"):
+        B.Ptycho(s.obj0, np.concatenate([s.probe0, s.probe0]), s.pos, s.intensities, B.default_params(dm_sweeps=1))
+
+
+def test_position_sequential_epie(B, oracle_mod):
+    """B = 1: the paper's position-sequential ePIE through the minibatch path, one frame per batch."""
+    s = synth.make_custom(64, 200, 5, 24, k=1, peak=2e4, dtype=np.float32, jitter=2, seed=43, probe_kind="disk")
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(batch_size=1))
+    g = make(B, s, batch_size=1)
+    for it in range(3):
+        o.iterate("EPIE_MB", 1)
+        g.iterate("EPIE_MB", 1)
+        assert rel(g.fetch_object(), o.O) < TOL_ITER * (it + 1) and rel(g.fetch_probe(), o.P) < TOL_ITER * (it + 1), it
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)

@@ -477,3 +477,30 @@ def test_position_sequential_epie_is_single_frame_steps_in_sequence(oracle_mod):
         one = oracle_mod.Oracle(O, P, s.pos[j:j + 1], cnt[j:j + 1]).iterate("EPIE_MB", 1)
         O, P = one.O, one.P
     assert rel(seq.O, O) < 1e-13 and rel(seq.P, P) < 1e-13
+
+
+def test_prepare_frames_rotation_and_normalisation_by_hand(oracle_mod):
+    """rot90 (R23) and frame_scale (R24) on a 7 x 7 detector indexed by hand.  Centre (3, 3), n = 4.  A quarter turn
+    counter-clockwise (numpy.rot90 convention: the pixel to the RIGHT of the centre moves to ABOVE it) means the output pixel at
+    centred offset (dy, dx) comes from the source pixel at offset (dx, -dy); two turns: (-dy, -dx); three: (-dx, dy)."""
+    raw = (np.arange(49, dtype=np.uint16).reshape(1, 7, 7) + 100)
+    c = (3, 3)
+    off = [0, 1, -2, -1]                                   # centred offset of FFT-order index 0..3
+    src = {0: lambda dy, dx: (dy, dx), 1: lambda dy, dx: (dx, -dy), 2: lambda dy, dx: (-dy, -dx), 3: lambda dy, dx: (-dx, dy)}
+    for k in range(4):
+        out = oracle_mod.prepare_frames(raw, c, 4, rot90=k)
+        want = np.array([[raw[0, 3 + src[k](dy, dx)[0], 3 + src[k](dy, dx)[1]] for dx in off] for dy in off], np.uint16)
+        assert np.array_equal(out[0], want), k
+    # the defining property, on one pixel: right of the centre (offset (0, +1), value raw[3, 4]) lands above it (offset (-1, 0))
+    assert oracle_mod.prepare_frames(raw, c, 4, rot90=1)[0, 3, 0] == raw[0, 3, 4]
+    # rotation about an off-centre pixel near the edge: what leaves the detector is masked
+    edge = oracle_mod.prepare_frames(raw, (0, 6), 4, rot90=1)
+    # (dy, dx) = (1, 0) <- source offset (0, -1) = raw[0, 5]; (0, 1) <- (1, 0) = raw[1, 6]; (0, -1) <- (-1, 0): row -1, off the detector
+    assert edge[0, 0, 0] == raw[0, 0, 6] and edge[0, 1, 0] == raw[0, 0, 5] and edge[0, 0, 1] == raw[0, 1, 6] and edge[0, 0, 3] == 65535
+    # normalisation: one factor per frame, after the threshold, fp32 product rounded to nearest for uint16
+    two = np.concatenate([raw, raw])
+    sc = oracle_mod.prepare_frames(two, c, 4, threshold=125.0, frame_scale=np.array([1.0, 0.5], np.float32))
+    assert sc[1, 0, 1] == round(float(raw[0, 3, 4]) * 0.5) and sc[0, 0, 1] == raw[0, 3, 4]       # 125 -> 62 (round half to even: 62.5 -> 62)
+    assert sc[1, 0, 0] == 0 and sc[0, 0, 0] == 0                                                    # 124 < threshold -> 0 in both
+    f32 = oracle_mod.prepare_frames(two.astype(np.float32), c, 4, frame_scale=np.array([2.0, 0.25], np.float32), out_dtype=np.float32)
+    assert f32[0, 0, 0] == 248.0 and f32[1, 0, 0] == 31.0

@@ -91,8 +91,8 @@ void ptycho_default_params(ptycho_params *p);
 
 /* Bytes of device workspace ptycho_init needs for these sizes (0 on invalid sizes).  It holds
  * O, P, the DM exit-wave store (J*K*N*N complex64), the overlap canvases, the transform scratch,
- * the sort tables and, if the intensities are passed from host memory, a copy of them
- * (`intensities_on_host` != 0). */
+ * the sort tables and, if the intensities are passed from host memory AND disable_dm is set, a copy of them (otherwise the copy is staged in the exit-wave store during init)
+ * (`intensities_on_host`: 0 = device pointer, 1 = host pointer, 2 = none at init: streaming context, see ptycho_append_frames). */
 size_t ptycho_workspace_bytes(int obj_h, int obj_w, int n, int n_modes, int n_pos,
                               ptycho_itype itype, int intensities_on_host,
                               const ptycho_params *params /* NULL = defaults */);
@@ -146,6 +146,21 @@ ptycho_status ptycho_set_exit_waves(ptycho_ctx *ctx, const float *psi /* n_pos*n
  * state change; R7).  Synchronises. */
 ptycho_status ptycho_eval_error(ptycho_ctx *ctx, double *out);
 
+/* ---- streaming ingestion ----
+ * PAPER.md:9 ("several TB's of data per second ... processed in real time") and PAPER.md:29 (3 kHz frames, 6 GB/s raw data): the
+ * frames of a scan arrive while the reconstruction already runs.  A context created with intensities == NULL (and a workspace
+ * sized with intensities_on_host = 2) knows every position but holds no frame.  ptycho_append_frames hands over the next `count`
+ * frames, first_frame == ptycho_frames_present(ctx) (acquisition order, no gaps; PTYCHO_EINVAL otherwise).  The call returns at
+ * once: the host->device copy (through a 64 MB staging piece of the workspace), the re-tiling and the intensity sum run on a
+ * copy stream of the context, so they overlap a ptycho_iterate that is in flight on the context's stream; `intensities` (host,
+ * pinned for a truly asynchronous copy, or device) must stay valid until ptycho_wait_frames returns.  ptycho_iterate waits
+ * (on the device) for the frames appended before the call and works on frames [0, present): the minibatch algorithms form their
+ * batches over those frames (R8 with J = present); PTYCHO_DM needs every frame and returns PTYCHO_ESTATE earlier,
+ * as do ptycho_eval_error and a call with no frame present. */
+ptycho_status ptycho_append_frames(ptycho_ctx *ctx, int first_frame, int count, const void *intensities);
+ptycho_status ptycho_wait_frames(ptycho_ctx *ctx);     /* blocks until every appended frame is on the device */
+int ptycho_frames_present(const ptycho_ctx *ctx);
+
 /* Per-kernel-class device timing (SURVEY.md 8(d) "Evidence to collect"; bench.py's roofline
  * object).  ptycho_profile(ctx, 1) resets the totals and makes every later launch of this context
  * be bracketed by two cudaEvents on the context's stream; ptycho_profile(ctx, 0) stops that.
@@ -166,7 +181,7 @@ ptycho_status ptycho_profile_fetch(ptycho_ctx *ctx, int kclass, double *total_ms
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 long long ptycho_launch_count(const ptycho_ctx *ctx);
 
-const char *ptycho_last_error(const ptycho_ctx *ctx); /* never NULL; "" if none */
+const char *ptycho_last_error(const ptycho_ctx *ctx); /* never NULL; "" if none; ctx == NULL: the last failing ptycho_init */
 void ptycho_destroy(ptycho_ctx *ctx);                 /* frees host state; the workspace is the caller's */
 
 /* ---- init-time preparation of raw detector frames (first item beyond the hot path) ----
@@ -175,18 +190,27 @@ void ptycho_destroy(ptycho_ctx *ctx);                 /* frees host state; the w
  * pixels are detected from the detector bit depth.  This call does that on the GPU and writes the
  * intensities in the layout ptycho_init takes (reading R1: FFT order, DC at [0,0]; reading R3: masked
  * pixels carry the sentinel 65535 (uint16) or -1 (fp32)).  For output pixel (ky, kx), 0 <= ky, kx < n:
- *     sy = center_y + (ky < n/2 ? ky : ky - n),   sx = center_x + (kx < n/2 ? kx : kx - n)
+ *     dy = ky < n/2 ? ky : ky - n,   dx = kx < n/2 ? kx : kx - n        (offset from the centre pixel)
+ *     (uy, ux) = (dy, dx), (dx, -dy), (-dy, -dx), (-dx, dy) for rot90 = 0, 1, 2, 3: the pattern turned counter-clockwise by
+ *                rot90 quarter turns about the centre pixel ("the rotation angles of the diffraction patterns";
+ *                multiples of 90 degrees only, reading R23: any other angle needs an interpolation rule the paper does not give)
+ *     sy = center_y + uy,   sx = center_x + ux
  *     v  = raw[frame][sy][sx]            (a source pixel outside the detector, or a raw value that already is
  *                                         the sentinel -- 65535 in uint16, negative in fp32: masked)
  *     saturation > 0 and v >= saturation : masked
  *     threshold  > 0 and v <  threshold  : 0
- *     otherwise v (uint16 output: rounded to nearest, clipped to 65534)
+ *     otherwise v
+ *     frame_scale != NULL: v <- v * frame_scale[frame] in fp32 ("diffraction pattern normalization"; reading R24:
+ *                one factor per frame, e.g. monitor / exposure normalisation, applied after the threshold; masks are decided
+ *                on the raw counts)
+ *     uint16 output: rounded to nearest (ties to even), clipped to 65534
  * raw: n_frames x det_h x det_w, uint16 or fp32, row-major, host or device; out: n_frames x n x n, host or
  * device; n is any even size >= 2 (not only the FFT sizes).  Integer / byte work: results are bit-exact
  * against the oracle.  Synchronises the stream before returning.  PTYCHO_EINVAL on null pointers, odd n,
- * non-positive sizes or unknown types. */
+ * non-positive sizes, rot90 outside 0..3 or unknown types. */
 ptycho_status ptycho_prepare_frames(const void *raw, ptycho_itype raw_type, int n_frames, int det_h, int det_w,
                                     int center_y, int center_x, int n, float threshold, float saturation,
+                                    int rot90, const float *frame_scale /* n_frames floats, host or device, or NULL */,
                                     void *out, ptycho_itype out_type, void *cuda_stream);
 
 /* Unit-test entry points of single kernels (tier T2).  Device pointers. */

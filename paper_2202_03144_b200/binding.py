@@ -85,10 +85,13 @@ def lib():
         l.ptycho_last_error.restype = C.c_char_p
         l.ptycho_last_error.argtypes = [C.c_void_p]
         l.ptycho_destroy.argtypes = [C.c_void_p]
+        l.ptycho_append_frames.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        l.ptycho_wait_frames.argtypes = [C.c_void_p]
+        l.ptycho_frames_present.argtypes = [C.c_void_p]
         l.ptycho_default_params.argtypes = [C.POINTER(Params)]
         l.ptycho_test_fft2.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
         l.ptycho_prepare_frames.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float,
-                                            C.c_float, C.c_void_p, C.c_int, C.c_void_p]
+                                            C.c_float, C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         _lib = l
     return _lib
 
@@ -130,7 +133,8 @@ def _c64(a):
 class Ptycho:
     """One reconstruction context (ptycho_ctx).  Arrays may be numpy (host) or torch (host/device)."""
 
-    def __init__(self, obj, probe, pos, intensities, params: Params | None = None, stream=None, device="cuda:0"):
+    def __init__(self, obj, probe, pos, intensities, params: Params | None = None, stream=None, device="cuda:0", stream_dtype=None):
+        """intensities = None with stream_dtype (np.uint16 / np.float32): a streaming context, frames come through append_frames."""
         import torch
         if not torch.cuda.is_available():
             raise PtychoError(5, "no CUDA device: the projection cycle has no CPU path")
@@ -144,12 +148,12 @@ class Ptycho:
         self.K, self.n = probe.shape[0], probe.shape[-1]
         pos = np.ascontiguousarray(pos, np.int32) if isinstance(pos, np.ndarray) else pos.contiguous()
         self.J = pos.shape[0]
-        dt = intensities.dtype
+        dt = np.dtype(stream_dtype) if intensities is None else intensities.dtype
         self.itype = 1 if str(dt).endswith("uint16") else 0
         if self.itype == 0:
             assert str(dt).endswith("float32"), "intensities must be float32 or uint16"
         self._I = intensities if not isinstance(intensities, np.ndarray) else np.ascontiguousarray(intensities)
-        on_host = isinstance(self._I, np.ndarray) or not self._I.is_cuda
+        on_host = 2 if intensities is None else (isinstance(self._I, np.ndarray) or not self._I.is_cuda)
         self.params = params if params is not None else default_params()
         need = self._l.ptycho_workspace_bytes(self.H, self.W, self.n, self.K, self.J, self.itype, int(on_host),
                                               C.byref(self.params))
@@ -163,10 +167,21 @@ class Ptycho:
                                      self.J, _ptr(self._I), self.itype, C.byref(self.params),
                                      C.c_void_p(self.workspace.data_ptr()), need, C.c_void_p(self._stream.cuda_stream))
         if st != 0:
-            raise PtychoError(st, "ptycho_init")
+            raise PtychoError(st, "ptycho_init: " + lib().ptycho_last_error(None).decode())
         self._h = h
 
     # ---- the calls of the C ABI, same names -------------------------------------------------
+    def append_frames(self, first_frame: int, intensities):
+        intensities = intensities if not isinstance(intensities, np.ndarray) else np.ascontiguousarray(intensities)
+        self._keep = intensities                                # must stay valid until wait_frames()
+        self._check(self._l.ptycho_append_frames(self._h, int(first_frame), int(intensities.shape[0]), _ptr(intensities)))
+
+    def wait_frames(self):
+        self._check(self._l.ptycho_wait_frames(self._h))
+
+    def frames_present(self) -> int:
+        return int(self._l.ptycho_frames_present(self._h))
+
     def _check(self, st):
         if st != 0:
             raise PtychoError(st, self._l.ptycho_last_error(self._h).decode())
@@ -263,7 +278,8 @@ class Ptycho:
             pass
 
 
-def prepare_frames(raw, center, n: int, threshold: float = 0.0, saturation: float = 0.0, out_dtype=np.uint16, out=None):
+def prepare_frames(raw, center, n: int, threshold: float = 0.0, saturation: float = 0.0, out_dtype=np.uint16, out=None,
+                   rot90: int = 0, frame_scale=None):
     """ptycho_prepare_frames: raw detector frames (F, det_h, det_w), uint16 or float32, numpy or torch CUDA ->
     FFT-order intensities (F, n, n) with masked pixels as the sentinel.  Marshalling only."""
     import torch
@@ -277,8 +293,10 @@ def prepare_frames(raw, center, n: int, threshold: float = 0.0, saturation: floa
         out = (torch.empty((f, n, n), dtype=torch.uint16 if itype(out_dtype) else torch.float32, device=raw.device) if is_t
                else np.empty((f, n, n), np.uint16 if itype(out_dtype) else np.float32))
     stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+    if frame_scale is not None and not is_t:
+        frame_scale = np.ascontiguousarray(frame_scale, np.float32)
     st = lib().ptycho_prepare_frames(_ptr(raw), itype(raw.dtype), f, dh, dw, int(center[0]), int(center[1]), int(n), float(threshold),
-                                     float(saturation), _ptr(out), itype(out.dtype), C.c_void_p(stream))
+                                     float(saturation), int(rot90), _ptr(frame_scale), _ptr(out), itype(out.dtype), C.c_void_p(stream))
     if st != 0:
         raise PtychoError(st, "ptycho_prepare_frames")
     return out

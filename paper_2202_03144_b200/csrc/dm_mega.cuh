@@ -25,6 +25,13 @@
 
 namespace ptycho {
 
+// Experiment switches (m.flags: 1 = no L2 prefetch, 4 = immediate signals) exist in debug builds only (-DPTYCHO_DEBUG).
+#ifdef PTYCHO_DEBUG
+#define MEGA_FLAG(m, bit) ((m).flags & (bit))
+#else
+#define MEGA_FLAG(m, bit) 0
+#endif
+
 struct MegaArgs {
     FrameArgs f;        // psi = slot 0 of the store; S = ring base; frames = slot -> caller frame; e_part [J][NCB]
     int J, M, D, R, nW;
@@ -33,7 +40,7 @@ struct MegaArgs {
     int corr;           // object canvas holds only the correction sum_j keep_j conj(P) v_j; d_O is gathered by k_dm_blend_gather (dm_det.cuh)
     int det;            // deterministic mode: no floating-point atomics here (dm_det.cuh forms the overlap sums)
     int pf;             // slots ahead that the L2 prefetches reach (megakernel: M, the next wave; split kernels: the next chunk)
-    int flags;          // experiment switches: 1 = no L2 prefetch, 4 = immediate signals
+    int flags;          // experiment switches (debug builds only): 1 = no L2 prefetch, 4 = immediate signals
     const void* It;     // intensities re-tiled at init into pass-2 register order (k_tile_intensity)
     const YX* spos;     // [J] position of each SLOT (pos[frames[slot]], one load instead of two chained)
     int* head;          // queue head
@@ -162,6 +169,20 @@ template <int N, typename TI> __global__ void __launch_bounds__(kThreads) k_tile
     for (int r = 0; r < E; ++r) dst[((size_t)(r / EPC) * kThreads + tid) * EPC + r % EPC] = src[(size_t)freq_b<N>(t, r) * N];
 }
 
+// The same re-tiling for a chunk of appended frames (streaming ingestion): frame `first + blockIdx.x` of the caller's numbering,
+// read from the staged chunk, written to its slot.
+template <int N, typename TI> __global__ void __launch_bounds__(kThreads) k_tile_intensity_chunk(TI* __restrict__ out, const TI* __restrict__ chunk,
+                                                                                                  const int* __restrict__ slot_of, int first) {
+    using G = Geo<N>;
+    constexpr int E = G::E, CB = G::LPB, EPC = 16 / (int)sizeof(TI);
+    const int slot = slot_of[first + blockIdx.x], blk = blockIdx.y, tid = threadIdx.x;
+    const int c = tid % CB, t = tid / CB;
+    const TI* src = chunk + (size_t)blockIdx.x * N * N + blk * CB + c;
+    TI* dst = out + ((size_t)slot * G::NCB + blk) * N * CB;
+#pragma unroll
+    for (int r = 0; r < E; ++r) dst[((size_t)(r / EPC) * kThreads + tid) * EPC + r % EPC] = src[(size_t)freq_b<N>(t, r) * N];
+}
+
 template <int N> struct MegaGeo {
     using G = Geo<N>;
     static constexpr int LINE = (G::LS_ROW > G::LS_COL ? G::LS_ROW : G::LS_COL);
@@ -189,7 +210,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(co
     __syncwarp();
     {   // psi of the NEXT wave's slots (this warp's lines): start HBM -> L2 now
         const int s = s_begin + m.pf + lane;
-        if (!(m.flags & 1) && lane < m.M && s < m.J)
+        if (!MEGA_FLAG(m, 1) && lane < m.M && s < m.J)
             l2_prefetch_bulk(a.psi + (size_t)s * N * N + (size_t)(blk * G::LPB + (threadIdx.x >> 5) * LW) * N, LW * N * 8);
     }
     PhaseClock pc;
@@ -227,7 +248,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(co
 #pragma unroll
         for (int r = 0; r < E; ++r) __stcg(srow + freq_b<N>(t, r), v[r]);
         if (SYNC) df.cnt = m.cnt1 + slot;
-        if (m.flags & 4) df.flush_warp();
+        if (MEGA_FLAG(m, 4)) df.flush_warp();
         pc.lap(3);
     }
     if (m.update_probe) {
@@ -256,7 +277,7 @@ template <int N, bool U16, int MODE, bool SYNC = true> __device__ __forceinline_
     constexpr float kAmp2Floor = 1e-30f;
     const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
     const size_t tile_bytes = (size_t)N * CB * (U16 ? 2 : 4);   // this block's intensities of one slot: contiguous
-    if (!(m.flags & 1) && threadIdx.x < m.M) {                              // I of the NEXT wave: HBM -> L2 now
+    if (!MEGA_FLAG(m, 1) && threadIdx.x < m.M) {                              // I of the NEXT wave: HBM -> L2 now
         const int s = s_begin + m.pf + threadIdx.x;
         if (s < m.J) l2_prefetch_bulk(reinterpret_cast<const char*>(m.It) + ((size_t)s * G::NCB + blk) * tile_bytes, (uint32_t)tile_bytes);
     }
@@ -332,7 +353,7 @@ template <int N, bool U16, int MODE, bool SYNC = true> __device__ __forceinline_
         for (int r = 0; r < E; ++r) __stcg(base + (size_t)pos_a_inv<N>(t, r) * N, v[r]);
         __syncthreads();                                                    // sx and s_red free; stores issued by all
         if (SYNC) df.cnt = m.cnt2 + slot;
-        if (m.flags & 4) df.flush_cta_after_barrier();
+        if (MEGA_FLAG(m, 4)) df.flush_cta_after_barrier();
         pc.lap(3);
     }
 }

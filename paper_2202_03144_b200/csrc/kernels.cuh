@@ -374,7 +374,8 @@ struct Scalars {            // device-resident scalars (no host round trip insid
     float max_p2;           // max_r sum_k |P_k|^2 of the current probe
     float max_dp;           // max_r d_P of the current batch
     float step_a, step_b;   // steps applied by the apply kernels
-    double sum_I;           // sum of unmasked intensities
+    double sum_I;           // sum of unmasked intensities of the frames present
+    double sum_I_iter;      // its value when the running iteration started (frames may be appended meanwhile)
     float eps_O, eps_P;     // DM blend constants (fixed at init)
     unsigned int max_bits;  // scratch for atomicMax on non-negative floats
 };
@@ -540,11 +541,13 @@ __global__ void k_sum_intensity(const void* __restrict__ I, int itype, size_t co
     __syncthreads();
     if (threadIdx.x == 0) { for (int w = 1; w < (int)blockDim.x / 32; ++w) acc += sa[w]; part[blockIdx.x] = acc; }
 }
-__global__ void k_finish_sum_I(const double* part, int n, Scalars* sc) {
-    if (threadIdx.x || blockIdx.x) return;
-    double s = 0; for (int i = 0; i < n; ++i) s += part[i];
-    sc->sum_I = s;
+__global__ void k_finish_sum_I(const double* part, int n, Scalars* sc, int accumulate) {   // one warp, fixed order
+    double s = 0;
+    for (int i = threadIdx.x; i < n; i += 32) s += part[i];
+    for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+    if (threadIdx.x == 0) sc->sum_I = accumulate ? sc->sum_I + s : s;
 }
+__global__ void k_snap_sum_I(Scalars* sc) { sc->sum_I_iter = sc->sum_I; }
 // E_t = (sum of all error partials, fixed order, double) / sum_I.  Two steps, both in a fixed order: kErrBlocks CTAs each
 // reduce a contiguous piece to part[block]; the last CTA to finish (atomic ticket) adds the pieces in index order.
 constexpr int kErrBlocks = 148;
@@ -569,7 +572,7 @@ __global__ void __launch_bounds__(1024) k_sum_error(const float* __restrict__ e_
     __threadfence();
     double tot = 0.0;
     for (unsigned b = 0; b < gridDim.x; ++b) tot += __ldcg(part + b);
-    *out = tot / (sc->sum_I > 0 ? sc->sum_I : 1.0);
+    *out = tot / (sc->sum_I_iter > 0 ? sc->sum_I_iter : 1.0);
     *ticket = 0;
 }
 __global__ void k_finish_init(Scalars* sc, float delta, int J, int which) {
@@ -581,8 +584,18 @@ __global__ void k_finish_init(Scalars* sc, float delta, int J, int which) {
 // ------------------------------------------------------------------------------------------
 // init-time preparation of raw detector frames (include/ptycho_b200.h: ptycho_prepare_frames)
 // ------------------------------------------------------------------------------------------
+// (uy, ux) = source offset from the centre pixel for the output offset (dy, dx) after `rot` quarter turns counter-clockwise
+// (R23; numpy.rot90 convention).
+__device__ __forceinline__ void rot_offset(int rot, int dy, int dx, int& uy, int& ux) {
+    switch (rot & 3) {
+        case 0: uy = dy; ux = dx; break;
+        case 1: uy = dx; ux = -dy; break;
+        case 2: uy = -dy; ux = -dx; break;
+        default: uy = -dx; ux = dy; break;
+    }
+}
 template <typename TI, typename TO> __device__ __forceinline__ TO prepare_pixel(const TI* __restrict__ raw, size_t f, int det_h, int det_w, int sy,
-                                                                                 int sx, float threshold, float saturation) {
+                                                                                 int sx, float threshold, float saturation, float scale) {
     bool masked = sy < 0 || sx < 0 || sy >= det_h || sx >= det_w;
     float v = 0.f;
     if (!masked) {
@@ -591,22 +604,29 @@ template <typename TI, typename TO> __device__ __forceinline__ TO prepare_pixel(
         if (sizeof(TI) == 4 && v < 0.f) masked = true;
         if (saturation > 0.f && v >= saturation) masked = true;
         if (threshold > 0.f && v < threshold) v = 0.f;
+        v *= scale;                                                    // R24: per-frame normalisation, after the threshold
     }
     if (sizeof(TO) == 2) return (TO)(masked ? 65535.f : fminf(rintf(v), 65534.f));
     return (TO)(masked ? -1.0f : v);
 }
-// V output pixels along kx per thread (V = 8 when n % 8 == 0 and `out` is 16-byte aligned: one or two 16-byte
+// V output pixels along kx per thread (V = 8 when n % 16 == 0, no rotation and `out` is 16-byte aligned: one or two 16-byte
 // stores; the V source pixels are contiguous too, because a group of 8 never straddles kx = n/2), else V = 1.
 template <typename TI, typename TO, int V> __global__ void __launch_bounds__(256) k_prepare_frames(
-    const TI* __restrict__ raw, int det_h, int det_w, int cy, int cx, int n, float threshold, float saturation, TO* __restrict__ out, size_t total) {
+    const TI* __restrict__ raw, int det_h, int det_w, int cy, int cx, int n, float threshold, float saturation, int rot,
+    const float* __restrict__ frame_scale, TO* __restrict__ out, size_t total) {
     for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g * V < total; g += (size_t)gridDim.x * blockDim.x) {
         const size_t i = g * V;
         const int kx = (int)(i % n), ky = (int)((i / n) % n);
         const size_t f = i / ((size_t)n * n);
-        const int sy = cy + (ky < n / 2 ? ky : ky - n), sx = cx + (kx < n / 2 ? kx : kx - n);
+        const int dy = ky < n / 2 ? ky : ky - n, dx = kx < n / 2 ? kx : kx - n;
+        const float sc = frame_scale ? __ldg(frame_scale + f) : 1.0f;
         TO v[V];
 #pragma unroll
-        for (int k = 0; k < V; ++k) v[k] = prepare_pixel<TI, TO>(raw, f, det_h, det_w, sy, sx + k, threshold, saturation);
+        for (int k = 0; k < V; ++k) {
+            int uy, ux;
+            rot_offset(rot, dy, dx + k, uy, ux);
+            v[k] = prepare_pixel<TI, TO>(raw, f, det_h, det_w, cy + uy, cx + ux, threshold, saturation, sc);
+        }
         if (V == 1) out[i] = v[0];
         else {
             const uint4* src = reinterpret_cast<const uint4*>(v);

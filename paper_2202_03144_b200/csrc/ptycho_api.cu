@@ -74,6 +74,15 @@ struct ptycho_ctx {
     std::vector<int> slot_of_h;                // caller frame -> slot
     std::vector<int> mb_offsets;               // batch b = mb_frames[mb_offsets[b] .. mb_offsets[b+1])
     int t = 0;                                 // global iteration counter
+    // streaming ingestion (ptycho_append_frames): frames [0, present) have arrived; the copies run on their own stream
+    bool streaming = false;
+    int present = 0, mb_built_for = -1, stage_frames = 0;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_append = nullptr;
+    void* stage = nullptr;                     // device staging piece of the H2D copies
+    double* scratch_s = nullptr;               // partial sums of the appended chunk's intensities (copy stream)
+    std::vector<int32_t> pos_h;                // positions, caller order (batch rebuilds)
+    std::vector<int> batch_order_h, mb_h;
     long long n_steps = 0;
     bool psi_valid = false;
     long long launches = 0;
@@ -84,7 +93,11 @@ struct ptycho_ctx {
     std::vector<ProfEv> prof_ev;
     double prof_ms[PTYCHO_KCLASS_COUNT] = {};
     long long prof_n[PTYCHO_KCLASS_COUNT] = {};
-    ~ptycho_ctx() { for (auto& e : prof_ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); } }
+    ~ptycho_ctx() {
+        for (auto& e : prof_ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+        if (ev_append) cudaEventDestroy(ev_append);
+        if (copy_stream) cudaStreamDestroy(copy_stream);
+    }
 };
 
 namespace {
@@ -97,6 +110,8 @@ namespace {
             return PTYCHO_ECUDA;                                                                   \
         }                                                                                          \
     } while (0)
+
+std::string g_init_error;   // message of the last failing ptycho_init (no context exists to hold it): ptycho_last_error(NULL)
 
 ptycho_status fail(ptycho_ctx* c, ptycho_status s, const char* msg) {
     if (c) c->err = msg;
@@ -150,6 +165,9 @@ int chunk_frames(int n, int K, int J) {
     return (int)std::max<long long>(1, std::min<long long>(c, J));
 }
 
+// The only environment switches of the library: the queue geometry of the DM megakernel (PTYCHO_MEGA_M / _D / _X / _RING_MB) and
+// the chunk size of the three-pass kernels (PTYCHO_CHUNK_MB).  They change scheduling, never results (tests/test_gpu_parity.py:
+// test_dm_queue_geometry_does_not_change_the_result, test_handoff_stress_deterministic_bitwise).
 int env_int(const char* name, int dflt) {
     const char* e = getenv(name);
     return (e && *e) ? atoi(e) : dflt;
@@ -162,19 +180,22 @@ int ncb_of(int n);
 // D = X = 8 against D = 4, X = 0 is 9.3 ms against 12.4 ms), and M shrinks until the ring fits the L2 share.
 void mega_config(ptycho_ctx* c) {
     c->mega_M = c->mega_D = c->mega_R = 0;
-    if (c->K != 1 || c->par.disable_dm || !env_int("PTYCHO_MEGA", 1)) return;
+    if (c->K != 1 || c->par.disable_dm) return;
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) { int v = 0; if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v; }
     cudaGetLastError();
     const int grid = sms * (c->N >= 512 ? 1 : PTYCHO_MEGA_OCC);
-    const int inflight = (grid + 3 * ncb_of(c->N) - 1) / (3 * ncb_of(c->N));
-    c->mega_D = std::max(2, env_int("PTYCHO_MEGA_D", inflight + 2));
-    const int X = std::max(0, env_int("PTYCHO_MEGA_X", inflight + 2));
-    int M = std::max(1, std::min(env_int("PTYCHO_MEGA_M", 4), c->J));
-    // 48 MB keeps the ring resident in L2 (config 2: 1.26 x algorithmic DRAM traffic; at 64 MB it is 2 % faster but
-    // the ring is written back: 1.73 x); 512^2 frames need 64 MB for two slots per item (config 4: 86.9 -> 74.8 ms)
-    // The split form of the queue (dm_mega.cuh) puts three lags between pass 1 and pass 3 of a frame, so the ring spans 3 D + 1 + X waves.
-    const double ring_mb = env_int("PTYCHO_MEGA_RING_MB", c->N >= 512 ? 96 : 64);
+    // About grid / (4 NCB) queue waves are in flight in the split form (four item kinds per wave), grid / (3 NCB) in the fused one.
+    // Measured on config 2 (B200, round 2): D = 6, X = 5, M = 6 (ring 102 frames, 53 MB) 7.95 / 6.03 ms per early / steady-state
+    // iteration; D = X = 9, M = 3: 8.33 / 6.73; M = 2: 8.9 / 7.4.  More slots per item amortise the item's probe rows, its claim and
+    // its probe-sum flush.
+    const int inflight = (grid + 4 * ncb_of(c->N) - 1) / (4 * ncb_of(c->N));
+    c->mega_D = std::max(2, env_int("PTYCHO_MEGA_D", inflight + 1));
+    const int X = std::max(0, env_int("PTYCHO_MEGA_X", inflight));
+    int M = std::max(1, std::min(env_int("PTYCHO_MEGA_M", 6), c->J));
+    // The split form of the queue (dm_mega.cuh) puts three lags between pass 1 and pass 3 of a frame, so the ring spans 3 D + 1 + X
+    // waves.  The cap keeps it inside the 126 MB L2 next to the streamed exit waves (part of it is still written back: profiles/r02.md).
+    const double ring_mb = env_int("PTYCHO_MEGA_RING_MB", 96);
     while (M > 1 && (double)(3 * c->mega_D + 1 + X) * M * c->N * c->N * 8.0 > ring_mb * 1048576.0) --M;
     c->mega_M = M;
     c->mega_R = (3 * c->mega_D + 1 + X) * M;
@@ -231,7 +252,14 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
         if (c->par.deterministic || c->par.dm_sweeps > 0) c->det_partial = w.take<float4>((size_t)kDetGroups * nn);
         if (c->par.dm_sweeps > 0) c->tile_slots = w.take<int>((size_t)c->J * (c->N / kDetTileW + 1) * (c->N / kDetTileH + 1));
     }
-    if (copy_I) c->I = w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
+    // Intensities passed from host memory are needed on the device only during init (sum, re-tiling): they are staged in the
+    // exit-wave store, which is not written before the first DM iteration; only without that store do they get their own piece.
+    if (c->streaming) {
+        c->stage_frames = std::max(1, std::min(c->J, (int)((64ull << 20) / (nn * (c->itype == PTYCHO_I_U16 ? 2 : 4)))));
+        c->stage = w.take<char>((size_t)c->stage_frames * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
+        c->scratch_s = w.take<double>(kRedBlocks);
+    }
+    if (copy_I && !c->streaming) c->I = !c->par.disable_dm ? reinterpret_cast<const void*>(c->psi) : w.take<char>((size_t)c->J * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
     return (w.off + 255) & ~size_t(255);
 }
 
@@ -327,6 +355,43 @@ void spatial_sort(std::vector<int>& idx, const int32_t* pos, int n) {
     });
 }
 
+// Minibatch composition (R8) over the frames present, [0, np): strided batches, or runs of the caller's permutation restricted to
+// them; every batch spatially sorted.  Rebuilt when more frames have arrived (streaming).
+ptycho_status build_batches(ptycho_ctx* c, int np) {
+    if (c->mb_built_for == np) return PTYCHO_OK;
+    std::vector<int>& mb = c->mb_h;
+    if (np < c->J && c->mb_built_for >= 0) CU(cudaStreamSynchronize(c->stream));   // the previous list may still be in flight
+    mb.clear();
+    c->mb_offsets.assign(1, 0);
+    const int B = c->par.batch_size;
+    const int32_t* pos = c->pos_h.data();
+    if (B <= 0 || B >= np) {
+        for (int f : c->dm_order) if (f < np) mb.push_back(f);
+        c->mb_offsets.push_back(np);
+    } else if (!c->batch_order_h.empty()) {
+        std::vector<int> ord;
+        for (int f : c->batch_order_h) if (f < np) ord.push_back(f);
+        for (int s0 = 0; s0 < np; s0 += B) {
+            std::vector<int> fr(ord.begin() + s0, ord.begin() + std::min(np, s0 + B));
+            spatial_sort(fr, pos, c->N);
+            mb.insert(mb.end(), fr.begin(), fr.end());
+            c->mb_offsets.push_back((int)mb.size());
+        }
+    } else {
+        const int nb = (np + B - 1) / B;
+        for (int b = 0; b < nb; ++b) {
+            std::vector<int> fr;
+            for (int j = b; j < np; j += nb) fr.push_back(j);
+            spatial_sort(fr, pos, c->N);
+            mb.insert(mb.end(), fr.begin(), fr.end());
+            c->mb_offsets.push_back((int)mb.size());
+        }
+    }
+    CU(cudaMemcpyAsync(c->mb_frames, mb.data(), (size_t)np * 4, cudaMemcpyHostToDevice, c->stream));
+    c->mb_built_for = np;
+    return PTYCHO_OK;
+}
+
 ptycho_status dm_iteration(ptycho_ctx* c) {
     const size_t nn = (size_t)c->N * c->N, knn = nn * c->K, HW = (size_t)c->H * c->W;
     const int ncb = ncb_of(c->N);
@@ -338,7 +403,6 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         const dim3 g(c->J, (unsigned)((knn + 255) / 256));   // frame index in grid.x: J may exceed 65535
         LAUNCH(c, PTYCHO_K_OTHER, (k_init_psi<<<g, 256, 0, c->stream>>>(c->psi, c->O, c->W, c->P, c->K, c->N, c->pos, c->dm_frames)));
     }
-    c->psi_valid = true;
     const int upd = c->t >= c->par.probe_start;
     if (c->mega_M > 0) {
         MegaArgs m{};
@@ -358,8 +422,12 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         }
         m.spos = c->spos;
         m.It = c->It;
-        m.flags = env_int("PTYCHO_MEGA_FLAGS", 0);
-        m.pf = m.M;
+#ifdef PTYCHO_DEBUG
+        m.flags = env_int("PTYCHO_MEGA_FLAGS", 0);          // experiment switches of dm_mega.cuh: debug builds only
+#else
+        m.flags = 0;
+#endif
+        m.pf = m.M * std::max(1, env_int("PTYCHO_MEGA_PF", 1));
         m.head = c->mega_ctr; m.cnt1 = c->mega_ctr + 64; m.cnt2 = m.cnt1 + c->J; m.cnt3 = m.cnt2 + c->J; m.cnt2a = m.cnt3 + c->J;
         m.stat = c->dm_stat;
         if (fresh) CU(cudaMemsetAsync(c->dm_stat, 0, 2 * sizeof(int), c->stream));   // first iteration: fused form
@@ -411,9 +479,10 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
                 LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(nn), 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, 1)));
             }
         }
-        return PTYCHO_OK;
-    }
-    LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(nn), 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd)));
+    } else
+        LAUNCH(c, PTYCHO_K_UPDATE, (k_dm_blend<<<ew_blocks(nn), 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd)));
+    CU(cudaGetLastError());
+    c->psi_valid = true;                                    // only once every launch of the iteration has been accepted
     return PTYCHO_OK;
 }
 
@@ -486,7 +555,8 @@ size_t ptycho_workspace_bytes(int obj_h, int obj_w, int n, int n_modes, int n_po
     if (params) tmp.par = *params; else ptycho_default_params(&tmp.par);
     tmp.chunk = chunk_frames(n, n_modes, n_pos);
     mega_config(&tmp);
-    return layout(&tmp, nullptr, intensities_on_host != 0);
+    tmp.streaming = intensities_on_host == 2;
+    return layout(&tmp, nullptr, intensities_on_host == 1);
 }
 
 ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int obj_w, const float* probe,
@@ -496,7 +566,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     ptycho_ctx* c = nullptr;
     if (!out) return PTYCHO_EINVAL;
     *out = nullptr;
-    if (!object || !probe || !pos_yx || !intensities || !workspace) return PTYCHO_EINVAL;
+    if (!object || !probe || !pos_yx || !workspace) return PTYCHO_EINVAL;   // intensities == NULL: streaming context (ptycho_append_frames)
     if (!valid_n(n) || n_modes < 1 || n_pos < 1 || obj_h < n || obj_w < n) return PTYCHO_EINVAL;
     if (itype != PTYCHO_I_F32 && itype != PTYCHO_I_U16) return PTYCHO_EINVAL;
     if (n_modes > PTYCHO_MAX_MODES) return PTYCHO_EUNSUPPORTED;
@@ -505,7 +575,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     if (par.batch_size < 0 || par.pbound < 0 || par.delta_blend <= 0 || par.delta_obj <= 0 || par.delta_probe <= 0)
         return PTYCHO_EINVAL;
     // deterministic mode (dm_det.cuh) is built for the single-mode DM megakernel path only
-    if (par.deterministic && (n_modes != 1 || par.disable_dm || !env_int("PTYCHO_MEGA", 1))) return PTYCHO_EUNSUPPORTED;
+    if (par.deterministic && (n_modes != 1 || par.disable_dm)) return PTYCHO_EUNSUPPORTED;
     if (par.dm_sweeps < 0) return PTYCHO_EINVAL;
     if (par.dm_sweeps > 0 && (n_modes != 1 || par.disable_dm || par.deterministic)) return PTYCHO_EUNSUPPORTED;
     if (cols_smem(n, n_modes) > 227 * 1024) return PTYCHO_EUNSUPPORTED;
@@ -534,16 +604,21 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     c->chunk = chunk_frames(n, n_modes, n_pos);
     mega_config(c);
-    const bool dev_I = is_device_ptr(intensities);
+    c->streaming = intensities == nullptr;
+    const bool dev_I = c->streaming || is_device_ptr(intensities);
     const size_t need = layout(c, nullptr, !dev_I);
     if (workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 255)) { delete c; return PTYCHO_ENOMEM; }
     layout(c, workspace, !dev_I);
     if (dev_I) c->I = intensities;
+    c->present = c->streaming ? 0 : n_pos;
+    if (c->streaming) {
+        if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess || cudaEventCreateWithFlags(&c->ev_append, cudaEventDisableTiming) != cudaSuccess) { delete c; return PTYCHO_ECUDA; }
+    }
 
-#define CUI(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { fprintf(stderr, "ptycho_init: %s: %s\n", #call, cudaGetErrorString(e_)); delete c; return PTYCHO_ECUDA; } } while (0)
+#define CUI(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { g_init_error = std::string(#call) + ": " + cudaGetErrorString(e_); delete c; return PTYCHO_ECUDA; } } while (0)
     ptycho_status st = PTYCHO_OK;
     dispatch_n(n, [&](auto nn) { st = set_attrs<decltype(nn)::value>(c); });
-    if (st != PTYCHO_OK) { fprintf(stderr, "ptycho_init: %s\n", c->err.c_str()); delete c; return st; }
+    if (st != PTYCHO_OK) { g_init_error = c->err; delete c; return st; }
 
     const size_t HW = (size_t)obj_h * obj_w, nn = (size_t)n * n, knn = nn * n_modes;
     cudaStream_t s = c->stream;
@@ -558,6 +633,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     CUI(cudaMemsetAsync(c->sc, 0, sizeof(Scalars), s));
     CUI(cudaMemsetAsync(c->err_hist, 0, sizeof(double) * kErrCap, s));
     CUI(cudaMemsetAsync(c->err_ticket, 0, sizeof(unsigned int), s));
+    CUI(cudaMemsetAsync(c->e_part, 0, sizeof(float) * (size_t)n_pos * ncb_of(n), s));
     CUI(cudaMemsetAsync(c->dm_stat, 0, 2 * sizeof(int), s));
 
     std::vector<float2> tw, twi;
@@ -572,36 +648,13 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     spatial_sort(c->dm_order, pos.data(), n);
     c->slot_of_h.resize(n_pos);
     for (int sidx = 0; sidx < n_pos; ++sidx) c->slot_of_h[c->dm_order[sidx]] = sidx;
-    std::vector<int> mb;
-    mb.reserve(n_pos);
-    c->mb_offsets.assign(1, 0);
-    const int B = par.batch_size;
-    if (B <= 0 || B >= n_pos) {
-        mb = c->dm_order;
-        c->mb_offsets.push_back(n_pos);
-    } else if (par.batch_order) {
-        for (int s0 = 0; s0 < n_pos; s0 += B) {
-            std::vector<int> fr(par.batch_order + s0, par.batch_order + std::min(n_pos, s0 + B));
-            spatial_sort(fr, pos.data(), n);
-            mb.insert(mb.end(), fr.begin(), fr.end());
-            c->mb_offsets.push_back((int)mb.size());
-        }
-    } else {
-        const int nb = (n_pos + B - 1) / B;
-        for (int b = 0; b < nb; ++b) {
-            std::vector<int> fr;
-            for (int j = b; j < n_pos; j += nb) fr.push_back(j);
-            spatial_sort(fr, pos.data(), n);
-            mb.insert(mb.end(), fr.begin(), fr.end());
-            c->mb_offsets.push_back((int)mb.size());
-        }
-    }
+    c->pos_h = pos;
+    if (par.batch_order) c->batch_order_h.assign(par.batch_order, par.batch_order + n_pos);
     c->par.batch_order = nullptr;   // copied; the caller's pointer is not kept
     CUI(cudaMemcpyAsync(c->dm_frames, c->dm_order.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
     std::vector<int32_t> spos(2 * (size_t)n_pos);
     for (int sidx = 0; sidx < n_pos; ++sidx) { spos[2 * sidx] = pos[2 * c->dm_order[sidx]]; spos[2 * sidx + 1] = pos[2 * c->dm_order[sidx] + 1]; }
     CUI(cudaMemcpyAsync(c->spos, spos.data(), spos.size() * 4, cudaMemcpyHostToDevice, s));
-    CUI(cudaMemcpyAsync(c->mb_frames, mb.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
     CUI(cudaMemcpyAsync(c->slot_of, c->slot_of_h.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
 
     if (par.deterministic || c->p2) {                       // frames per object tile, ascending slot (dm_det.cuh)
@@ -643,7 +696,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
         CUI(cudaMemcpyAsync(c->tile_list, list.data(), list.size() * 4, cudaMemcpyHostToDevice, s));
         CUI(cudaStreamSynchronize(s));                      // the host vectors go out of scope
     }
-    {                                                       // intensities in pass-2 tile order (dm_mega.cuh)
+    if (!c->streaming) {                                    // intensities in pass-2 tile order (dm_mega.cuh)
         const dim3 g(n_pos, ncb_of(n));   // frame index in grid.x: J may exceed 65535
 #define TILE_I(NN) do { if (itype == PTYCHO_I_U16) k_tile_intensity<NN, unsigned short><<<g, kThreads, 0, s>>>((unsigned short*)c->It, (const unsigned short*)c->I, c->dm_frames); \
                         else k_tile_intensity<NN, float><<<g, kThreads, 0, s>>>((float*)c->It, (const float*)c->I, c->dm_frames); } while (0)
@@ -656,12 +709,16 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     k_finish_init<<<1, 1, 0, s>>>(c->sc, par.delta_blend, n_pos, 0);
     k_abs2_max<<<ew_blocks(HW), 256, 0, s>>>(c->O, HW, c->sc);
     k_finish_init<<<1, 1, 0, s>>>(c->sc, par.delta_blend, n_pos, 1);
-    k_sum_intensity<<<kRedBlocks, 256, 0, s>>>(c->I, itype, (size_t)n_pos * nn, c->scratch_d);
-    k_finish_sum_I<<<1, 1, 0, s>>>(c->scratch_d, kRedBlocks, c->sc);
-    c->launches += 6;
+    if (!c->streaming) {
+        k_sum_intensity<<<kRedBlocks, 256, 0, s>>>(c->I, itype, (size_t)n_pos * nn, c->scratch_d);
+        k_finish_sum_I<<<1, 32, 0, s>>>(c->scratch_d, kRedBlocks, c->sc, 0);
+        c->launches += 2;
+    }
+    c->launches += 4;
     CUI(cudaStreamSynchronize(s));
     CUI(cudaGetLastError());
 #undef CUI
+    if ((!dev_I && !c->par.disable_dm) || c->streaming) c->I = nullptr;       // the staging copy lived in the exit-wave store: gone after init
     *out = c;
     return PTYCHO_OK;
 }
@@ -671,6 +728,14 @@ ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
     if (alg != PTYCHO_EPIE_MB && alg != PTYCHO_DM && alg != PTYCHO_LSQML) return fail(c, PTYCHO_EINVAL, "unknown algorithm");
     if (alg != PTYCHO_DM && c->par.deterministic) return fail(c, PTYCHO_EUNSUPPORTED, "deterministic mode covers DM only");
     if (alg == PTYCHO_DM && !c->psi) return fail(c, PTYCHO_ESTATE, "DM needs the exit-wave store (disable_dm was set)");
+    if (c->streaming) {
+        if (c->present == 0) return fail(c, PTYCHO_ESTATE, "no frame has been appended yet");
+        if (alg == PTYCHO_DM && c->present < c->J) return fail(c, PTYCHO_ESTATE, "DM needs every frame (PAPER.md:58); append the rest first");
+        CU(cudaStreamWaitEvent(c->stream, c->ev_append, 0));   // the frames appended so far have been copied and re-tiled
+    }
+    if (alg != PTYCHO_DM) { ptycho_status st = build_batches(c, c->present); if (st != PTYCHO_OK) return st; }
+    k_snap_sum_I<<<1, 1, 0, c->stream>>>(c->sc);
+    ++c->launches;
     for (int it = 0; it < n_iters; ++it) {
         ptycho_status st = alg == PTYCHO_DM ? dm_iteration(c) : minibatch_iteration(c, alg);
         if (st != PTYCHO_OK) return st;
@@ -778,6 +843,9 @@ ptycho_status ptycho_revised_waves(ptycho_ctx* c, const int32_t* idx, int count,
 
 ptycho_status ptycho_eval_error(ptycho_ctx* c, double* out) {
     if (!c || !out) return PTYCHO_EINVAL;
+    if (c->present < c->J) return fail(c, PTYCHO_ESTATE, "eval_error needs every frame");
+    if (c->streaming) CU(cudaStreamWaitEvent(c->stream, c->ev_append, 0));
+    k_snap_sum_I<<<1, 1, 0, c->stream>>>(c->sc);
     const int ncb = ncb_of(c->N);
     for (int s0 = 0; s0 < c->J; s0 += c->chunk) {
         const int nf = std::min(c->chunk, c->J - s0);
@@ -791,6 +859,41 @@ ptycho_status ptycho_eval_error(ptycho_ctx* c, double* out) {
     CU(cudaStreamSynchronize(c->stream));
     return PTYCHO_OK;
 }
+
+ptycho_status ptycho_append_frames(ptycho_ctx* c, int first_frame, int count, const void* intensities) {
+    if (!c || !intensities || count < 1) return PTYCHO_EINVAL;
+    if (!c->streaming) return fail(c, PTYCHO_ESTATE, "not a streaming context (ptycho_init was given the intensities)");
+    if (first_frame != c->present || first_frame + count > c->J) return fail(c, PTYCHO_EINVAL, "frames must be appended in order, without gaps");
+    const size_t nn = (size_t)c->N * c->N, bpp = c->itype == PTYCHO_I_U16 ? 2 : 4;
+    const bool dev = is_device_ptr(intensities);
+    cudaStream_t s = c->copy_stream;
+    for (int f0 = 0; f0 < count; f0 += c->stage_frames) {
+        const int nf = std::min(c->stage_frames, count - f0);
+        const char* src = static_cast<const char*>(intensities) + (size_t)f0 * nn * bpp;
+        const void* chunk = src;
+        if (!dev) { CU(cudaMemcpyAsync(c->stage, src, (size_t)nf * nn * bpp, cudaMemcpyHostToDevice, s)); chunk = c->stage; }
+        const dim3 g(nf, ncb_of(c->N));
+        const int first = first_frame + f0;
+        dispatch_n(c->N, [&](auto nn_) {
+            constexpr int NN = decltype(nn_)::value;
+            if (c->itype == PTYCHO_I_U16) k_tile_intensity_chunk<NN, unsigned short><<<g, kThreads, 0, s>>>((unsigned short*)c->It, (const unsigned short*)chunk, c->slot_of, first);
+            else k_tile_intensity_chunk<NN, float><<<g, kThreads, 0, s>>>((float*)c->It, (const float*)chunk, c->slot_of, first);
+        });
+        k_sum_intensity<<<kRedBlocks, 256, 0, s>>>(chunk, c->itype, (size_t)nf * nn, c->scratch_s);
+        k_finish_sum_I<<<1, 32, 0, s>>>(c->scratch_s, kRedBlocks, c->sc, 1);
+        c->launches += 3;
+    }
+    CU(cudaEventRecord(c->ev_append, s));
+    CU(cudaGetLastError());
+    c->present += count;
+    return PTYCHO_OK;
+}
+ptycho_status ptycho_wait_frames(ptycho_ctx* c) {
+    if (!c) return PTYCHO_EINVAL;
+    if (c->copy_stream) CU(cudaStreamSynchronize(c->copy_stream));
+    return PTYCHO_OK;
+}
+int ptycho_frames_present(const ptycho_ctx* c) { return c ? c->present : 0; }
 
 ptycho_status ptycho_profile(ptycho_ctx* c, int enable) {
     if (!c) return PTYCHO_EINVAL;
@@ -827,12 +930,12 @@ int ptycho_debug_phase(unsigned long long* out16) {
 #endif
 
 long long ptycho_launch_count(const ptycho_ctx* c) { return c ? c->launches : 0; }
-const char* ptycho_last_error(const ptycho_ctx* c) { return c ? c->err.c_str() : ""; }
+const char* ptycho_last_error(const ptycho_ctx* c) { return c ? c->err.c_str() : g_init_error.c_str(); }
 void ptycho_destroy(ptycho_ctx* c) { delete c; }
 
 ptycho_status ptycho_prepare_frames(const void* raw, ptycho_itype raw_type, int n_frames, int det_h, int det_w, int center_y,
-                                    int center_x, int n, float threshold, float saturation, void* out, ptycho_itype out_type,
-                                    void* cuda_stream) {
+                                    int center_x, int n, float threshold, float saturation, int rot90, const float* frame_scale,
+                                    void* out, ptycho_itype out_type, void* cuda_stream) {
     ptycho_ctx* c = nullptr;
     if (!raw || !out || n_frames < 1 || det_h < 1 || det_w < 1 || n < 2 || (n & 1)) return PTYCHO_EINVAL;
     if ((raw_type != PTYCHO_I_F32 && raw_type != PTYCHO_I_U16) || (out_type != PTYCHO_I_F32 && out_type != PTYCHO_I_U16)) return PTYCHO_EINVAL;
@@ -841,13 +944,20 @@ ptycho_status ptycho_prepare_frames(const void* raw, ptycho_itype raw_type, int 
     const size_t total = (size_t)n_frames * n * n, out_bytes = total * (out_type == PTYCHO_I_U16 ? 2 : 4);
     const bool dev_in = is_device_ptr(raw), dev_out = is_device_ptr(out);
     void *d_in = const_cast<void*>(raw), *d_out = out;
-    struct Tmp { void* p = nullptr; ~Tmp() { if (p) cudaFree(p); } } t_in, t_out;   // staging: freed on every return path
+    if (rot90 < 0 || rot90 > 3) return PTYCHO_EINVAL;
+    struct Tmp { void* p = nullptr; ~Tmp() { if (p) cudaFree(p); } } t_in, t_out, t_sc;   // staging: freed on every return path
+    const float* d_sc = frame_scale;
+    if (frame_scale && !is_device_ptr(frame_scale)) {
+        CU(cudaMalloc(&t_sc.p, (size_t)n_frames * 4));
+        CU(cudaMemcpyAsync(t_sc.p, frame_scale, (size_t)n_frames * 4, cudaMemcpyHostToDevice, s));
+        d_sc = static_cast<const float*>(t_sc.p);
+    }
     if (!dev_in) { CU(cudaMalloc(&t_in.p, in_bytes)); d_in = t_in.p; CU(cudaMemcpyAsync(d_in, raw, in_bytes, cudaMemcpyHostToDevice, s)); }
     if (!dev_out) { CU(cudaMalloc(&t_out.p, out_bytes)); d_out = t_out.p; }
     const bool vec = (n % 16 == 0) && ((reinterpret_cast<uintptr_t>(d_out) & 15) == 0);   // n/2 a multiple of 8: a group of 8 never straddles kx = n/2
     const int grid = (int)std::min<size_t>((total / (vec ? 8 : 1) + 255) / 256, (size_t)148 * 64);
-#define PREP(TI, TO) do { if (vec) k_prepare_frames<TI, TO, 8><<<grid, 256, 0, s>>>((const TI*)d_in, det_h, det_w, center_y, center_x, n, threshold, saturation, (TO*)d_out, total); \
-                          else k_prepare_frames<TI, TO, 1><<<grid, 256, 0, s>>>((const TI*)d_in, det_h, det_w, center_y, center_x, n, threshold, saturation, (TO*)d_out, total); } while (0)
+#define PREP(TI, TO) do { if (vec) k_prepare_frames<TI, TO, 8><<<grid, 256, 0, s>>>((const TI*)d_in, det_h, det_w, center_y, center_x, n, threshold, saturation, rot90, d_sc, (TO*)d_out, total); \
+                          else k_prepare_frames<TI, TO, 1><<<grid, 256, 0, s>>>((const TI*)d_in, det_h, det_w, center_y, center_x, n, threshold, saturation, rot90, d_sc, (TO*)d_out, total); } while (0)
     if (raw_type == PTYCHO_I_U16 && out_type == PTYCHO_I_U16) PREP(unsigned short, unsigned short);
     else if (raw_type == PTYCHO_I_U16) PREP(unsigned short, float);
     else if (out_type == PTYCHO_I_U16) PREP(float, unsigned short);

@@ -65,8 +65,15 @@ def test_workspace_bytes_argument_checks_and_scaling(lib):
     assert f(4096, 4096, 200, 1, 10000, 1, 0, None) == 0     # n not in {64,128,256,512}
     assert f(100, 4096, 256, 1, 10, 1, 0, None) == 0         # object smaller than a frame
     assert f(4096, 4096, 256, 0, 10, 1, 0, None) == 0
-    host = f(4096, 4096, 256, 1, 10000, 1, 1, None)          # host intensities are copied into the workspace
-    assert host - ok == 10000 * 256 * 256 * 2
+    host = f(4096, 4096, 256, 1, 10000, 1, 1, None)          # host intensities are staged in the exit-wave store during init:
+    assert host == ok                                        # no extra copy
+    from paper_2202_03144_b200 import binding as _b
+    nodm = _b.Params()
+    lib.ptycho_default_params(C.byref(nodm))
+    nodm.disable_dm = 1                                      # without that store they get their own piece
+    assert f(4096, 4096, 256, 1, 10000, 1, 1, C.byref(nodm)) - f(4096, 4096, 256, 1, 10000, 1, 0, C.byref(nodm)) == 10000 * 256 * 256 * 2
+    stream = f(4096, 4096, 256, 1, 10000, 1, 2, None)        # streaming context: a 64 MB staging piece instead
+    assert 0 < stream - ok <= (64 << 20) + (1 << 20)
     from paper_2202_03144_b200 import binding
     p = binding.Params()
     lib.ptycho_default_params(C.byref(p))

@@ -341,6 +341,12 @@ def test_prepare_frames_bit_exact(B, oracle_mod, in_dt, out_dt):
         assert np.array_equal(got_d.cpu().numpy(), ref), (center, n)
     plain = B.prepare_frames(raw, (75, 85), 64, out_dtype=out_dt)        # no threshold, no saturation
     assert np.array_equal(plain, oracle_mod.prepare_frames(raw, (75, 85), 64, out_dtype=out_dt))
+    scale = (0.5 + rng.random(5)).astype(np.float32)                     # R23 rotation, R24 normalisation
+    for rot in range(4):
+        for center, n in (((75, 85), 64), ((3, 160), 32), ((70, 90), 24)):
+            ref = oracle_mod.prepare_frames(raw, center, n, threshold=300.0, saturation=60000.0, out_dtype=out_dt, rot90=rot, frame_scale=scale)
+            got = B.prepare_frames(raw, center, n, threshold=300.0, saturation=60000.0, out_dtype=out_dt, rot90=rot, frame_scale=scale)
+            assert np.array_equal(got, ref), (rot, center, n)
 
 
 # ------------------------------------------------- the steady-state path bench.py times, at full size
@@ -550,3 +556,42 @@ def test_position_sequential_epie(B, oracle_mod):
         g.iterate("EPIE_MB", 1)
         assert rel(g.fetch_object(), o.O) < TOL_ITER * (it + 1) and rel(g.fetch_probe(), o.P) < TOL_ITER * (it + 1), it
     assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+
+
+# ------------------------------------------------------------------ f3: streaming ingestion
+@pytest.mark.parametrize("dtype", [np.uint16, np.float32])
+def test_streaming_ingestion(B, oracle_mod, dtype):
+    """Frames arrive in three pieces while the reconstruction runs: every ptycho_iterate works on the frames
+    present, with the batches of R8 formed over them.  The oracle sees the same thing as a chain of runs on the growing prefix,
+    each continuing from the object and probe of the last."""
+    import torch
+    s = synth.make_custom(64, 220, 6, 24, k=1, peak=2e4, dtype=dtype, jitter=2, seed=51, probe_kind="disk")
+    J = len(s.pos)
+    g = B.Ptycho(s.obj0, s.probe0, s.pos, None, B.default_params(batch_size=5), stream_dtype=dtype)
+    with pytest.raises(B.PtychoError, match="ESTATE"):
+        g.iterate("EPIE_MB", 1)                                  # nothing present yet
+    O, P = s.obj0.astype(complex), s.probe0.astype(complex)
+    errs = []
+    pinned = torch.from_numpy(s.intensities).pin_memory()
+    for lo, hi in ((0, 10), (10, 23), (23, J)):
+        with pytest.raises(B.PtychoError, match="EINVAL"):
+            g.append_frames(lo + 1, s.intensities[lo + 1:hi])    # a gap
+        g.append_frames(lo, pinned[lo:hi] if lo else s.intensities[lo:hi])   # pinned torch slice and plain numpy
+        assert g.frames_present() == hi
+        if hi < J:
+            with pytest.raises(B.PtychoError, match="ESTATE"):
+                g.iterate("DM", 1)                               # DM wants every frame
+        g.iterate("EPIE_MB", 2)
+        o = oracle_mod.Oracle(O, P, s.pos[:hi], s.intensities[:hi], dict(batch_size=5)).iterate("EPIE_MB", 2)
+        O, P = o.O, o.P
+        errs += o.err
+        assert rel(g.fetch_object(), O) < 4 * TOL_ITER and rel(g.fetch_probe(), P) < 4 * TOL_ITER, hi
+    g.wait_frames()
+    assert np.allclose(g.fetch_error(), errs, rtol=2e-3)
+    g.iterate("DM", 2)                                           # complete now
+    o = oracle_mod.Oracle(O, P, s.pos, s.intensities)
+    first = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities)
+    o.eps_O, o.eps_P = first.eps_O, first.eps_P                 # R5: the blend constants were fixed at init, from the initial state
+    o.iterate("DM", 2)
+    assert rel(g.fetch_object(), o.O) < 8 * TOL_ITER
+    assert g.eval_error() == pytest.approx(o.eval_error(), rel=2e-3)

@@ -18,7 +18,7 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-ALG = {"EPIE_MB": 0, "DM": 1, "LSQML": 2}
+ALG = {"EPIE_MB": 0, "DM": 1, "LSQML": 2, "LSQML_PF": 3}
 DEFAULTS = dict(batch_size=0, probe_start=0, delta_blend=1e-2, delta_obj=1.0, delta_probe=1.0,
                 alpha_obj=1.0, alpha_probe=1.0, lsq_lambda=0.1, pbound=0.0, batch_order=None, dm_sweeps=0)
 
@@ -41,7 +41,7 @@ def lib(precision: str = "f64"):
         build()
         l = C.CDLL(os.path.join(_HERE, f"liboracle_{precision}.so"))
         l.orc_modulus_project.restype = C.c_double if precision == "f64" else C.c_float
-        for f in ("orc_sum_intensity", "orc_eval_error_num", "orc_dm_iteration", "orc_minibatch_step"):
+        for f in ("orc_sum_intensity", "orc_eval_error_num", "orc_dm_iteration", "orc_minibatch_step", "orc_minibatch_step_perframe"):
             getattr(l, f).restype = C.c_double
         _libs[precision] = l
     return _libs[precision]
@@ -176,6 +176,13 @@ class Oracle:
                 num = 0.0
                 for fr in batches(self.J, p["batch_size"], p["batch_order"]):
                     fr = np.ascontiguousarray(fr, np.int32)
+                    if alg == "LSQML_PF":                      # per-frame step lengths; steps: one pair per frame
+                        stf = np.zeros((len(fr), 2))
+                        num += self.l.orc_minibatch_step_perframe(
+                            *self._dims(), _p(self.O), _p(self.P), _p(self.pos), _p(self.I), _p(fr), C.c_int(len(fr)), C.c_int(upd),
+                            self.cr(p["delta_obj"]), self.cr(p["delta_probe"]), self.cr(p["lsq_lambda"]), self.cr(p["pbound"]), _p(stf))
+                        self.steps += [tuple(v) for v in stf]
+                        continue
                     st = (C.c_double * 2)()
                     rb = np.empty((len(fr), self.K, self.n, self.n), self.cdt) if rev is not None else None
                     num += self.l.orc_minibatch_step(

@@ -428,3 +428,98 @@ void orc_probe_from_waves(int H, int W, int n, int K, int J, const cplx *O, cplx
             P[k * np + q] = (nP[k * np + q] + eps_P * P[k * np + q]) / (dP[q] + eps_P);
     free(nP); free(dP);
 }
+
+/* ------------------------------------------------------------------------------------------
+ * LSQML-style minibatch with PER-FRAME step lengths (reading R25; ref [18] of the paper
+ * is not available, so this is a definition in the spirit of R9, not a reproduction).  Directions dO, dP_k
+ * as in orc_minibatch_step.  For every frame j of the batch the real pair (a_j, b_j) minimises
+ *     sum_k || chi_jk - a_j P_k dO_j - b_j dP_k O_j ||^2  + lambda (A11_j a_j^2 + A22_j b_j^2)
+ * (2x2 normal equations; frozen probe: a_j = b1_j / (A11_j (1 + lambda)), b_j = 0; determinant <= 0: 0, 0).
+ * Update ("weighted second scatter"): with w_j(r) = sum_k |P_k(r - r_j)|^2 on the frame's window,
+ *     O(r) += dO(r) * sum_j a_j w_j(r) / sum_j w_j(r)     (pixels with sum_j w_j = 0 keep their value)
+ *     P_k  += mean_j(b_j) * dP_k.
+ * steps_out (optional): nb pairs (a_j, b_j), in batch order.  Returns the batch's error term.
+ * ------------------------------------------------------------------------------------------ */
+double orc_minibatch_step_perframe(int H, int W, int n, int K, cplx *O, cplx *P, const int32_t *pos, const real *Inten,
+                                   const int32_t *frames, int nb, int update_probe, real delta_O, real delta_P,
+                                   real lsq_lambda, real pbound, double *steps_out) {
+    const long np = (long)n * n, knp = K * np, HW = (long)H * W;
+    cplx *chi = (cplx *)malloc(sizeof(cplx) * (size_t)(nb * knp));
+    cplx *psi = (cplx *)malloc(sizeof(cplx) * (size_t)knp);
+    cplx *Phi = (cplx *)malloc(sizeof(cplx) * (size_t)knp);
+    cplx *nO = (cplx *)calloc((size_t)HW, sizeof(cplx));
+    real *dO = (real *)calloc((size_t)HW, sizeof(real));
+    cplx *nP = (cplx *)calloc((size_t)knp, sizeof(cplx));
+    real *dP = (real *)calloc((size_t)np, sizeof(real));
+    double tot = 0;
+    for (int i = 0; i < nb; ++i) {                                      /* chi_j = F^-1[Pi_M F[P O_j]] - P O_j */
+        int j = frames[i];
+        exit_wave(W, n, K, O, P, pos + 2 * j, psi);
+        memcpy(Phi, psi, sizeof(cplx) * (size_t)knp);
+        for (int k = 0; k < K; ++k) orc_fft2(n, Phi + k * np, 0);
+        cplx *c = chi + i * knp;
+        tot += orc_modulus_project(n, K, Phi, Inten + j * np, pbound, c);
+        for (int k = 0; k < K; ++k) orc_fft2(n, c + k * np, 1);
+        for (long q = 0; q < knp; ++q) c[q] -= psi[q];
+    }
+    for (int i = 0; i < nb; ++i) {                                      /* batch sums (as in orc_minibatch_step) */
+        const int32_t *r = pos + 2 * frames[i];
+        for (int y = 0; y < n; ++y)
+            for (int x = 0; x < n; ++x) {
+                long o = (long)(r[0] + y) * W + r[1] + x, q = y * n + x;
+                cplx Oj = O[o];
+                for (int k = 0; k < K; ++k) {
+                    cplx Pk = P[k * np + q], c = chi[i * knp + k * np + q];
+                    nO[o] += conj(Pk) * c; dO[o] += CABS2(Pk); nP[k * np + q] += conj(Oj) * c;
+                }
+                dP[q] += CABS2(Oj);
+            }
+    }
+    real maxP = 0, maxdP = 0;
+    for (long q = 0; q < np; ++q) {
+        real s = 0;
+        for (int k = 0; k < K; ++k) s += CABS2(P[k * np + q]);
+        if (s > maxP) maxP = s;
+        if (dP[q] > maxdP) maxdP = dP[q];
+    }
+    for (long o = 0; o < HW; ++o) nO[o] = nO[o] / (dO[o] + delta_O * maxP);            /* dO direction */
+    for (int k = 0; k < K; ++k)
+        for (long q = 0; q < np; ++q) nP[k * np + q] = nP[k * np + q] / (dP[q] + delta_P * maxdP);
+
+    double *aw = (double *)calloc((size_t)HW, sizeof(double)), *ww = (double *)calloc((size_t)HW, sizeof(double));
+    double bsum = 0;
+    const double l = 1.0 + (double)lsq_lambda;
+    for (int i = 0; i < nb; ++i) {                                      /* per-frame 2x2 solves */
+        const int32_t *r = pos + 2 * frames[i];
+        double A11 = 0, A22 = 0, A12 = 0, b1 = 0, b2 = 0;
+        for (int k = 0; k < K; ++k)
+            for (int y = 0; y < n; ++y)
+                for (int x = 0; x < n; ++x) {
+                    long o = (long)(r[0] + y) * W + r[1] + x, q = k * np + y * n + x;
+                    double complex u = (double complex)(P[q] * nO[o]), v = (double complex)(nP[q] * O[o]);
+                    double complex c = (double complex)chi[i * knp + q];
+                    A11 += creal(conj(u) * u); A22 += creal(conj(v) * v); A12 += creal(conj(u) * v);
+                    b1 += creal(conj(u) * c); b2 += creal(conj(v) * c);
+                }
+        double a, b;
+        if (!update_probe) { a = (A11 > 0) ? b1 / (A11 * l) : 0; b = 0; }
+        else {
+            double det = A11 * l * A22 * l - A12 * A12;
+            if (!(det > 0) || !isfinite(det)) { a = 0; b = 0; }
+            else { a = (b1 * A22 * l - A12 * b2) / det; b = (A11 * l * b2 - A12 * b1) / det; }
+        }
+        if (steps_out) { steps_out[2 * i] = a; steps_out[2 * i + 1] = b; }
+        bsum += b;
+        for (int y = 0; y < n; ++y)                                      /* weighted second scatter */
+            for (int x = 0; x < n; ++x) {
+                long o = (long)(r[0] + y) * W + r[1] + x;
+                double w = 0;
+                for (int k = 0; k < K; ++k) w += (double)CABS2(P[k * np + y * n + x]);
+                aw[o] += a * w; ww[o] += w;
+            }
+    }
+    for (long o = 0; o < HW; ++o) if (ww[o] > 0) O[o] += (real)(aw[o] / ww[o]) * nO[o];
+    if (update_probe) { real bm = (real)(bsum / nb); for (long q = 0; q < knp; ++q) P[q] += bm * nP[q]; }
+    free(chi); free(psi); free(Phi); free(nO); free(dO); free(nP); free(dP); free(aw); free(ww);
+    return tot;
+}

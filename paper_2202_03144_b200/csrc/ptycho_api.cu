@@ -427,7 +427,7 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
 #else
         m.flags = 0;
 #endif
-        m.pf = m.M * std::max(1, env_int("PTYCHO_MEGA_PF", 1));
+        m.pf = m.M;
         m.head = c->mega_ctr; m.cnt1 = c->mega_ctr + 64; m.cnt2 = m.cnt1 + c->J; m.cnt3 = m.cnt2 + c->J; m.cnt2a = m.cnt3 + c->J;
         m.stat = c->dm_stat;
         if (fresh) CU(cudaMemsetAsync(c->dm_stat, 0, 2 * sizeof(int), c->stream));   // first iteration: fused form

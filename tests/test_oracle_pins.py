@@ -504,3 +504,48 @@ def test_prepare_frames_rotation_and_normalisation_by_hand(oracle_mod):
     assert sc[1, 0, 0] == 0 and sc[0, 0, 0] == 0                                                    # 124 < threshold -> 0 in both
     f32 = oracle_mod.prepare_frames(two.astype(np.float32), c, 4, frame_scale=np.array([2.0, 0.25], np.float32), out_dtype=np.float32)
     assert f32[0, 0, 0] == 248.0 and f32[1, 0, 0] == 31.0
+
+
+def test_lsqml_per_frame_steps_against_per_frame_lstsq(oracle_mod):
+    """LSQML_PF (R25): (a_j, b_j) of every frame against numpy.linalg.lstsq of that frame's own stacked system; the object update
+    against the weighted-scatter formula typed with numpy slices; the probe moves by the mean b_j.  J = 4, N = 8, K = 2."""
+    s, lam = f64_scan(n=8, h=20, side=2, step=4, k=2)
+    cnt = RNG.poisson(lam * 30).astype(np.float64)
+    p0 = s.probe_true * np.sqrt(30)
+    obj0 = 1 + 0.1 * crandn(*s.obj_true.shape)
+    lam_t, n = 0.1, s.n
+    ep = oracle_mod.Oracle(obj0, p0, s.pos, cnt, keep_revised=True).iterate("EPIE_MB", 1)   # directions (alpha = 1) and revised waves
+    pf = oracle_mod.Oracle(obj0, p0, s.pos, cnt, dict(lsq_lambda=lam_t)).iterate("LSQML_PF", 1)
+    d_o, d_p = ep.O - obj0, ep.P - p0
+    ri = lambda z: np.concatenate([z.real.ravel(), z.imag.ravel()])
+    aw, ww, bs = np.zeros(obj0.shape), np.zeros(obj0.shape), []
+    for j, (y, x) in enumerate(s.pos):
+        oj, doj = obj0[y:y + n, x:x + n], d_o[y:y + n, x:x + n]
+        u, v, c = p0 * doj[None], d_p * oj[None], ep.revised[j] - p0 * oj[None]
+        a11, a22 = np.vdot(u, u).real, np.vdot(v, v).real
+        m = np.stack([np.concatenate([ri(u), [np.sqrt(lam_t * a11), 0]]), np.concatenate([ri(v), [0, np.sqrt(lam_t * a22)]])], 1)
+        sol = np.linalg.lstsq(m, np.concatenate([ri(c), [0, 0]]), rcond=None)[0]
+        assert pf.steps[j][0] == pytest.approx(sol[0], rel=1e-9) and pf.steps[j][1] == pytest.approx(sol[1], rel=1e-9), j
+        w = np.sum(np.abs(p0) ** 2, 0)
+        aw[y:y + n, x:x + n] += sol[0] * w
+        ww[y:y + n, x:x + n] += w
+        bs.append(sol[1])
+    want_o = obj0 + np.where(ww > 0, aw / np.where(ww > 0, ww, 1), 0) * d_o
+    assert rel(pf.O, want_o) < 1e-12 and rel(pf.P, p0 + np.mean(bs) * d_p) < 1e-12
+    assert pf.err[0] == pytest.approx(ep.err[0], rel=1e-12)
+
+
+def test_lsqml_per_frame_reduces_to_joint_step_for_one_frame(oracle_mod):
+    """J = 1: the per-frame step IS the joint step of R9 (two code paths, one answer); ground truth stays a fixed point."""
+    s, lam = f64_scan(n=8, h=14, side=1, step=4, k=2)
+    cnt = RNG.poisson(lam * 30).astype(np.float64)
+    p0, obj0 = s.probe_true * np.sqrt(30), 1 + 0.1 * crandn(*s.obj_true.shape)
+    a = oracle_mod.Oracle(obj0, p0, s.pos, cnt).iterate("LSQML", 1)
+    b = oracle_mod.Oracle(obj0, p0, s.pos, cnt).iterate("LSQML_PF", 1)
+    assert rel(b.O, a.O) < 1e-12 and rel(b.P, a.P) < 1e-12 and b.steps[0] == pytest.approx(a.steps[0], rel=1e-10)
+    s4, lam4 = f64_scan(k=3)
+    t = oracle_mod.Oracle(s4.obj_true, s4.probe_true, s4.pos, lam4, dict(batch_size=5)).iterate("LSQML_PF", 2)
+    assert max(t.err) < 1e-25 and rel(t.O, s4.obj_true) < 1e-13 and rel(t.P, s4.probe_true) < 1e-13
+    c = synth.make_config(0)
+    e = np.array(oracle_mod.Oracle(c.obj0, c.probe0, c.pos, c.intensities, dict(batch_size=16)).iterate("LSQML_PF", 30).err)
+    assert np.all(np.diff(e) < 0) and e[-1] < 1e-2 * e[0], e                    # R22: monotone on noiseless data

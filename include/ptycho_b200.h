@@ -47,7 +47,12 @@ typedef enum {
 typedef enum {
     PTYCHO_EPIE_MB = 0, /* ePIE, minibatch form (reading R8)                             */
     PTYCHO_DM = 1,      /* difference map, all positions at once (reading R4) */
-    PTYCHO_LSQML = 2    /* LSQML-style minibatch with one joint step per batch (R9)       */
+    PTYCHO_LSQML = 2,   /* LSQML-style minibatch with one joint step per batch (R9)       */
+    PTYCHO_LSQML_PF = 3 /* the same directions, but one step pair (a_j, b_j) per FRAME and the weighted second scatter
+                           O += dO sum_j a_j w_j / sum_j w_j, w_j = sum_k |P_k|^2 on the frame's window; P_k += mean_j(b_j) dP_k
+                           (reading R25).  Costs a second transform cycle per batch (chi is recomputed,
+                           not kept).  ptycho_fetch_steps then returns one pair per frame, batch after batch; inside a batch
+                           in the library's own (spatially sorted) frame order                                       */
 } ptycho_alg;
 
 typedef enum {

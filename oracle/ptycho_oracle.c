@@ -20,8 +20,11 @@
  * and plane-wave closed forms; projection: |Phi'|^2 = I, phase kept, idempotent, relaxed closed
  * form; zero error and fixed point at ground truth; closed-form overlap update; ePIE<->DM
  * cross-check; LSQML K=1 / forced steps <-> ePIE; step solve vs numpy.linalg.lstsq of the explicit
- * system; symmetries.  PARITY UNPINNED: fidelity of "LSQML-style" to the LSQML of the paper's
- * ref [18] (that text is not available; reading R9 is a definition, not a reproduction).
+ * system; symmetries; eval_error off zero against numpy's FFT; the probe direction n_P/(d_P + delta max d_P) from numpy
+ * slices; masked pixels excluded from sum I; the sequential overlap projection against the overlap closed forms; B = 1
+ * against single-frame steps in sequence; the per-frame steps against per-frame numpy.linalg.lstsq and the weighted-scatter
+ * formula.  PARITY UNPINNED: fidelity of "LSQML-style" (R9) and of its per-frame variant (R25) to the LSQML of the paper's
+ * ref [18] (that text is not available; both readings are definitions, not reproductions).
  *
  * Parallelism: OpenMP over frames for the per-frame transforms only; every cross-frame sum is
  * accumulated serially in frame order, so results do not depend on the thread count.

@@ -20,7 +20,7 @@ _CSRC = os.path.join(_HERE, "csrc")
 # the product library always holds all four sizes.
 _ONLY_N = os.environ.get("PTYCHO_BUILD_ONLY_N")
 LIB_PATH = os.environ.get("PTYCHO_B200_LIB") or os.path.join(_CSRC, f"libptycho_dev{_ONLY_N}.so" if _ONLY_N else "libptycho_b200.so")
-ALG = {"EPIE_MB": 0, "DM": 1, "LSQML": 2}
+ALG = {"EPIE_MB": 0, "DM": 1, "LSQML": 2, "LSQML_PF": 3}
 KCLASS = ["rows_fwd", "cols", "rows_inv", "update", "other", "mega"]   # ptycho_kclass
 STATUS = ["OK", "EINVAL", "EBOUNDS", "EUNSUPPORTED", "ENOMEM", "ECUDA", "ESTATE"]
 NVCC_FLAGS = ["--threads", "0", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -19,7 +19,7 @@ struct YX { int y, x; };
 
 enum RowFwdMode { RF_EXIT = 0, RF_DM = 1, RF_PLAIN = 2 };
 enum ColMode { CM_FULL = 0, CM_ERRONLY = 1, CM_PLAIN_FWD = 2, CM_PLAIN_INV = 3 };
-enum RowInvMode { RI_MINIBATCH = 0, RI_DM = 1, RI_REVISED = 2, RI_PLAIN = 3 };
+enum RowInvMode { RI_MINIBATCH = 0, RI_DM = 1, RI_REVISED = 2, RI_PLAIN = 3, RI_LSQ_PF = 4 };
 
 #ifndef PTYCHO_THREADS
 #define PTYCHO_THREADS 256
@@ -44,6 +44,7 @@ struct FrameArgs {
     float2* nP; float* dP;          // probe canvases K x N x N, N x N
     float pbound;
     float2* out;                    // RI_REVISED: nframes x K x N x N
+    double* pf_part;                // RI_LSQ_PF: per slot of this launch, NCB x 5 partial sums (A11, A22, A12, b1, b2)
     const float2* __restrict__ tw;  // twiddles [ka*T + b]
     const float2* __restrict__ twi; // twiddles [b*E + ka]
 };
@@ -301,6 +302,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_in
     for (int r = 0; r < E; ++r) o[r] = __ldg(a.O + obase + pos_a_inv<N>(t, r));
     float2 accO[E];
     float accD[E];
+    float pfs[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
     for (int r = 0; r < E; ++r) { accO[r] = make_float2(0.f, 0.f); accD[r] = 0.f; }
 
@@ -328,6 +330,15 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_in
                 const float2 pf = make_float2(fmaf(rb, po.x - v[r].x, v[r].x), fmaf(rb, po.y - v[r].y, v[r].y));
                 if (MODE == RI_REVISED) { a.out[fr + off + x] = pf; continue; }
                 w = make_float2(pf.x - po.x, pf.y - po.y);                 // chi
+                if (MODE == RI_LSQ_PF) {                                   // R25: this frame's five sums; nO / nP hold the directions dO / dP_k
+                    const float2 u = cmul(p, a.nO[obase + x]), vv = cmul(a.nP[off + x], o[r]);
+                    pfs[0] = fmaf(u.x, u.x, fmaf(u.y, u.y, pfs[0]));
+                    pfs[1] = fmaf(vv.x, vv.x, fmaf(vv.y, vv.y, pfs[1]));
+                    pfs[2] = fmaf(u.x, vv.x, fmaf(u.y, vv.y, pfs[2]));
+                    pfs[3] = fmaf(u.x, w.x, fmaf(u.y, w.y, pfs[3]));
+                    pfs[4] = fmaf(vv.x, w.x, fmaf(vv.y, w.y, pfs[4]));
+                    continue;
+                }
                 red_add(a.nP + off + x, cmulc(w, o[r]));                   // a9 conj(O_j) chi
             }
             accO[r] = cadd(accO[r], cmulc(w, p));                          // a8 conj(P_k) w
@@ -336,6 +347,22 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_in
         __syncwarp();
     }
     if (MODE == RI_REVISED) return;
+    if (MODE == RI_LSQ_PF) {                                               // block reduction in a fixed order, in double
+        __shared__ double s_pf[kThreads / 32][5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+            double d = (double)pfs[q];
+            for (int sft = 16; sft > 0; sft >>= 1) d += __shfl_xor_sync(0xffffffffu, d, sft);
+            if ((threadIdx.x & 31) == 0) s_pf[threadIdx.x >> 5][q] = d;
+        }
+        __syncthreads();
+        if (threadIdx.x < 5) {
+            double d = 0.0;
+            for (int wv = 0; wv < kThreads / 32; ++wv) d += s_pf[wv][threadIdx.x];
+            a.pf_part[((size_t)slot * G::NCB + blockIdx.x) * 5 + threadIdx.x] = d;
+        }
+        return;
+    }
 #pragma unroll
     for (int r = 0; r < E; ++r) {
         const int x = pos_a_inv<N>(t, r);
@@ -508,6 +535,54 @@ __global__ void k_lsq_solve(const double* partO, int nO, const double* partP, in
     }
     sc->step_a = (float)a; sc->step_b = (float)b;
     steps_out[0] = a; steps_out[1] = b;
+}
+// R25: per-frame 2x2 solves from the partial sums of RI_LSQ_PF (NCB x 5 per frame, added in block order), one CTA; the probe
+// step is the mean b_j (fixed-order tree).  ab: nb x (a_j, b_j) floats for the scatter; steps_out (optional): the same pairs, double.
+__global__ void __launch_bounds__(1024) k_lsq_pf_solve(const double* __restrict__ part, int nb, int ncb, float lambda, int update_probe, float2* ab,
+                                                       Scalars* sc, double* steps_out, int steps_cap) {
+    __shared__ double sb[1024];
+    const double l = 1.0 + (double)lambda;
+    double bsum = 0.0;
+    for (int j = threadIdx.x; j < nb; j += 1024) {
+        double v[5] = {0, 0, 0, 0, 0};
+        for (int b = 0; b < ncb; ++b)
+            for (int q = 0; q < 5; ++q) v[q] += part[((size_t)j * ncb + b) * 5 + q];
+        const double A11 = v[0], A22 = v[1], A12 = v[2], b1 = v[3], b2 = v[4];
+        double a, b;
+        if (!update_probe) { a = (A11 > 0) ? b1 / (A11 * l) : 0.0; b = 0.0; }
+        else {
+            const double det = A11 * l * A22 * l - A12 * A12;
+            if (!(det > 0) || !isfinite(det)) { a = 0; b = 0; }
+            else { a = (b1 * A22 * l - A12 * b2) / det; b = (A11 * l * b2 - A12 * b1) / det; }
+        }
+        ab[j] = make_float2((float)a, (float)b);
+        if (steps_out && j < steps_cap) { steps_out[2 * j] = a; steps_out[2 * j + 1] = b; }
+        bsum += b;
+    }
+    sb[threadIdx.x] = bsum;
+    __syncthreads();
+    for (int w = 512; w > 0; w >>= 1) { if ((int)threadIdx.x < w) sb[threadIdx.x] += sb[threadIdx.x + w]; __syncthreads(); }
+    if (threadIdx.x == 0) { sc->step_a = 1.f; sc->step_b = (float)(sb[0] / nb); }
+}
+// R25 weighted second scatter: aw += a_j w_j, ww += w_j, w_j = sum_k |P_k|^2 on the frame's window.  grid (nframes, n*n/256)
+__global__ void k_lsq_pf_scatter(float* aw, float* ww, int W, const float2* __restrict__ P, int K, int n, const YX* __restrict__ pos,
+                                 const int* __restrict__ frames, const float2* __restrict__ ab) {
+    const int q = blockIdx.y * blockDim.x + threadIdx.x, nn = n * n;
+    if (q >= nn) return;
+    const YX p0 = pos[frames[blockIdx.x]];
+    float w = 0.f;
+    for (int k = 0; k < K; ++k) { const float2 p = P[(size_t)k * nn + q]; w = fmaf(p.x, p.x, fmaf(p.y, p.y, w)); }
+    const size_t o = (size_t)(p0.y + q / n) * W + p0.x + q % n;
+    atomicAdd(aw + o, ab[blockIdx.x].x * w);
+    atomicAdd(ww + o, w);
+}
+// O += dO * aw / ww where ww > 0; zero dO (dir), aw, ww.
+__global__ void k_lsq_pf_apply(float2* x, float2* dir, float* aw, float* ww, size_t plane) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < plane; i += (size_t)gridDim.x * blockDim.x) {
+        const float wv = ww[i];
+        if (wv > 0.f) { const float st = aw[i] / wv; const float2 d = dir[i]; float2 xv = x[i]; xv.x = fmaf(st, d.x, xv.x); xv.y = fmaf(st, d.y, xv.y); x[i] = xv; }
+        dir[i] = make_float2(0.f, 0.f); aw[i] = 0.f; ww[i] = 0.f;
+    }
 }
 __global__ void k_set_steps(Scalars* sc, float a, float b, double* steps_out) {
     sc->step_a = a; sc->step_b = b;

@@ -67,6 +67,8 @@ struct ptycho_ctx {
     int mega_M = 0, mega_D = 0, mega_R = 0, mega_grid = 0;
     int* mega_ctr = nullptr;                   // device: [head | pad to 64 ints | cnt1[J] | cnt2[J] | cnt3[J]]
     float* p2 = nullptr;                       // |P|^2 of the current probe (d_O gather, dm_det.cuh)
+    float* wO = nullptr;                       // LSQML_PF: sum_j w_j canvas (the a_j w_j canvas reuses dO)
+    double* pf_part = nullptr; float2* pf_ab = nullptr;   // LSQML_PF: per-frame partial sums (J x NCB x 5) and steps (J)
     double* err_part = nullptr; unsigned int* err_ticket = nullptr;   // k_sum_error: per-CTA pieces and the finishing ticket
     int* dm_stat = nullptr;                    // [0] frames inside the power bound in the previous DM iteration, [1] running count
     int sms = 148;
@@ -221,6 +223,9 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
     c->dO = w.take<float>(HW);
     c->nP = w.take<float2>(knn);
     c->dP = w.take<float>(nn);
+    c->wO = w.take<float>(HW);
+    c->pf_part = w.take<double>((size_t)c->J * ncb_of(c->N) * 5);
+    c->pf_ab = w.take<float2>(c->J);
     c->S = w.take<float2>((size_t)std::max(c->chunk, c->mega_R) * knn);
     c->mega_ctr = w.take<int>(64 + 4 * (size_t)c->J);
     c->e_part = w.take<float>((size_t)c->J * ncb_of(c->N));
@@ -279,6 +284,7 @@ template <int N> ptycho_status set_attrs(ptycho_ctx* c) {
     CU(cudaFuncSetAttribute(k_rows_inv<N, RI_DM>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_inv<N, RI_REVISED>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_inv<N, RI_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_rows_inv<N, RI_LSQ_PF>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_cols<N, CM_FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
     CU(cudaFuncSetAttribute(k_cols<N, CM_ERRONLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
     CU(cudaFuncSetAttribute(k_cols<N, CM_PLAIN_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, cols));
@@ -334,6 +340,7 @@ template <int N> void launch_passes(ptycho_ctx* c, const FrameArgs& a, int nfram
         if (inv == RI_MINIBATCH) k_rows_inv<N, RI_MINIBATCH><<<grid, blk, sr, s>>>(a);
         else if (inv == RI_DM) k_rows_inv<N, RI_DM><<<grid, blk, sr, s>>>(a);
         else if (inv == RI_REVISED) k_rows_inv<N, RI_REVISED><<<grid, blk, sr, s>>>(a);
+        else if (inv == RI_LSQ_PF) k_rows_inv<N, RI_LSQ_PF><<<grid, blk, sr, s>>>(a);
         else k_rows_inv<N, RI_PLAIN><<<grid, blk, sr, s>>>(a);
     });
 }
@@ -502,7 +509,7 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
             a.e_part = c->e_part + (size_t)s0 * ncb;
             passes(c, a, nf, RF_EXIT, CM_FULL, RI_MINIBATCH);
         }
-        const bool lsq = alg == PTYCHO_LSQML;
+        const bool lsq = alg == PTYCHO_LSQML, pfm = alg == PTYCHO_LSQML_PF;
         const int gO = ew_blocks(HW), gP = ew_blocks(nn);
         LAUNCH(c, PTYCHO_K_UPDATE, (k_direction<<<gO, 256, 0, c->stream>>>(c->nO, c->dO, HW, 1, c->par.delta_obj, c->sc, 0, lsq ? c->partO : nullptr)));
         if (upd) {
@@ -511,6 +518,28 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
             LAUNCH(c, PTYCHO_K_UPDATE, (k_direction<<<gP, 256, 0, c->stream>>>(c->nP, c->dP, nn, c->K, c->par.delta_probe, c->sc, 1, lsq ? c->partP : nullptr)));
         }
         double* step_slot = c->n_steps < kStepCap ? c->steps + 2 * c->n_steps : nullptr;
+        if (pfm) {
+            // R25: a second transform cycle over the batch recomputes chi_j and leaves every frame's five sums; then the per-frame
+            // solves, the weighted second scatter (a_j w_j into dO, which the directions no longer need; w_j into wO) and the updates.
+            for (int s0 = b0; s0 < b1; s0 += c->chunk) {
+                const int nf = std::min(c->chunk, b1 - s0);
+                FrameArgs a = base_args(c);
+                a.frames = c->mb_frames + s0;
+                a.e_part = c->e_part + (size_t)s0 * ncb;
+                a.pf_part = c->pf_part + (size_t)(s0 - b0) * ncb * 5;
+                passes(c, a, nf, RF_EXIT, CM_FULL, RI_LSQ_PF);
+            }
+            const int cap = (int)std::max<long long>(0, std::min<long long>(b1 - b0, kStepCap - c->n_steps));
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_pf_solve<<<1, 1024, 0, c->stream>>>(c->pf_part, b1 - b0, ncb, c->par.lsq_lambda, upd, c->pf_ab, c->sc,
+                                                                               cap > 0 ? c->steps + 2 * c->n_steps : nullptr, cap)));
+            CU(cudaMemsetAsync(c->dO, 0, HW * 4, c->stream));
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_pf_scatter<<<dim3(b1 - b0, (unsigned)((nn + 255) / 256)), 256, 0, c->stream>>>(
+                                            c->dO, c->wO, c->W, c->P, c->K, c->N, c->pos, c->mb_frames + b0, c->pf_ab)));
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_pf_apply<<<gO, 256, 0, c->stream>>>(c->O, c->nO, c->dO, c->wO, HW)));
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_apply<<<gP, 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->sc, 1, upd)));
+            c->n_steps += b1 - b0;
+            continue;
+        }
         if (lsq) {
             if (upd) {
                 LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_cross<<<dim3(b1 - b0, kCrossParts), 256, 0, c->stream>>>(c->O, c->nO, c->W, c->P, c->nP, c->K, c->N, c->pos,
@@ -630,6 +659,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     CUI(cudaMemsetAsync(c->dO, 0, HW * 4, s));
     CUI(cudaMemsetAsync(c->nP, 0, knn * 8, s));
     CUI(cudaMemsetAsync(c->dP, 0, nn * 4, s));
+    CUI(cudaMemsetAsync(c->wO, 0, HW * 4, s));
     CUI(cudaMemsetAsync(c->sc, 0, sizeof(Scalars), s));
     CUI(cudaMemsetAsync(c->err_hist, 0, sizeof(double) * kErrCap, s));
     CUI(cudaMemsetAsync(c->err_ticket, 0, sizeof(unsigned int), s));
@@ -725,7 +755,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
 
 ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
     if (!c || n_iters < 0) return PTYCHO_EINVAL;
-    if (alg != PTYCHO_EPIE_MB && alg != PTYCHO_DM && alg != PTYCHO_LSQML) return fail(c, PTYCHO_EINVAL, "unknown algorithm");
+    if (alg != PTYCHO_EPIE_MB && alg != PTYCHO_DM && alg != PTYCHO_LSQML && alg != PTYCHO_LSQML_PF) return fail(c, PTYCHO_EINVAL, "unknown algorithm");
     if (alg != PTYCHO_DM && c->par.deterministic) return fail(c, PTYCHO_EUNSUPPORTED, "deterministic mode covers DM only");
     if (alg == PTYCHO_DM && !c->psi) return fail(c, PTYCHO_ESTATE, "DM needs the exit-wave store (disable_dm was set)");
     if (c->streaming) {

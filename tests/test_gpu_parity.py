@@ -595,3 +595,27 @@ def test_streaming_ingestion(B, oracle_mod, dtype):
     o.iterate("DM", 2)
     assert rel(g.fetch_object(), o.O) < 8 * TOL_ITER
     assert g.eval_error() == pytest.approx(o.eval_error(), rel=2e-3)
+
+
+@pytest.mark.parametrize("n,h,side,step,k,batch", [(64, 200, 5, 24, 1, 7), (128, 300, 5, 31, 3, 0), (256, 520, 4, 61, 2, 6)])
+def test_lsqml_per_frame_steps(B, oracle_mod, n, h, side, step, k, batch):
+    """LSQML_PF (R25): one (a_j, b_j) per frame, weighted second scatter, mean probe step -- against the oracle, free-running."""
+    s = synth.make_custom(n, h, side, step, k=k, peak=2e4, dtype=np.uint16, jitter=3, seed=n + 3 * k, probe_kind="disk")
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(batch_size=batch))
+    g = make(B, s, batch_size=batch)
+    lit = well_lit(s)
+    for it in range(4):
+        o.iterate("LSQML_PF", 1)
+        g.iterate("LSQML_PF", 1)
+        Og = g.fetch_object()
+        assert rel(Og, o.O) < TOL_ITER * (it + 1) and rel(Og[lit], o.O[lit]) < TOL_ITER * (it + 1), it
+        assert rel(g.fetch_probe(), o.P) < TOL_ITER * (it + 1), it
+    gs, os_ = g.fetch_steps(), np.array(o.steps)               # one pair per frame; inside a batch the library visits frames in its
+    assert gs.shape == os_.shape                               # own (spatial) order, so batches are compared as sets
+    sizes = [len(b) for b in oracle_mod.batches(len(s.pos), batch)] * 4
+    i0 = 0
+    for sz in sizes:
+        a, b = gs[i0:i0 + sz], os_[i0:i0 + sz]
+        assert np.allclose(a[np.lexsort(a.T)], b[np.lexsort(b.T)], rtol=2e-3, atol=1e-5), i0
+        i0 += sz
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)

@@ -188,7 +188,7 @@ void mega_config(ptycho_ctx* c) {
     cudaGetLastError();
     const int grid = sms * (c->N >= 512 ? 1 : PTYCHO_MEGA_OCC);
     // About grid / (4 NCB) queue waves are in flight in the split form (four item kinds per wave), grid / (3 NCB) in the fused one.
-    // Measured on config 2 (B200, round 2): D = 6, X = 5, M = 6 (ring 102 frames, 53 MB) 7.95 / 6.03 ms per early / steady-state
+    // Measured on config 2 (B200, round 2): D = 6, X = 5, M = 6 (ring 144 frames, 75 MB) 7.95 / 6.03 ms per early / steady-state
     // iteration; D = X = 9, M = 3: 8.33 / 6.73; M = 2: 8.9 / 7.4.  More slots per item amortise the item's probe rows, its claim and
     // its probe-sum flush.
     const int inflight = (grid + 4 * ncb_of(c->N) - 1) / (4 * ncb_of(c->N));
@@ -196,7 +196,8 @@ void mega_config(ptycho_ctx* c) {
     const int X = std::max(0, env_int("PTYCHO_MEGA_X", inflight));
     int M = std::max(1, std::min(env_int("PTYCHO_MEGA_M", 6), c->J));
     // The split form of the queue (dm_mega.cuh) puts three lags between pass 1 and pass 3 of a frame, so the ring spans 3 D + 1 + X
-    // waves.  The cap keeps it inside the 126 MB L2 next to the streamed exit waves (part of it is still written back: profiles/r02.md).
+    // waves.  The cap keeps it below the 126 MB L2; next to the streamed exit waves it is nevertheless written back once per
+    // iteration (profiles/r02.md: 1.57 x the algorithmic DRAM bytes; a 48 MB ring avoids that and is 0.4-0.7 ms slower).
     const double ring_mb = env_int("PTYCHO_MEGA_RING_MB", 96);
     while (M > 1 && (double)(3 * c->mega_D + 1 + X) * M * c->N * c->N * 8.0 > ring_mb * 1048576.0) --M;
     c->mega_M = M;

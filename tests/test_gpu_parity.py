@@ -352,7 +352,7 @@ def test_prepare_frames_bit_exact(B, oracle_mod, in_dt, out_dt):
 # ------------------------------------------------- the steady-state path bench.py times, at full size
 def test_cfg2_full_size_steady_state_teacher_forced(B, oracle_mod, record_property):
     """Config 2 as `bench.py` times it AFTER the first iteration: psi_j is read from the 5.2 GB store, the reflector is not
-    the identity, the ring wraps ~90 times.  psi_j' of a DM iteration depends only on (O, P, psi_j, I_j), so it is teacher-forced:
+    the identity, the ring wraps ~70 times.  psi_j' of a DM iteration depends only on (O, P, psi_j, I_j), so it is teacher-forced:
     a perturbed object, psi_j = Q O_j for a perturbed probe Q (built on the device), ONE iteration, then 48 sampled frames (first,
     last, random: both sides of many ring wraps) against oracles holding just those frames with the same psi_j.  The object is
     compared with the oracle on a window, from an oracle that holds every frame overlapping the window."""

@@ -115,6 +115,12 @@ __global__ void __launch_bounds__(kDetTileW * kDetTileH) k_dm_blend_gather(float
     const int tile = blockIdx.y * gridDim.x + blockIdx.x, tid = threadIdx.y * kDetTileW + threadIdx.x;
     const int qx = blockIdx.x * kDetTileW + threadIdx.x, qy = blockIdx.y * kDetTileH + threadIdx.y;
     const int e0 = tile_start[tile], em = tile_mid[tile], e1 = tile_start[tile + 1];
+    const bool in = qy < H && qx < W;
+    const size_t i = (size_t)qy * W + qx;
+    const float2 c = in ? cO[i] : make_float2(0.f, 0.f);
+    // A tile whose correction is zero everywhere (every frame over it is inside its power bound: the steady state) keeps its
+    // object values exactly; d_O is not needed there.
+    if (!__syncthreads_or(c.x != 0.f || c.y != 0.f)) return;
     const float* pb = p2 + qy * n + qx;
     float d0 = 0.f, d1 = 0.f, d2 = 0.f, d3 = 0.f;
     for (int c0 = e0; c0 < em; c0 += NT) {                           // frames covering the whole tile: no per-pixel test, four loads in flight
@@ -139,10 +145,9 @@ __global__ void __launch_bounds__(kDetTileW * kDetTileH) k_dm_blend_gather(float
         }
     }
     const float d = (d0 + d1) + (d2 + d3);
-    if (qy >= H || qx >= W) return;
-    const size_t i = (size_t)qy * W + qx;
+    if (!in) return;
     const float inv = 1.0f / (d + sc->eps_O);
-    const float2 c = cO[i], o = O[i];
+    const float2 o = O[i];
     O[i] = make_float2(fmaf(c.x, inv, o.x), fmaf(c.y, inv, o.y));
     cO[i] = make_float2(0.f, 0.f);
 }

@@ -98,6 +98,14 @@ __device__ __forceinline__ void warp_wait(const int* cnt, int target) {
     }
     __syncwarp();
 }
+// 1 - rb of the relaxed projection (R6) of one frame from its error partials, summed in a fixed order.
+template <int N> __device__ __forceinline__ float frame_keep(const FrameArgs& a, int slot) {
+    if (!(a.pbound > 0.f)) return 1.f;
+    float e = 0.f;
+    for (int i = 0; i < Geo<N>::NCB; ++i) e += __ldcg(a.e_part + (size_t)slot * Geo<N>::NCB + i);
+    e *= 1.0f / ((float)N * (float)N);
+    return (e <= a.pbound) ? 0.f : 1.f - sqrtf(a.pbound / e);
+}
 // HBM -> L2 ahead of use (no register or shared-memory cost); bytes is a multiple of 16.
 __device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
@@ -263,10 +271,11 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(co
 // ---- pass 2: a3 column FFTs, a4 error partial, a5 modulus projection (as s - 1), a6 inverse columns
 // MODE 0: the whole pass (fused form).  Split form, used when most frames were inside the power bound in the previous iteration (R6:
 // their projection is the identity, so nothing has to be transformed back): MODE 1 = pass 2a, column FFTs and error partials only,
-// S is left untouched; MODE 2 = pass 2b, the whole pass again, but only for the frames whose error turned out to exceed the bound.
-enum { P2_FUSED = 0, P2_ERR_ONLY = 1, P2_IF_NEEDED = 2 };
-template <int N, bool U16, int MODE, bool SYNC = true> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
-                                                            float* s_red, Deferred& df) {
+// S is left untouched; MODE 2 = the whole pass once more for ONE frame whose error turned out to exceed the bound (mega_pass2b
+// below: pass 1 is known to be complete, no wait).  s_lo / s_hi >= 0 restrict the call to those slots of the wave.
+enum { P2_FUSED = 0, P2_ERR_ONLY = 1, P2_REDO = 2 };
+template <int N, bool U16, int MODE> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
+                                                            float* s_red, Deferred& df, int s_lo = -1, int s_hi = -1) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T, CB = G::LPB;
     const FrameArgs& a = m.f;
@@ -275,27 +284,16 @@ template <int N, bool U16, int MODE, bool SYNC = true> __device__ __forceinline_
     const int col = blk * CB + c;
     constexpr float inv_n2 = 1.0f / ((float)N * (float)N);
     constexpr float kAmp2Floor = 1e-30f;
-    const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
+    const int s_begin = s_lo >= 0 ? s_lo : wave * m.M, s_end = s_lo >= 0 ? s_hi : min(m.J, (wave + 1) * m.M);
     const size_t tile_bytes = (size_t)N * CB * (U16 ? 2 : 4);   // this block's intensities of one slot: contiguous
-    if (!MEGA_FLAG(m, 1) && threadIdx.x < m.M) {                              // I of the NEXT wave: HBM -> L2 now
+    if (MODE != P2_REDO && !MEGA_FLAG(m, 1) && threadIdx.x < m.M) {           // I of the NEXT wave: HBM -> L2 now
         const int s = s_begin + m.pf + threadIdx.x;
         if (s < m.J) l2_prefetch_bulk(reinterpret_cast<const char*>(m.It) + ((size_t)s * G::NCB + blk) * tile_bytes, (uint32_t)tile_bytes);
     }
     PhaseClock pc;
     for (int slot = s_begin; slot < s_end; ++slot) {
         pc.start(1);
-        if (MODE == P2_IF_NEEDED) {
-            warp_wait(m.cnt2a + slot, G::NCB);                              // every error partial of the frame is there
-            float e = 0.f;
-            for (int i = 0; i < G::NCB; ++i) e += __ldcg(a.e_part + (size_t)slot * G::NCB + i);
-            e *= 1.0f / ((float)N * (float)N);
-            if (e <= a.pbound) {                                            // inside the bound: pass 3 needs nothing from S
-                __syncthreads();
-                df.flush_cta_after_barrier();
-                df.cnt = m.cnt2 + slot;
-                continue;
-            }
-        } else if (SYNC) warp_wait(m.cnt1 + slot, G::NCB * kWarps);
+        if (MODE != P2_REDO) warp_wait(m.cnt1 + slot, G::NCB * kWarps);
         pc.lap(0);
         float2* base = a.S + (size_t)(slot % m.R) * N * N + col;
         float2 v[E];
@@ -352,9 +350,28 @@ template <int N, bool U16, int MODE, bool SYNC = true> __device__ __forceinline_
 #pragma unroll
         for (int r = 0; r < E; ++r) __stcg(base + (size_t)pos_a_inv<N>(t, r) * N, v[r]);
         __syncthreads();                                                    // sx and s_red free; stores issued by all
-        if (SYNC) df.cnt = m.cnt2 + slot;
+        df.cnt = m.cnt2 + slot;
         if (MEGA_FLAG(m, 4)) df.flush_cta_after_barrier();
         pc.lap(3);
+    }
+}
+
+// ---- pass 2b of the split form: ONE item per wave.  For every frame of the wave: once all its error partials are there, a frame
+// inside its power bound is passed on to pass 3 at once (the common case: a few microseconds per wave); a frame outside it gets
+// the whole pass 2, all NCB column blocks, from this CTA (rare once the split form is in use).
+template <int N, bool U16> __device__ __forceinline__ void mega_pass2b(const MegaArgs& m, int wave, float2* sm, const float4* s_tw, float* s_red,
+                                                                       Deferred& df) {
+    using G = Geo<N>;
+    const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
+    for (int slot = s_begin; slot < s_end; ++slot) {
+        warp_wait(m.cnt2a + slot, G::NCB);                                  // every error partial of the frame is there
+        if (frame_keep<N>(m.f, slot) == 0.f) {                              // inside the bound: pass 3 needs nothing from S
+            __syncthreads();
+            df.flush_cta_after_barrier();
+            if (threadIdx.x == 0) asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(m.cnt2 + slot), "r"(G::NCB) : "memory");
+            continue;
+        }
+        for (int blk = 0; blk < G::NCB; ++blk) mega_pass2<N, U16, P2_REDO>(m, blk, wave, sm, s_tw, s_red, df, slot, slot + 1);
     }
 }
 
@@ -376,17 +393,14 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
     PhaseClock pc;
     for (int slot = s_begin; slot < s_end; ++slot) {
         pc.start(2);
+        const YX p0 = m.spos[slot];                                         // (independent of the hand-off: in flight during the poll)
         if (SYNC) warp_wait(m.cnt2 + slot, G::NCB);
         pc.lap(0);
-        const YX p0 = m.spos[slot];
-        float keep = 1.f;                                                   // 1 - rb  (R6)
-        if (a.pbound > 0.f) {
-            float e = 0.f;
-            for (int i = 0; i < G::NCB; ++i) e += __ldcg(a.e_part + (size_t)slot * G::NCB + i);
-            e *= 1.0f / ((float)N * (float)N);
-            keep = (e <= a.pbound) ? 0.f : 1.f - sqrtf(a.pbound / e);
-        }
         const size_t obase = (size_t)(p0.y + y) * a.W + p0.x;
+        float2 o[E];                                                        // O_j (natural order), needed by both branches: issued before
+#pragma unroll                                                              // the blend weight's loads, one latency for both
+        for (int i = 0; i < E; ++i) o[i] = __ldg(a.O + obase + t + T * i);
+        const float keep = frame_keep<N>(a, slot);                          // 1 - rb  (R6)
         float2* prow = a.psi + (size_t)slot * N * N + off;
         if (m.corr && blk == 0 && threadIdx.x == 0 && keep == 0.f) atomicAdd(m.stat + 1, 1);   // statistic for the next iteration's form
         if (m.corr && keep == 0.f) {
@@ -396,7 +410,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
 #pragma unroll
             for (int i = 0; i < E; ++i) {
                 const int x = t + T * i;
-                __stcs(prow + x, cmul(sP[x], __ldg(a.O + obase + x)));
+                __stcs(prow + x, cmul(sP[x], o[i]));
             }
             continue;
         }
@@ -404,9 +418,6 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
         float2 v[E];
 #pragma unroll
         for (int r = 0; r < E; ++r) v[r] = __ldcg(srow + freq_b<N>(t, r));
-        float2 o[E];                                                        // O_j: in flight during the butterflies
-#pragma unroll
-        for (int r = 0; r < E; ++r) o[r] = __ldg(a.O + obase + pos_a_inv<N>(t, r));
         PHASE_TOUCH(v[E - 1].x + keep);
         pc.lap(1);
         fft_line_inv<N, true>(v, t, sx, s_tw + N);                          // v = F^-1[(s-1) Phi]
@@ -417,7 +428,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
         for (int r = 0; r < E; ++r) {
             const int x = pos_a_inv<N>(t, r);
             const float2 p = sP[x];
-            const float2 po = cmul(p, o[r]);
+            const float2 po = cmul(p, o[brev<E>(r)]);                     // x = t + T brev(r)
             const float2 kv = make_float2(keep * v[r].x, keep * v[r].y);
             const float2 w = cadd(po, kv);                                  // a7
             __stcs(prow + x, w);
@@ -442,9 +453,10 @@ template <int N, bool U16> __global__ void __launch_bounds__(kThreads, (N >= 512
     load_tw(s_tw, m.f.tw, m.f.twi, N);
     // split form when most frames were inside the power bound last time (their projection is the identity)
     const bool split = m.corr && m.f.pbound > 0.f && 2 * m.stat[0] > m.J;
-    const int nk = split ? 4 : 3;                             // item kinds per queue wave
-    const int per_qw = nk * G::NCB;
-    const int total = (m.nW + (nk - 1) * m.D) * per_qw;
+    // fused form: NCB pass-3, NCB pass-2, NCB pass-1 items per queue wave, lags 2D / D / 0.  split form: NCB pass-3 items, ONE
+    // pass-2b item, NCB pass-2a items, NCB pass-1 items, lags 3D / 2D / D / 0.
+    const int per_qw = 3 * G::NCB + (split ? 1 : 0);
+    const int total = (m.nW + (split ? 3 : 2) * m.D) * per_qw;
     Deferred df;
     bool df_cta = false;                                      // the pending signal is a CTA-level one (pass 2)
 #ifdef PTYCHO_PHASE_PROF
@@ -463,15 +475,20 @@ template <int N, bool U16> __global__ void __launch_bounds__(kThreads, (N >= 512
         const int q = s_item;
         if (q >= total) break;
         const int qw = q / per_qw, idx = q % per_qw;
-        const int kind = idx / G::NCB, blk = idx % G::NCB;    // fused: 0 pass 3, 1 pass 2, 2 pass 1; split: 0 pass 3, 1 pass 2b, 2 pass 2a, 3 pass 1
-        const int wave = qw - (nk - 1 - kind) * m.D;
+        int kind, blk;                                           // 0 pass 3, 1 pass 2 (fused) / 2b (split), 2 pass 2a (split only), 3 pass 1
+        if (idx < G::NCB) { kind = 0; blk = idx; }
+        else if (!split) { kind = idx < 2 * G::NCB ? 1 : 3; blk = idx % G::NCB; }
+        else if (idx == G::NCB) { kind = 1; blk = 0; }
+        else { kind = idx <= 2 * G::NCB ? 2 : 3; blk = (idx - 1) % G::NCB; }
+        const int lag = kind == 3 ? 0 : split ? (3 - kind) : (2 - kind);
+        const int wave = qw - lag * m.D;
         if (wave < 0 || wave >= m.nW) continue;
-        df_cta = kind == 1 || (split && kind == 2);
-        if (kind == nk - 1) mega_pass1<N>(m, blk, wave, sm, s_tw, df);
+        df_cta = kind == 1 || kind == 2;
+        if (kind == 3) mega_pass1<N>(m, blk, wave, sm, s_tw, df);
         else if (kind == 0) mega_pass3<N>(m, blk, wave, sm, s_tw, df);
         else if (!split) mega_pass2<N, U16, P2_FUSED>(m, blk, wave, sm, s_tw, s_red, df);
         else if (kind == 2) mega_pass2<N, U16, P2_ERR_ONLY>(m, blk, wave, sm, s_tw, s_red, df);
-        else mega_pass2<N, U16, P2_IF_NEEDED>(m, blk, wave, sm, s_tw, s_red, df);
+        else mega_pass2b<N, U16>(m, wave, sm, s_tw, s_red, df);
     }
 #ifdef PTYCHO_PHASE_PROF
     __syncthreads();

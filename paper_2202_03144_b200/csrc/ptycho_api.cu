@@ -187,13 +187,13 @@ void mega_config(ptycho_ctx* c) {
     if (cudaGetDevice(&dev) == cudaSuccess) { int v = 0; if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v; }
     cudaGetLastError();
     const int grid = sms * (c->N >= 512 ? 1 : PTYCHO_MEGA_OCC);
-    // About grid / (4 NCB) queue waves are in flight in the split form (four item kinds per wave), grid / (3 NCB) in the fused one.
-    // Measured on config 2 (B200, round 2): D = 6, X = 5, M = 6 (ring 144 frames, 75 MB) 7.95 / 6.03 ms per early / steady-state
-    // iteration; D = X = 9, M = 3: 8.33 / 6.73; M = 2: 8.9 / 7.4.  More slots per item amortise the item's probe rows, its claim and
+    // About grid / (3 NCB) queue waves are in flight (3 NCB items per wave, + 1 in the split form).
+    // Measured on config 2 (B200, round 2): D = 6, X = 5, M = 6 (ring 144 frames, 75 MB) 8.03 / 5.10 ms per early / steady-state
+    // iteration (D = 8, X = 7: 8.4 / 5.4); with the earlier sixteen-item pass 2b: M = 6 7.95 / 6.03, M = 3 8.33 / 6.73, M = 2 8.9 / 7.4.  More slots per item amortise the item's probe rows, its claim and
     // its probe-sum flush.
-    const int inflight = (grid + 4 * ncb_of(c->N) - 1) / (4 * ncb_of(c->N));
-    c->mega_D = std::max(2, env_int("PTYCHO_MEGA_D", inflight + 1));
-    const int X = std::max(0, env_int("PTYCHO_MEGA_X", inflight));
+    const int inflight = grid / (3 * ncb_of(c->N) + 1);
+    c->mega_D = std::max(2, env_int("PTYCHO_MEGA_D", std::max(3, inflight)));
+    const int X = std::max(0, env_int("PTYCHO_MEGA_X", std::max(2, inflight - 1)));
     int M = std::max(1, std::min(env_int("PTYCHO_MEGA_M", 6), c->J));
     // The split form of the queue (dm_mega.cuh) puts three lags between pass 1 and pass 3 of a frame, so the ring spans 3 D + 1 + X
     // waves.  The cap keeps it below the 126 MB L2; next to the streamed exit waves it is nevertheless written back once per

@@ -264,7 +264,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_cols(Fr
 // a6 (rows) / a7 / a8 / a9: inverse row FFTs -> revised wave -> exit-wave update -> scatter-add.
 // grid (NCB, nframes)
 // ------------------------------------------------------------------------------------------
-template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_inv(FrameArgs a) {
+template <int N, int MODE> __global__ void __launch_bounds__(kThreads, (N >= 512 ? 1 : 2)) k_rows_inv(FrameArgs a) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T;
     extern __shared__ __align__(16) float2 sm[];
@@ -587,6 +587,22 @@ __global__ void k_lsq_pf_apply(float2* x, float2* dir, float* aw, float* ww, siz
 __global__ void k_set_steps(Scalars* sc, float a, float b, double* steps_out) {
     sc->step_a = a; sc->step_b = b;
     if (steps_out) { steps_out[0] = a; steps_out[1] = b; }
+}
+
+// ePIE-minibatch (R8) in ONE pass over a canvas: x += alpha n / (d + delta max); zero n and d.  which = 0: object (max = max_p2),
+// 1: probe (max = max_dp).  (LSQML needs the directions before it knows its steps: k_direction, then k_apply.)
+__global__ void k_epie_update(float2* x, float2* n, float* d, size_t plane, int modes, float delta, float alpha, const Scalars* sc, int which,
+                              int update) {
+    const float reg = delta * (which ? sc->max_dp : sc->max_p2);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < plane; i += (size_t)gridDim.x * blockDim.x) {
+        const float st = alpha / (d[i] + reg);
+        for (int k = 0; k < modes; ++k) {
+            const size_t q = (size_t)k * plane + i;
+            if (update) { const float2 nv = n[q]; float2 xv = x[q]; xv.x = fmaf(st, nv.x, xv.x); xv.y = fmaf(st, nv.y, xv.y); x[q] = xv; }
+            n[q] = make_float2(0.f, 0.f);
+        }
+        d[i] = 0.f;
+    }
 }
 
 // x += step * dir; zero dir and d.  which = 0: step_a, 1: step_b.

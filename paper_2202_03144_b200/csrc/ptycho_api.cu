@@ -512,6 +512,17 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
         }
         const bool lsq = alg == PTYCHO_LSQML, pfm = alg == PTYCHO_LSQML_PF;
         const int gO = ew_blocks(HW), gP = ew_blocks(nn);
+        if (!lsq && !pfm) {                                 // ePIE: directions and steps in one pass per canvas
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_epie_update<<<gO, 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->par.delta_obj, c->par.alpha_obj, c->sc, 0, 1)));
+            if (upd) {
+                CU(cudaMemsetAsync(&c->sc->max_dp, 0, sizeof(float), c->stream));
+                LAUNCH(c, PTYCHO_K_UPDATE, (k_real_max<<<64, 256, 0, c->stream>>>(c->dP, (int)nn, c->sc)));
+            }
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_epie_update<<<gP, 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->par.delta_probe, c->par.alpha_probe, c->sc, 1, upd)));
+            if (c->n_steps < kStepCap) LAUNCH(c, PTYCHO_K_UPDATE, (k_set_steps<<<1, 1, 0, c->stream>>>(c->sc, c->par.alpha_obj, upd ? c->par.alpha_probe : 0.f, c->steps + 2 * c->n_steps)));
+            ++c->n_steps;
+            continue;
+        }
         LAUNCH(c, PTYCHO_K_UPDATE, (k_direction<<<gO, 256, 0, c->stream>>>(c->nO, c->dO, HW, 1, c->par.delta_obj, c->sc, 0, lsq ? c->partO : nullptr)));
         if (upd) {
             CU(cudaMemsetAsync(&c->sc->max_dp, 0, sizeof(float), c->stream));

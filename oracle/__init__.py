@@ -257,3 +257,30 @@ def prepare_frames(raw, center, n, threshold=0.0, saturation=0.0, out_dtype=np.u
         out = val.astype(np.float32)
         out[masked] = -1.0
     return out
+
+
+# --------------------------------------------------------------------------------------------------
+# Probe-mode orthogonalisation (reading R26; "several probe modes").  TEST INFRASTRUCTURE.
+# The K modes are mixed by the unitary that diagonalises their Gram matrix G_ij = sum_r P_i(r) conj(P_j(r)): P' = V^H P with
+# G = V diag(lambda) V^H, lambda descending (numpy.linalg.eigh is the library step).  Each eigenvector's phase is fixed by making its
+# largest-magnitude component real and positive.  sum_k |P'_k(r)|^2 = sum_k |P_k(r)|^2 at every pixel, so the model intensities do not
+# change; the same mixing applied to stored exit waves keeps them consistent.
+def mode_mixing_matrix(P):
+    K = P.shape[0]
+    flat = np.asarray(P, np.complex128).reshape(K, -1)
+    G = flat @ flat.conj().T
+    lam, V = np.linalg.eigh(G)
+    order = np.argsort(-lam, kind="stable")
+    V = V[:, order]
+    for m in range(K):
+        i = int(np.argmax(np.abs(V[:, m])))
+        V[:, m] *= np.exp(-1j * np.angle(V[i, m]))
+    return V.conj().T                                      # U = V^H: P' = U P
+
+
+def orthogonalize_modes(P, psi=None):
+    U = mode_mixing_matrix(P)
+    P2 = np.tensordot(U, np.asarray(P, np.complex128), axes=(1, 0))
+    if psi is None:
+        return P2
+    return P2, np.einsum("mk,jkyx->jmyx", U, np.asarray(psi, np.complex128))

@@ -549,3 +549,27 @@ def test_lsqml_per_frame_reduces_to_joint_step_for_one_frame(oracle_mod):
     c = synth.make_config(0)
     e = np.array(oracle_mod.Oracle(c.obj0, c.probe0, c.pos, c.intensities, dict(batch_size=16)).iterate("LSQML_PF", 30).err)
     assert np.all(np.diff(e) < 0) and e[-1] < 1e-2 * e[0], e                    # R22: monotone on noiseless data
+
+
+def test_mode_orthogonalisation_pins(oracle_mod):
+    """R26: the mixed modes have a diagonal Gram matrix with the eigenvalues of the old one (numpy.linalg.eigvalsh, a different
+    routine) in descending order; the incoherent sum sum_k |P_k|^2 is unchanged at every pixel; modes that are already orthogonal
+    with distinct powers come back unchanged; two identical modes collapse into one; exit waves mixed alike stay P'_k O_j."""
+    p = crandn(3, 12, 12) * np.array([1.0, 0.6, 0.3])[:, None, None]
+    p[1] += 0.5 * p[0]                                                           # make them clearly non-orthogonal
+    q = oracle_mod.orthogonalize_modes(p)
+    g = q.reshape(3, -1) @ q.reshape(3, -1).conj().T
+    lam = np.linalg.eigvalsh(p.reshape(3, -1) @ p.reshape(3, -1).conj().T)[::-1]
+    assert np.abs(g - np.diag(np.diag(g))).max() < 1e-10 * lam[0]
+    assert np.allclose(np.diag(g).real, lam, rtol=1e-12) and np.all(np.diff(np.diag(g).real) <= 0)
+    assert np.allclose(np.sum(np.abs(q) ** 2, 0), np.sum(np.abs(p) ** 2, 0), rtol=1e-12)
+    s, _ = f64_scan(k=3)                                                         # synth's modes: Gram-Schmidt, powers 0.80 / 0.15 / 0.05
+    assert rel(oracle_mod.orthogonalize_modes(s.probe_true), s.probe_true) < 1e-12
+    twin = np.stack([p[0], p[0]])
+    t = oracle_mod.orthogonalize_modes(twin)
+    assert rel(t[0], np.sqrt(2) * p[0]) < 1e-12 and np.abs(t[1]).max() < 1e-12 * np.abs(p).max()
+    obj = crandn(20, 20)
+    psi = np.stack([p * obj[None, y:y + 12, x:x + 12] for y, x in ((0, 0), (3, 5), (8, 8))])
+    q2, psi2 = oracle_mod.orthogonalize_modes(p, psi)
+    want = np.stack([q2 * obj[None, y:y + 12, x:x + 12] for y, x in ((0, 0), (3, 5), (8, 8))])
+    assert rel(psi2, want) < 1e-12

@@ -166,6 +166,14 @@ ptycho_status ptycho_append_frames(ptycho_ctx *ctx, int first_frame, int count, 
 ptycho_status ptycho_wait_frames(ptycho_ctx *ctx);     /* blocks until every appended frame is on the device */
 int ptycho_frames_present(const ptycho_ctx *ctx);
 
+/* Probe-mode orthogonalisation (reading R26; PAPER.md:49 several probe modes).  The K modes are replaced by
+ * P' = U P, U = V^H the unitary that diagonalises their Gram matrix G_ij = sum_r P_i(r) conj(P_j(r)) = V diag(lambda) V^H, lambda
+ * descending; each eigenvector's phase is fixed by making its largest-magnitude component real and positive.  sum_k |P_k(r)|^2
+ * is unchanged at every pixel, so the model intensities are unchanged; stored DM exit waves are mixed alike.  The Gram matrix is
+ * formed on the device in double; the K x K eigenproblem (K <= 8) is solved on the host (cyclic Jacobi): the call synchronises
+ * the stream.  K = 1: no-op. */
+ptycho_status ptycho_orthogonalize_modes(ptycho_ctx *ctx);
+
 /* Per-kernel-class device timing (SURVEY.md 8(d) "Evidence to collect"; bench.py's roofline
  * object).  ptycho_profile(ctx, 1) resets the totals and makes every later launch of this context
  * be bracketed by two cudaEvents on the context's stream; ptycho_profile(ctx, 0) stops that.

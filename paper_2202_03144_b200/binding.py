@@ -87,6 +87,7 @@ def lib():
         l.ptycho_destroy.argtypes = [C.c_void_p]
         l.ptycho_append_frames.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         l.ptycho_wait_frames.argtypes = [C.c_void_p]
+        l.ptycho_orthogonalize_modes.argtypes = [C.c_void_p]
         l.ptycho_frames_present.argtypes = [C.c_void_p]
         l.ptycho_default_params.argtypes = [C.POINTER(Params)]
         l.ptycho_test_fft2.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
@@ -175,6 +176,9 @@ class Ptycho:
         intensities = intensities if not isinstance(intensities, np.ndarray) else np.ascontiguousarray(intensities)
         self._keep = intensities                                # must stay valid until wait_frames()
         self._check(self._l.ptycho_append_frames(self._h, int(first_frame), int(intensities.shape[0]), _ptr(intensities)))
+
+    def orthogonalize_modes(self):
+        self._check(self._l.ptycho_orthogonalize_modes(self._h))
 
     def wait_frames(self):
         self._check(self._l.ptycho_wait_frames(self._h))

@@ -673,6 +673,43 @@ __global__ void k_finish_init(Scalars* sc, float delta, int J, int which) {
 }
 
 // ------------------------------------------------------------------------------------------
+// probe-mode orthogonalisation (include/ptycho_b200.h: ptycho_orthogonalize_modes; reading R26)
+// ------------------------------------------------------------------------------------------
+// Gram matrix partials: grid (K*K, kGramBlocks); block (i*K + j, b) sums P_i conj(P_j) over its share of the pixels, in double.
+constexpr int kGramBlocks = 32;
+__global__ void __launch_bounds__(256) k_gram(const float2* __restrict__ P, int K, int nn, double2* __restrict__ part) {
+    const int i = blockIdx.x / K, j = blockIdx.x % K;
+    double re = 0.0, im = 0.0;
+    for (int q = blockIdx.y * 256 + threadIdx.x; q < nn; q += gridDim.y * 256) {
+        const float2 a = P[(size_t)i * nn + q], b = P[(size_t)j * nn + q];
+        re += (double)a.x * b.x + (double)a.y * b.y;                  // a conj(b)
+        im += (double)a.y * b.x - (double)a.x * b.y;
+    }
+    __shared__ double sr[8], si[8];
+    for (int s = 16; s > 0; s >>= 1) { re += __shfl_xor_sync(0xffffffffu, re, s); im += __shfl_xor_sync(0xffffffffu, im, s); }
+    if ((threadIdx.x & 31) == 0) { sr[threadIdx.x >> 5] = re; si[threadIdx.x >> 5] = im; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) { re += sr[w]; im += si[w]; }
+        part[blockIdx.x * gridDim.y + blockIdx.y] = make_double2(re, im);
+    }
+}
+struct MixMatrix { float2 u[8][8]; };   // PTYCHO_MAX_MODES = 8
+// x'_m = sum_k U[m][k] x_k at every pixel of every frame (in place).  grid (ceil(nn / 256), frames)
+__global__ void __launch_bounds__(256) k_mix_modes(float2* __restrict__ x, int K, int nn, MixMatrix U) {
+    const int q = blockIdx.x * 256 + threadIdx.x;
+    if (q >= nn) return;
+    float2* base = x + (size_t)blockIdx.y * K * nn + q;
+    float2 in[8];
+    for (int k = 0; k < K; ++k) in[k] = base[(size_t)k * nn];
+    for (int m = 0; m < K; ++m) {
+        float2 acc = make_float2(0.f, 0.f);
+        for (int k = 0; k < K; ++k) acc = cadd(acc, cmul(U.u[m][k], in[k]));
+        base[(size_t)m * nn] = acc;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // init-time preparation of raw detector frames (include/ptycho_b200.h: ptycho_prepare_frames)
 // ------------------------------------------------------------------------------------------
 // (uy, ux) = source offset from the centre pixel for the output offset (dy, dx) after `rot` quarter turns counter-clockwise

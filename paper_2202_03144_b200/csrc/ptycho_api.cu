@@ -8,6 +8,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <complex>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -936,6 +937,77 @@ ptycho_status ptycho_wait_frames(ptycho_ctx* c) {
     return PTYCHO_OK;
 }
 int ptycho_frames_present(const ptycho_ctx* c) { return c ? c->present : 0; }
+
+// Hermitian K x K eigenproblem by cyclic complex Jacobi rotations (host, K <= 8).  On return g is diagonal (eigenvalues on the
+// diagonal) and the columns of v are the eigenvectors of the input.
+static void jacobi_hermitian(int K, std::vector<std::complex<double>>& g, std::vector<std::complex<double>>& v) {
+    using cd = std::complex<double>;
+    v.assign((size_t)K * K, cd(0, 0));
+    for (int i = 0; i < K; ++i) v[i * K + i] = 1.0;
+    for (int sweep = 0; sweep < 64; ++sweep) {
+        double off = 0, diag = 0;
+        for (int p = 0; p < K; ++p) for (int q = 0; q < K; ++q) (p == q ? diag : off) += std::norm(g[p * K + q]);
+        if (off <= 1e-30 * diag) break;
+        for (int p = 0; p < K; ++p)
+            for (int q = p + 1; q < K; ++q) {
+                const cd gpq = g[p * K + q];
+                const double apq = std::abs(gpq);
+                if (apq == 0) continue;
+                const cd ph = gpq / apq;                                  // e^{i phi}
+                const double app = g[p * K + p].real(), aqq = g[q * K + q].real();
+                const double th = 0.5 * std::atan2(2 * apq, app - aqq);
+                const double cs = std::cos(th), sn = std::sin(th);
+                // rotation R: column p = (cs, sn conj(ph)) , column q = (-sn ph, cs) in rows (p, q)
+                for (int k = 0; k < K; ++k) {                              // G <- G R
+                    const cd gp = g[k * K + p], gq = g[k * K + q];
+                    g[k * K + p] = cs * gp + sn * std::conj(ph) * gq;
+                    g[k * K + q] = -sn * ph * gp + cs * gq;
+                }
+                for (int k = 0; k < K; ++k) {                              // G <- R^H G
+                    const cd gp = g[p * K + k], gq = g[q * K + k];
+                    g[p * K + k] = cs * gp + sn * ph * gq;
+                    g[q * K + k] = -sn * std::conj(ph) * gp + cs * gq;
+                }
+                for (int k = 0; k < K; ++k) {                              // V <- V R
+                    const cd vp = v[k * K + p], vq = v[k * K + q];
+                    v[k * K + p] = cs * vp + sn * std::conj(ph) * vq;
+                    v[k * K + q] = -sn * ph * vp + cs * vq;
+                }
+            }
+    }
+}
+
+ptycho_status ptycho_orthogonalize_modes(ptycho_ctx* c) {
+    if (!c) return PTYCHO_EINVAL;
+    const int K = c->K, nn = c->N * c->N;
+    if (K == 1) return PTYCHO_OK;
+    using cd = std::complex<double>;
+    double2* part = reinterpret_cast<double2*>(c->scratch_d);             // K*K*kGramBlocks double2 = at most 4096 of its 4736 doubles
+    LAUNCH(c, PTYCHO_K_OTHER, (k_gram<<<dim3(K * K, kGramBlocks), 256, 0, c->stream>>>(c->P, K, nn, part)));
+    std::vector<double2> hp((size_t)K * K * kGramBlocks);
+    CU(cudaMemcpyAsync(hp.data(), part, hp.size() * sizeof(double2), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    std::vector<cd> g((size_t)K * K), v;
+    for (int e = 0; e < K * K; ++e) { cd s(0, 0); for (int b = 0; b < kGramBlocks; ++b) s += cd(hp[e * kGramBlocks + b].x, hp[e * kGramBlocks + b].y); g[e] = s; }
+    jacobi_hermitian(K, g, v);
+    std::vector<int> order(K);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return g[a * K + a].real() > g[b * K + b].real(); });
+    MixMatrix U{};
+    for (int m = 0; m < K; ++m) {
+        const int col = order[m];
+        int big = 0;
+        for (int i = 1; i < K; ++i) if (std::abs(v[i * K + col]) > std::abs(v[big * K + col])) big = i;
+        const cd ph = std::conj(v[big * K + col]) / std::abs(v[big * K + col]);   // makes the largest component real positive
+        for (int k = 0; k < K; ++k) { const cd u = std::conj(v[k * K + col] * ph); U.u[m][k] = make_float2((float)u.real(), (float)u.imag()); }   // U = V^H
+    }
+    LAUNCH(c, PTYCHO_K_OTHER, (k_mix_modes<<<dim3((nn + 255) / 256, 1), 256, 0, c->stream>>>(c->P, K, nn, U)));
+    if (c->psi && c->psi_valid)
+        LAUNCH(c, PTYCHO_K_OTHER, (k_mix_modes<<<dim3((nn + 255) / 256, c->J), 256, 0, c->stream>>>(c->psi, K, nn, U)));
+    CU(cudaStreamSynchronize(c->stream));
+    CU(cudaGetLastError());
+    return PTYCHO_OK;
+}
 
 ptycho_status ptycho_profile(ptycho_ctx* c, int enable) {
     if (!c) return PTYCHO_EINVAL;

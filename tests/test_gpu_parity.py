@@ -619,3 +619,27 @@ def test_lsqml_per_frame_steps(B, oracle_mod, n, h, side, step, k, batch):
         assert np.allclose(a[np.lexsort(a.T)], b[np.lexsort(b.T)], rtol=2e-3, atol=1e-5), i0
         i0 += sz
     assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+
+
+# ------------------------------------------------------------------ f4 (part): probe-mode orthogonalisation (R26)
+def test_mode_orthogonalisation(B, oracle_mod):
+    """After a few LSQML-style iterations the three modes are no longer orthogonal; ptycho_orthogonalize_modes must give the
+    oracle's mixing of the SAME modes (Gram eigen-decomposition, phase convention), leave sum_k |P_k|^2 alone, and mix stored DM
+    exit waves alike."""
+    s = synth.make_custom(64, 200, 5, 24, k=3, peak=2e4, dtype=np.float32, jitter=2, seed=61, probe_kind="disk")
+    g = make(B, s, batch_size=8)
+    g.iterate("LSQML", 3)
+    g.iterate("DM", 1)                                           # fills the exit-wave store (K = 3: three-pass DM path)
+    p_before, psi_before = g.fetch_probe(), g.fetch_exit_waves()
+    flat = p_before.reshape(3, -1).astype(np.complex128)
+    gram = flat @ flat.conj().T
+    assert np.abs(gram[0, 1]) > 1e-4 * gram[0, 0].real           # really non-orthogonal now
+    want_p, want_psi = oracle_mod.orthogonalize_modes(p_before, psi_before)
+    g.orthogonalize_modes()
+    p_after = g.fetch_probe()
+    assert rel(p_after, want_p) < 2e-6 and rel(g.fetch_exit_waves(), want_psi) < 2e-6
+    assert np.allclose(np.sum(np.abs(p_after) ** 2, 0), np.sum(np.abs(p_before) ** 2, 0), rtol=1e-5)
+    g.iterate("LSQML", 1)                                        # and the run goes on
+    assert np.isfinite(g.fetch_error()[-1])
+    one = make(B, synth.make_config(0))
+    one.orthogonalize_modes()                                    # K = 1: no-op

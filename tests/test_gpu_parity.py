@@ -389,6 +389,33 @@ def test_cfg2_full_size_steady_state_teacher_forced(B, oracle_mod, record_proper
     O_g = g.fetch_object()
     assert rel(O_g[y0:y0 + w, x0:x0 + w], ow.O[y0:y0 + w, x0:x0 + w]) < TOL_ITER
     assert np.isfinite(g.fetch_error()[-1])
+    # The same check in the regime most of bench.py's iterations are in: after 14 iterations every frame is inside its power bound,
+    # the kernel runs its split form and the short pass 3.  Iteration 15 is teacher-forced from the GPU's own state.
+    gs = make(B, s, **par)
+    gs.iterate("DM", 14)
+    O14, P14, psi14 = gs.fetch_object(), gs.fetch_probe(), gs.fetch_exit_waves(idx)
+    gs.iterate("DM", 1)
+    o15 = oracle_mod.Oracle(O14, P14, s.pos[idx], s.intensities[idx], par)
+    o15.psi = psi14.astype(np.complex128)
+    o15.iterate("DM", 1)
+    psi15 = gs.fetch_exit_waves(idx)
+    assert max(rel(psi15[k], o15.psi[k]) for k in range(len(idx))) < TOL_ITER
+    mean_e = o15.err[0] * o15.sum_I / (len(idx) * n * n)
+    assert mean_e < par["pbound"], mean_e                        # the sampled frames are inside the bound: this WAS the short path
+    ow15 = oracle_mod.Oracle(O14, P14, s.pos[cover], s.intensities[cover], par)
+    ow15.psi = gs.fetch_exit_waves(cover).astype(np.complex128)  # (already iteration 15's waves: the object step uses the NEW waves)
+    O15 = gs.fetch_object()
+    # object window from the closed form of step 5 with the new waves: O + sum_j conj(P)(psi'_j - P O_j) / (d_O + eps)
+    num = np.zeros((w, w), complex); den = np.zeros((w, w))
+    for k, j in enumerate(cover):
+        py, px = s.pos[j]
+        ys, ye, xs, xe = max(y0, py), min(y0 + w, py + n), max(x0, px), min(x0 + w, px + n)
+        sl = (slice(ys - py, ye - py), slice(xs - px, xe - px))
+        num[ys - y0:ye - y0, xs - x0:xe - x0] += np.conj(P14[0][sl]) * ow15.psi[k, 0][sl]
+        den[ys - y0:ye - y0, xs - x0:xe - x0] += np.abs(P14[0][sl]) ** 2
+    eps = 1e-2 * np.max(np.abs(s.probe0) ** 2)
+    assert rel(O15[y0:y0 + w, x0:x0 + w], (num + eps * O14[y0:y0 + w, x0:x0 + w]) / (den + eps)) < TOL_ITER
+    gs.destroy()
     # three free-running iterations against the full oracle, where the host can hold psi in double (10.5 GB)
     import psutil
     ran_full = psutil.virtual_memory().available > 40 * 2 ** 30
@@ -643,3 +670,22 @@ def test_mode_orthogonalisation(B, oracle_mod):
     assert np.isfinite(g.fetch_error()[-1])
     one = make(B, synth.make_config(0))
     one.orthogonalize_modes()                                    # K = 1: no-op
+
+
+def test_split_form_under_queue_geometries(B, oracle_mod, monkeypatch):
+    """The split form of the DM queue (error-only column pass, one pass-2b item per wave, short pass 3) under several queue
+    geometries, ragged last wave and ring wrap included: with a wide power bound the frames are inside it after a few
+    iterations, so the later ones run in that form; the oracle's result must come out whatever M, D, X are."""
+    s = synth.make_custom(128, 420, 7, 37, k=1, peak=2e4, dtype=np.uint16, jitter=3, seed=71, probe_kind="zone")
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, dict(pbound=3.0)).iterate("DM", 12)
+    assert o.err[6] * o.sum_I / (o.J * 128 * 128) < 3.0          # inside the bound half-way: the later iterations used the split form
+    for M, D, X in ((1, 2, 0), (3, 2, 1), (5, 3, 4), (64, 2, 0), (6, 6, 5)):
+        monkeypatch.setenv("PTYCHO_MEGA_M", str(M))
+        monkeypatch.setenv("PTYCHO_MEGA_D", str(D))
+        monkeypatch.setenv("PTYCHO_MEGA_X", str(X))
+        g = make(B, s, pbound=3.0)
+        g.iterate("DM", 12)
+        assert rel(g.fetch_object(), o.O) < 10 * TOL_ITER and rel(g.fetch_probe(), o.P) < 10 * TOL_ITER, (M, D, X)
+        assert rel(g.fetch_exit_waves(), o.psi) < 10 * TOL_ITER, (M, D, X)
+        assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+        g.destroy()

@@ -107,8 +107,12 @@ template <int N> __device__ __forceinline__ float frame_keep(const FrameArgs& a,
     return (e <= a.pbound) ? 0.f : 1.f - sqrtf(a.pbound / e);
 }
 // HBM -> L2 ahead of use (no register or shared-memory cost); bytes is a multiple of 16.
+// The prefetched data (exit waves, intensities) is streamed: used once, so it enters L2 as evict-first and does not push the
+// ring S out (the ring is what should stay resident).
 __device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(p), "r"(bytes), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void l2_prefetch(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 // A signal is sent one slot LATE (after the next slot's butterflies): by then the stores it covers
@@ -199,7 +203,7 @@ template <int N> struct MegaGeo {
 
 // ---- pass 1: a1 exit wave, a2 reflector, a9 lagged probe sums, a3 forward row FFTs -> S --------
 template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
-                                                            Deferred& df) {
+                                                            Deferred& df, bool split) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T, LW = 32 / T;
     const FrameArgs& a = m.f;
@@ -248,6 +252,9 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(co
                 accD[i] = fmaf(o.x, o.x, fmaf(o.y, o.y, accD[i]));
             }
             v[i] = make_float2(fmaf(2.f, po.x, -s.x), fmaf(2.f, po.y, -s.y));   // reflector
+            // split form: psi_j is overwritten with P O_j right away -- that IS the new exit wave of a frame inside its power bound
+            // (keep = 0), so such a frame needs no pass 3 at all; a frame outside it has psi' = P O_j + keep v written by pass 3.
+            if (split) __stcs(const_cast<float2*>(prow) + t + T * i, po);
         }
         fft_line_fwd<N, true>(v, t, sx, s_tw);
         __syncwarp();                                                       // sx is free for the next slot
@@ -365,10 +372,16 @@ template <int N, bool U16> __device__ __forceinline__ void mega_pass2b(const Meg
     const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
     for (int slot = s_begin; slot < s_end; ++slot) {
         warp_wait(m.cnt2a + slot, G::NCB);                                  // every error partial of the frame is there
-        if (frame_keep<N>(m.f, slot) == 0.f) {                              // inside the bound: pass 3 needs nothing from S
+        if (frame_keep<N>(m.f, slot) == 0.f) {
+            // Inside the bound: pass 1 has already written psi' = P O_j, nothing is scattered, S[slot] is not needed any more.  The
+            // frame is marked "nothing to do" for pass 3 (counter value 2 NCB) and its ring slot is released here.
             __syncthreads();
             df.flush_cta_after_barrier();
-            if (threadIdx.x == 0) asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(m.cnt2 + slot), "r"(G::NCB) : "memory");
+            if (threadIdx.x == 0) {
+                asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(m.cnt2 + slot), "r"(2 * G::NCB) : "memory");
+                asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(m.cnt3 + slot), "r"(G::NCB * kWarps) : "memory");
+                atomicAdd(m.stat + 1, 1);                                   // statistic for the next iteration's form
+            }
             continue;
         }
         for (int blk = 0; blk < G::NCB; ++blk) mega_pass2<N, U16, P2_REDO>(m, blk, wave, sm, s_tw, s_red, df, slot, slot + 1);
@@ -377,7 +390,7 @@ template <int N, bool U16> __device__ __forceinline__ void mega_pass2b(const Meg
 
 // ---- pass 3: a6 inverse row FFTs, a7 exit-wave update, a8 object scatter-add ---------------------
 template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
-                                                            Deferred& df) {
+                                                            Deferred& df, bool split) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T;
     const FrameArgs& a = m.f;
@@ -386,6 +399,13 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
     const int y = blk * G::LPB + l;
     const size_t off = (size_t)y * N;
     const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
+    if (split && SYNC) {
+        // One look at the whole wave first: if pass 2b has already marked every frame "inside its bound, nothing to do" (the steady
+        // state), the item ends here -- one L2 round trip instead of one hand-off per slot and a staging of probe rows nobody uses.
+        bool all_done = true;
+        for (int k = threadIdx.x & 31; k < s_end - s_begin; k += 32) all_done = all_done && ld_relaxed_gpu(m.cnt2 + s_begin + k) >= 2 * G::NCB;
+        if (__all_sync(0xffffffffu, all_done)) return;
+    }
     float2* sP = reinterpret_cast<float2*>(const_cast<float4*>(s_tw) + 2 * N) + l * N;                                      // this line's probe row, kept for the M slots
 #pragma unroll
     for (int i = 0; i < E; ++i) sP[t + T * i] = __ldg(a.P + off + t + T * i);
@@ -395,6 +415,11 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
         pc.start(2);
         const YX p0 = m.spos[slot];                                         // (independent of the hand-off: in flight during the poll)
         if (SYNC) warp_wait(m.cnt2 + slot, G::NCB);
+        if (split) {                                                        // split form: pass 2b marks a frame inside its bound with 2 NCB:
+            int done = 0;                                                   // psi' = P O_j is already in the store (pass 1), the ring slot released
+            if ((threadIdx.x & 31) == 0) done = ld_relaxed_gpu(m.cnt2 + slot) >= 2 * G::NCB;
+            if (__shfl_sync(0xffffffffu, done, 0)) continue;
+        }
         pc.lap(0);
         const size_t obase = (size_t)(p0.y + y) * a.W + p0.x;
         float2 o[E];                                                        // O_j (natural order), needed by both branches: issued before
@@ -402,7 +427,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
         for (int i = 0; i < E; ++i) o[i] = __ldg(a.O + obase + t + T * i);
         const float keep = frame_keep<N>(a, slot);                          // 1 - rb  (R6)
         float2* prow = a.psi + (size_t)slot * N * N + off;
-        if (m.corr && blk == 0 && threadIdx.x == 0 && keep == 0.f) atomicAdd(m.stat + 1, 1);   // statistic for the next iteration's form
+        if (m.corr && !split && blk == 0 && threadIdx.x == 0 && keep == 0.f) atomicAdd(m.stat + 1, 1);   // statistic for the next iteration's form
         if (m.corr && keep == 0.f) {
             // The frame's error is inside the power bound (R6: rb = 1): the relaxed projection is the identity, psi' = P O_j, and the
             // frame adds nothing to the object correction (dm_det.cuh k_dm_blend_gather).  S[slot] is not read, nothing is transformed.
@@ -484,8 +509,8 @@ template <int N, bool U16> __global__ void __launch_bounds__(kThreads, (N >= 512
         const int wave = qw - lag * m.D;
         if (wave < 0 || wave >= m.nW) continue;
         df_cta = kind == 1 || kind == 2;
-        if (kind == 3) mega_pass1<N>(m, blk, wave, sm, s_tw, df);
-        else if (kind == 0) mega_pass3<N>(m, blk, wave, sm, s_tw, df);
+        if (kind == 3) mega_pass1<N>(m, blk, wave, sm, s_tw, df, split);
+        else if (kind == 0) mega_pass3<N>(m, blk, wave, sm, s_tw, df, split);
         else if (!split) mega_pass2<N, U16, P2_FUSED>(m, blk, wave, sm, s_tw, s_red, df);
         else if (kind == 2) mega_pass2<N, U16, P2_ERR_ONLY>(m, blk, wave, sm, s_tw, s_red, df);
         else mega_pass2b<N, U16>(m, wave, sm, s_tw, s_red, df);

@@ -19,7 +19,8 @@ _CSRC = os.path.join(_HERE, "csrc")
 # Development only: PTYCHO_BUILD_ONLY_N=256 compiles one frame size into a separate file (a quarter of the build time);
 # the product library always holds all four sizes.
 _ONLY_N = os.environ.get("PTYCHO_BUILD_ONLY_N")
-LIB_PATH = os.environ.get("PTYCHO_B200_LIB") or os.path.join(_CSRC, f"libptycho_dev{_ONLY_N}.so" if _ONLY_N else "libptycho_b200.so")
+_TAG = os.environ.get("PTYCHO_BUILD_TAG", "")   # distinguishes development builds made with different PTYCHO_BUILD_DEFS
+LIB_PATH = os.environ.get("PTYCHO_B200_LIB") or os.path.join(_CSRC, f"libptycho_dev{_ONLY_N}{_TAG}.so" if _ONLY_N else "libptycho_b200.so")
 ALG = {"EPIE_MB": 0, "DM": 1, "LSQML": 2, "LSQML_PF": 3}
 KCLASS = ["rows_fwd", "cols", "rows_inv", "update", "other", "mega"]   # ptycho_kclass
 STATUS = ["OK", "EINVAL", "EBOUNDS", "EUNSUPPORTED", "ENOMEM", "ECUDA", "ESTATE"]

@@ -92,9 +92,18 @@ __device__ __forceinline__ void warp_signal_relaxed(int* cnt) {
     __syncwarp();
     if ((threadIdx.x & 31) == 0) asm volatile("red.relaxed.gpu.global.add.s32 [%0], 1;" ::"l"(cnt) : "memory");
 }
+// -DPTYCHO_STRICT_SYNC builds the formally clean variant: the poll is an acquire (ptxas adds CCTL.IVALL: slower, see above).  In
+// deterministic mode both variants must give bit-identical results (tests/test_gpu_parity.py::test_strict_sync_build_is_bit_identical).
+__device__ __forceinline__ int ld_poll_gpu(const int* p) {
+#ifdef PTYCHO_STRICT_SYNC
+    return ld_acquire_gpu(p);
+#else
+    return ld_relaxed_gpu(p);
+#endif
+}
 __device__ __forceinline__ void warp_wait(const int* cnt, int target) {
     if ((threadIdx.x & 31) == 0) {
-        while (ld_relaxed_gpu(cnt) < target) __nanosleep(64);
+        while (ld_poll_gpu(cnt) < target) __nanosleep(64);
     }
     __syncwarp();
 }

@@ -689,3 +689,31 @@ def test_split_form_under_queue_geometries(B, oracle_mod, monkeypatch):
         assert rel(g.fetch_exit_waves(), o.psi) < 10 * TOL_ITER, (M, D, X)
         assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
         g.destroy()
+
+
+def test_strict_sync_build_is_bit_identical(tmp_path):
+    """The megakernel's hand-off polls with relaxed loads (DESIGN.md section 5.2 says what that assumes).  A build with
+    -DPTYCHO_STRICT_SYNC polls with ld.acquire.gpu instead; in deterministic mode the two builds must agree bit for bit over a
+    multi-iteration run with ring wrap-around -- a reordering the relaxed protocol allowed would show up as a difference."""
+    import hashlib, os, subprocess, sys
+    script = tmp_path / "run.py"
+    script.write_text('''
+import hashlib, sys, numpy as np
+sys.path.insert(0, %r)
+from paper_2202_03144_b200 import binding, synth
+binding.build()
+s = synth.make_custom(64, 260, 9, 21, k=1, peak=2e4, dtype=np.uint16, jitter=3, seed=77, probe_kind="zone")
+g = binding.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, binding.default_params(pbound=0.3, deterministic=1))
+g.iterate("DM", 25)
+h = hashlib.sha1()
+for a in (g.fetch_object(), g.fetch_probe(), g.fetch_exit_waves(), g.fetch_error()):
+    h.update(np.ascontiguousarray(a).tobytes())
+print("HASH", h.hexdigest())
+''' % os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    out = {}
+    for tag, defs in (("relaxed", ""), ("strict", "-DPTYCHO_STRICT_SYNC")):
+        env = dict(os.environ, PTYCHO_BUILD_ONLY_N="64", PTYCHO_BUILD_TAG=tag, PTYCHO_BUILD_DEFS=defs, PTYCHO_MEGA_M="2", PTYCHO_MEGA_D="2", PTYCHO_MEGA_X="1")
+        r = subprocess.run([sys.executable, str(script)], env=env, capture_output=True, text=True, timeout=900)
+        assert r.returncode == 0, r.stderr[-2000:]
+        out[tag] = [l for l in r.stdout.splitlines() if l.startswith("HASH")][0]
+    assert out["relaxed"] == out["strict"]

@@ -380,6 +380,77 @@ def ours_line(args) -> dict | None:
     return line if rank == 0 else None
 
 
+def sharded_line(args) -> dict | None:
+    """--sharded: ONE scan of the config split over the N ranks: strong scaling.  Not the
+    driver's mode (B:ns asks for replicas); kept so that the sharded path can be timed the same way.  Timed region = `steps` DM
+    iterations, each ptycho_shard_begin + neighbour exchange of the correction canvas + all-reduce of the probe sums +
+    ptycho_shard_end, CUDA events, max over ranks."""
+    import torch
+    import torch.distributed as dist
+    rank, local, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the projection cycle has no CPU path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    else:
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % (29500 + os.getpid() % 2000), rank=0, world_size=1, device_id=dev)
+    from paper_2202_03144_b200 import binding, sharded, synth
+    binding.lib()
+    cfg = args.config
+    if DEFAULT_ALG[cfg] != "DM" or (args.alg or "DM") != "DM":
+        raise SystemExit("bench.py --sharded: DM configurations only (2, 4, or 1 with --alg DM is not sharded)")
+    steps, warmup = max(1, args.steps), max(3, args.warmup)
+    s = synth.make_config(cfg, n_pos=args.n_pos, replica=0, threads=max(2, (os.cpu_count() or 8) // world))   # the same scan on every rank
+    par = scan_params(s, "DM")
+    plan = sharded.shard_plan(s.pos, s.n, s.obj0.shape[0], s.obj0.shape[1], world)
+    mine = plan.frames[rank]
+    inten_d = torch.from_numpy(np.ascontiguousarray(s.intensities[mine])).to(dev)
+    comm = sharded.DistComm()
+    g = sharded.ShardedPtycho(plan, rank, torch.from_numpy(s.obj0.astype(np.complex64)).to(dev), torch.from_numpy(s.probe0.astype(np.complex64)).to(dev),
+                              s.pos, inten_d, comm=comm, device=dev, **par)
+    stream = torch.cuda.current_stream(dev)
+    g.iterate(warmup)
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(dev)
+    barrier(world)
+    l0 = g.core.launch_count()
+    t0 = time.perf_counter()
+    e0.record(stream)
+    g.iterate(steps)
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    t1 = time.perf_counter()
+    barrier(world)
+    ms = max_over_ranks(float(e0.elapsed_time(e1)), world, dev)
+    launches = g.core.launch_count() - l0
+    sampler.stop()
+    err = g.fetch_error()
+    assert np.all(np.isfinite(err))
+    halo_rows = sum(hi - lo for _, lo, hi in plan.exchange[rank])
+    g.destroy()
+    dist.destroy_process_group()
+    J = s.n_pos
+    alg_bytes = algorithmic_bytes_per_pattern(s.n, 1, s.intensities.dtype.itemsize)
+    hbm_peak, peak_src = measured_peaks()
+    achieved = alg_bytes * J * steps / (ms * 1e-3) / 1e9
+    line = {"metric": METRIC, "value": J * steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+            "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, "DM", s, J), "parallelism": f"one scan sharded over {world} GPU(s): row bands, per iteration "
+                       "a neighbour exchange of the correction canvas on shared rows and an all-reduce of the probe sums",
+                       "halo_bytes_sent_per_step_rank0": int(halo_rows * s.obj0.shape[1] * 8), "frames_rank0": int(len(mine)),
+                       "timed_iterations": f"{warmup}..{warmup + steps - 1}"},
+            "clocks": sampler.summary(t0, t1), "e2e": None, "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak * world, "unit": "GB/s", "frac": achieved / (hbm_peak * world),
+                         "peak_source": peak_src + f" x {world}", "algorithmic_bytes_per_pattern": alg_bytes, "traffic": None,
+                         "kernel": "whole step (k_dm_mega + exchange + updates), all ranks"},
+            "error_first_last": [float(err[0]), float(err[-1])]}
+    return line if rank == 0 else None
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -391,6 +462,7 @@ def main():
     ap.add_argument("--cufft-ref", action="store_true", help="print the torch.fft reference point instead (harness-side)")
     ap.add_argument("--n-pos", type=int, default=None, help="truncate the scan (debugging only; invalidates the metric)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sharded", action="store_true", help="split ONE scan over the ranks instead of running replicas (SURVEY 8(f) f4)")
     args = ap.parse_args()
     rank, _, world = dist_env()
     if args.cufft_ref:
@@ -401,7 +473,7 @@ def main():
         if rank == 0:
             print(json.dumps(reference_line(args)), flush=True)
         return
-    line = ours_line(args)
+    line = sharded_line(args) if args.sharded else ours_line(args)
     if line is not None:
         print(json.dumps(line), flush=True)
 

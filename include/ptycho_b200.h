@@ -90,6 +90,13 @@ typedef struct {
     const int32_t *batch_order; /* HOST pointer or NULL.  NULL: strided batches, n_b = ceil(J/B),
                            batch b = { j : j mod n_b = b } (R8).  Else a permutation of 0..J-1;
                            batch b = its entries [b*B, (b+1)*B).  Copied at init.                  */
+    /* One scan over several GPUs.  shard_total_pos > 0 makes the context a SHARD:
+       it holds n_pos of the scan's shard_total_pos frames and is driven by ptycho_shard_begin / ptycho_shard_end below.     */
+    int shard_total_pos;        /* 0 = an ordinary context.  Else J of the WHOLE scan (eps_P = delta J max|O|^2, R5)          */
+    int n_foreign;              /* number of entries of foreign_pos                                                          */
+    const int32_t *foreign_pos; /* HOST pointer or NULL: (y, x) of the frames held by OTHER shards that overlap the object rows
+                                   this shard's frames cover.  They enter d_O = sum_j |P(q - r_j)|^2 only (which needs the probe
+                                   and the positions, not the frames' data).  Copied at init.                                */
 } ptycho_params;
 
 void ptycho_default_params(ptycho_params *p);
@@ -190,6 +197,34 @@ typedef enum {
 } ptycho_kclass;
 ptycho_status ptycho_profile(ptycho_ctx *ctx, int enable);
 ptycho_status ptycho_profile_fetch(ptycho_ctx *ctx, int kclass, double *total_ms, long long *n_launches);
+
+/* ---- one scan over several GPUs: the exchange step ("the overlapping size where the data is
+ * shared between multiple GPUs", "the job could also run on multiple GPUs") ----
+ * Reading R27: the frames are partitioned over the GPUs; every GPU holds the exit waves and intensities of its own frames (all
+ * the bulk bytes) and a full-size object array of which it only ever touches the rows its frames cover.  Per DM iteration the
+ * overlap sums are taken over ALL frames before the divisions, so the result is the single-GPU result up to summation order
+ * (the paper's "share-frequency" > 1, an approximation it does not define, is not built).  What crosses GPUs per iteration: the
+ * object correction canvas c on the rows two shards both cover (neighbour exchange), the probe sums n_P, d_P (3 N^2 floats,
+ * all-reduce), and once the intensity sum.  The library does no communication: between the two calls below the CALLER adds the
+ * other shards' values into the buffers ptycho_shard_buffers names (the Python package does it with torch.distributed over NCCL:
+ * paper_2202_03144_b200/sharded.py).
+ *   ptycho_shard_begin: one DM iteration up to the exchange (a1-a9 of this shard's frames: the megakernel).  Afterwards
+ *       c_canvas holds this shard's part of c(q) = sum_j keep_j conj(P(q - r_j)) v_j(q - r_j) and probe_sums its part of n_P, d_P.
+ *   ptycho_shard_end: a10 with the summed buffers: O += c / (d_O + eps_O) with d_O over own AND foreign positions, the probe
+ *       blend, the error term of this shard's frames divided by *sum_I (so the scan's E_t is the sum of the shards' values).
+ * Only for contexts made with shard_total_pos > 0; those refuse ptycho_iterate.  Single-mode DM, atomic-scatter mode, all frames
+ * given at init (PTYCHO_EUNSUPPORTED otherwise at init).  PTYCHO_ESTATE when the two calls do not alternate. */
+typedef struct {
+    float *c_canvas;    /* device, obj_h * obj_w complex64, row-major: rows [row0, row1) can be non-zero                      */
+    float *probe_sums;  /* device, 3 * n * n floats: n_P (n*n complex64) followed by d_P (n*n floats)                       */
+    double *sum_I;      /* device, one double: sum of this shard's unmasked intensities; to be replaced by the scan's total
+                           once, before the first ptycho_shard_begin                                                       */
+    double *err_hist;   /* device: E_t of the iterations run so far (this shard's share once sum_I is the total)            */
+    int row0, row1;     /* object rows covered by this shard's frames                                                       */
+} ptycho_shard_bufs;
+ptycho_status ptycho_shard_buffers(ptycho_ctx *ctx, ptycho_shard_bufs *out);
+ptycho_status ptycho_shard_begin(ptycho_ctx *ctx);
+ptycho_status ptycho_shard_end(ptycho_ctx *ctx);
 
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 long long ptycho_launch_count(const ptycho_ctx *ctx);

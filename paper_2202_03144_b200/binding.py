@@ -40,7 +40,14 @@ class Params(C.Structure):
                 ("delta_obj", C.c_float), ("delta_probe", C.c_float), ("alpha_obj", C.c_float),
                 ("alpha_probe", C.c_float), ("lsq_lambda", C.c_float), ("pbound", C.c_float),
                 ("disable_dm", C.c_int), ("deterministic", C.c_int), ("dm_sweeps", C.c_int),
-                ("batch_order", C.POINTER(C.c_int32))]
+                ("batch_order", C.POINTER(C.c_int32)), ("shard_total_pos", C.c_int), ("n_foreign", C.c_int),
+                ("foreign_pos", C.POINTER(C.c_int32))]
+
+
+class ShardBufs(C.Structure):
+    """ptycho_shard_bufs (include/ptycho_b200.h)."""
+    _fields_ = [("c_canvas", C.c_void_p), ("probe_sums", C.c_void_p), ("sum_I", C.c_void_p), ("err_hist", C.c_void_p),
+                ("row0", C.c_int), ("row1", C.c_int)]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -90,6 +97,9 @@ def lib():
         l.ptycho_wait_frames.argtypes = [C.c_void_p]
         l.ptycho_orthogonalize_modes.argtypes = [C.c_void_p]
         l.ptycho_frames_present.argtypes = [C.c_void_p]
+        l.ptycho_shard_buffers.argtypes = [C.c_void_p, C.POINTER(ShardBufs)]
+        l.ptycho_shard_begin.argtypes = [C.c_void_p]
+        l.ptycho_shard_end.argtypes = [C.c_void_p]
         l.ptycho_default_params.argtypes = [C.POINTER(Params)]
         l.ptycho_test_fft2.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
         l.ptycho_prepare_frames.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float,
@@ -107,6 +117,11 @@ def default_params(**over) -> Params:
             if v is not None:
                 keep = np.ascontiguousarray(v, np.int32)
                 p.batch_order = keep.ctypes.data_as(C.POINTER(C.c_int32))
+        elif k == "foreign_pos":
+            if v is not None and len(v):
+                p._keep_foreign = np.ascontiguousarray(v, np.int32).reshape(-1, 2)
+                p.foreign_pos = p._keep_foreign.ctypes.data_as(C.POINTER(C.c_int32))
+                p.n_foreign = p._keep_foreign.shape[0]
         else:
             if not hasattr(p, k):
                 raise KeyError(k)
@@ -180,6 +195,28 @@ class Ptycho:
 
     def orthogonalize_modes(self):
         self._check(self._l.ptycho_orthogonalize_modes(self._h))
+
+    def shard_buffers(self) -> dict:
+        """ptycho_shard_buffers as torch views of the workspace: c_canvas (H, W, 2) float32 (re, im), probe_sums (3 n^2,) float32,
+        sum_I (1,) float64, err_hist float64, and the covered rows (row0, row1)."""
+        b = ShardBufs()
+        self._check(self._l.ptycho_shard_buffers(self._h, C.byref(b)))
+        base, torch = self.workspace.data_ptr(), self._torch
+
+        def view(ptr, nbytes, dtype):
+            off = ptr - base
+            assert 0 <= off and off + nbytes <= self.workspace.numel()
+            return self.workspace[off:off + nbytes].view(dtype)
+        return {"c_canvas": view(b.c_canvas, self.H * self.W * 8, torch.float32).view(self.H, self.W, 2),
+                "probe_sums": view(b.probe_sums, 3 * self.n * self.n * 4, torch.float32),
+                "sum_I": view(b.sum_I, 8, torch.float64), "err_hist": view(b.err_hist, 8 * 65536, torch.float64),
+                "row0": b.row0, "row1": b.row1}
+
+    def shard_begin(self):
+        self._check(self._l.ptycho_shard_begin(self._h))
+
+    def shard_end(self):
+        self._check(self._l.ptycho_shard_end(self._h))
 
     def wait_frames(self):
         self._check(self._l.ptycho_wait_frames(self._h))

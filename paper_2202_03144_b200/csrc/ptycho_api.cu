@@ -88,6 +88,10 @@ struct ptycho_ctx {
     std::vector<int> batch_order_h, mb_h;
     long long n_steps = 0;
     bool psi_valid = false;
+    // shard of a scan held by several GPUs (ptycho_shard_begin / _end): positions of the other shards' frames over our rows
+    std::vector<int32_t> foreign_h;
+    bool shard_open = false;                   // between ptycho_shard_begin and ptycho_shard_end
+    int shard_row0 = 0, shard_row1 = 0;
     long long launches = 0;
     std::string err;
     // per-kernel-class CUDA-event timing (ptycho_profile): (class, start, stop) of every launch
@@ -255,7 +259,7 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
         c->det_tx = (c->W + kDetTileW - 1) / kDetTileW; c->det_ty = (c->H + kDetTileH - 1) / kDetTileH;
         c->tile_start = w.take<int>((size_t)c->det_tx * c->det_ty + 1);
         c->tile_mid = w.take<int>((size_t)c->det_tx * c->det_ty);
-        c->tile_list = w.take<int>((size_t)c->J * (c->N / kDetTileW + 1) * (c->N / kDetTileH + 1));   // upper bound
+        c->tile_list = w.take<int>((size_t)(c->J + c->par.n_foreign) * (c->N / kDetTileW + 1) * (c->N / kDetTileH + 1));   // upper bound
         if (c->par.deterministic || c->par.dm_sweeps > 0) c->det_partial = w.take<float4>((size_t)kDetGroups * nn);
         if (c->par.dm_sweeps > 0) c->tile_slots = w.take<int>((size_t)c->J * (c->N / kDetTileW + 1) * (c->N / kDetTileH + 1));
     }
@@ -401,7 +405,9 @@ ptycho_status build_batches(ptycho_ctx* c, int np) {
     return PTYCHO_OK;
 }
 
-ptycho_status dm_iteration(ptycho_ctx* c) {
+// phase: 1 = up to the overlap sums (a1-a9), 2 = the normalising updates (a10), 3 = both.  A shard of a multi-GPU scan runs the
+// two halves separately (ptycho_shard_begin / _end) so that the caller can add the other shards' sums in between.
+ptycho_status dm_iteration(ptycho_ctx* c, int phase = 3) {
     const size_t nn = (size_t)c->N * c->N, knn = nn * c->K, HW = (size_t)c->H * c->W;
     const int ncb = ncb_of(c->N);
     // R4: psi_j = P O_j before the first DM iteration.  The plain megakernel forms it on the fly in pass 1 (saves a
@@ -413,6 +419,7 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         LAUNCH(c, PTYCHO_K_OTHER, (k_init_psi<<<g, 256, 0, c->stream>>>(c->psi, c->O, c->W, c->P, c->K, c->N, c->pos, c->dm_frames)));
     }
     const int upd = c->t >= c->par.probe_start;
+    if (!(phase & 1)) goto updates;
     if (c->mega_M > 0) {
         MegaArgs m{};
         m.f = base_args(c);
@@ -462,6 +469,9 @@ ptycho_status dm_iteration(ptycho_ctx* c) {
         a.e_part = c->e_part + (size_t)s0 * ncb;
         passes(c, a, nf, RF_DM, CM_FULL, RI_DM);
     }
+    c->psi_valid = true;                                    // (a failed launch returns above)
+    if (!(phase & 2)) { CU(cudaGetLastError()); return PTYCHO_OK; }
+updates:
     if (c->par.deterministic)                               // object sums from the new psi, fixed order
         LAUNCH(c, PTYCHO_K_OTHER, (k_det_object<<<dim3(c->det_tx, c->det_ty), dim3(kDetTileW, kDetTileH), 0, c->stream>>>(
                                        c->nO, c->dO, c->H, c->W, c->psi, c->P, c->N, c->spos, c->tile_start, c->tile_list)));
@@ -621,6 +631,15 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     if (par.dm_sweeps < 0) return PTYCHO_EINVAL;
     if (par.dm_sweeps > 0 && (n_modes != 1 || par.disable_dm || par.deterministic)) return PTYCHO_EUNSUPPORTED;
     if (cols_smem(n, n_modes) > 227 * 1024) return PTYCHO_EUNSUPPORTED;
+    const bool shard = par.shard_total_pos > 0;
+    if (par.shard_total_pos < 0 || par.n_foreign < 0 || (par.n_foreign > 0 && !par.foreign_pos)) return PTYCHO_EINVAL;
+    if (!shard && par.n_foreign > 0) return PTYCHO_EINVAL;
+    if (shard && par.shard_total_pos < n_pos + par.n_foreign) return PTYCHO_EINVAL;
+    if (shard && (n_modes != 1 || par.disable_dm || par.deterministic || par.dm_sweeps > 0 || !intensities)) return PTYCHO_EUNSUPPORTED;
+    for (int j = 0; j < par.n_foreign; ++j) {
+        const int y = par.foreign_pos[2 * j], x = par.foreign_pos[2 * j + 1];
+        if (y < 0 || x < 0 || y + n > obj_h || x + n > obj_w) return PTYCHO_EBOUNDS;
+    }
 
     // positions: copy, check bounds (R10), accept host or device memory
     std::vector<int32_t> pos(2 * (size_t)n_pos);
@@ -694,6 +713,14 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     c->pos_h = pos;
     if (par.batch_order) c->batch_order_h.assign(par.batch_order, par.batch_order + n_pos);
     c->par.batch_order = nullptr;   // copied; the caller's pointer is not kept
+    if (par.n_foreign > 0) c->foreign_h.assign(par.foreign_pos, par.foreign_pos + 2 * (size_t)par.n_foreign);
+    c->par.foreign_pos = nullptr;
+    if (shard) {
+        if (!c->p2) { g_init_error = "a shard needs the DM megakernel path"; delete c; return PTYCHO_EUNSUPPORTED; }
+        int r0 = obj_h, r1 = 0;
+        for (int j = 0; j < n_pos; ++j) { r0 = std::min(r0, pos[2 * j]); r1 = std::max(r1, pos[2 * j] + n); }
+        c->shard_row0 = r0; c->shard_row1 = r1;
+    }
     CUI(cudaMemcpyAsync(c->dm_frames, c->dm_order.data(), n_pos * 4, cudaMemcpyHostToDevice, s));
     std::vector<int32_t> spos(2 * (size_t)n_pos);
     for (int sidx = 0; sidx < n_pos; ++sidx) { spos[2 * sidx] = pos[2 * c->dm_order[sidx]]; spos[2 * sidx + 1] = pos[2 * c->dm_order[sidx] + 1]; }
@@ -718,8 +745,11 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
                 for (size_t i = 0; i < ntiles; ++i) { fill_b[i] = start[i] + mid[i]; mid[i] = fill_b[i]; }
                 if (want_slots) fill_s.assign(start.begin(), start.end() - 1);
             }
-            for (int sidx = 0; sidx < n_pos; ++sidx) {
-                const int y = spos[2 * sidx], x = spos[2 * sidx + 1];
+            // a shard also lists the other shards' frames over its rows (they enter d_O only): entries n_pos .. n_pos + n_foreign - 1
+            const int n_list = n_pos + (gather ? par.n_foreign : 0);
+            for (int sidx = 0; sidx < n_list; ++sidx) {
+                const int y = sidx < n_pos ? spos[2 * sidx] : c->foreign_h[2 * (size_t)(sidx - n_pos)];
+                const int x = sidx < n_pos ? spos[2 * sidx + 1] : c->foreign_h[2 * (size_t)(sidx - n_pos) + 1];
                 for (int ty = y / kDetTileH; ty <= (y + n - 1) / kDetTileH; ++ty)
                     for (int tx = x / kDetTileW; tx <= (x + n - 1) / kDetTileW; ++tx) {
                         const size_t tl = (size_t)ty * c->det_tx + tx;
@@ -733,6 +763,11 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
             }
             if (pass == 0) { for (size_t i = 0; i < ntiles; ++i) start[i + 1] += start[i]; list.resize(start[ntiles]); if (want_slots) slots.resize(start[ntiles]); }
         }
+        if (shard)                                          // one summation order of d_O on every shard that covers a tile: by position
+            for (size_t i = 0; i < ntiles; ++i) {
+                std::sort(list.begin() + start[i], list.begin() + mid[i]);
+                std::sort(list.begin() + mid[i], list.begin() + start[i + 1]);
+            }
         if (want_slots) CUI(cudaMemcpyAsync(c->tile_slots, slots.data(), slots.size() * 4, cudaMemcpyHostToDevice, s));
         CUI(cudaMemcpyAsync(c->tile_start, start.data(), start.size() * 4, cudaMemcpyHostToDevice, s));
         CUI(cudaMemcpyAsync(c->tile_mid, mid.data(), mid.size() * 4, cudaMemcpyHostToDevice, s));
@@ -751,7 +786,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     k_probe_max<<<64, 256, 0, s>>>(c->P, c->K, (int)nn, c->sc);   // sc was zeroed above
     k_finish_init<<<1, 1, 0, s>>>(c->sc, par.delta_blend, n_pos, 0);
     k_abs2_max<<<ew_blocks(HW), 256, 0, s>>>(c->O, HW, c->sc);
-    k_finish_init<<<1, 1, 0, s>>>(c->sc, par.delta_blend, n_pos, 1);
+    k_finish_init<<<1, 1, 0, s>>>(c->sc, par.delta_blend, shard ? par.shard_total_pos : n_pos, 1);
     if (!c->streaming) {
         k_sum_intensity<<<kRedBlocks, 256, 0, s>>>(c->I, itype, (size_t)n_pos * nn, c->scratch_d);
         k_finish_sum_I<<<1, 32, 0, s>>>(c->scratch_d, kRedBlocks, c->sc, 0);
@@ -771,6 +806,7 @@ ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
     if (alg != PTYCHO_EPIE_MB && alg != PTYCHO_DM && alg != PTYCHO_LSQML && alg != PTYCHO_LSQML_PF) return fail(c, PTYCHO_EINVAL, "unknown algorithm");
     if (alg != PTYCHO_DM && c->par.deterministic) return fail(c, PTYCHO_EUNSUPPORTED, "deterministic mode covers DM only");
     if (alg == PTYCHO_DM && !c->psi) return fail(c, PTYCHO_ESTATE, "DM needs the exit-wave store (disable_dm was set)");
+    if (c->par.shard_total_pos > 0) return fail(c, PTYCHO_ESTATE, "a shard is driven by ptycho_shard_begin / ptycho_shard_end");
     if (c->streaming) {
         if (c->present == 0) return fail(c, PTYCHO_ESTATE, "no frame has been appended yet");
         if (alg == PTYCHO_DM && c->present < c->J) return fail(c, PTYCHO_ESTATE, "DM needs every frame (PAPER.md:58); append the rest first");
@@ -786,6 +822,41 @@ ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
         LAUNCH(c, PTYCHO_K_UPDATE, (k_sum_error<<<kErrBlocks, 1024, 0, c->stream>>>(c->e_part, (size_t)c->J * ncb_of(c->N), c->sc, slot, c->err_part, c->err_ticket)));
         ++c->t;
     }
+    CU(cudaGetLastError());
+    return PTYCHO_OK;
+}
+
+ptycho_status ptycho_shard_buffers(ptycho_ctx* c, ptycho_shard_bufs* out) {
+    if (!c || !out) return PTYCHO_EINVAL;
+    if (c->par.shard_total_pos <= 0) return fail(c, PTYCHO_ESTATE, "not a shard (params.shard_total_pos)");
+    out->c_canvas = reinterpret_cast<float*>(c->nO);
+    out->probe_sums = reinterpret_cast<float*>(c->nP);     // n_P (N^2 complex64) and d_P (N^2 floats) are adjacent for K = 1 (layout)
+    if (reinterpret_cast<char*>(c->dP) != reinterpret_cast<char*>(c->nP) + (size_t)c->N * c->N * 8) return fail(c, PTYCHO_ESTATE, "probe sums not adjacent");
+    out->sum_I = &c->sc->sum_I;
+    out->err_hist = c->err_hist;
+    out->row0 = c->shard_row0; out->row1 = c->shard_row1;
+    return PTYCHO_OK;
+}
+ptycho_status ptycho_shard_begin(ptycho_ctx* c) {
+    if (!c) return PTYCHO_EINVAL;
+    if (c->par.shard_total_pos <= 0) return fail(c, PTYCHO_ESTATE, "not a shard (params.shard_total_pos)");
+    if (c->shard_open) return fail(c, PTYCHO_ESTATE, "ptycho_shard_end has not been called");
+    k_snap_sum_I<<<1, 1, 0, c->stream>>>(c->sc);
+    ++c->launches;
+    ptycho_status st = dm_iteration(c, 1);
+    if (st != PTYCHO_OK) return st;
+    c->shard_open = true;
+    return PTYCHO_OK;
+}
+ptycho_status ptycho_shard_end(ptycho_ctx* c) {
+    if (!c) return PTYCHO_EINVAL;
+    if (!c->shard_open) return fail(c, PTYCHO_ESTATE, "ptycho_shard_begin has not been called");
+    ptycho_status st = dm_iteration(c, 2);
+    if (st != PTYCHO_OK) return st;
+    double* slot = c->err_hist + (c->t < kErrCap ? c->t : kErrCap - 1);
+    LAUNCH(c, PTYCHO_K_UPDATE, (k_sum_error<<<kErrBlocks, 1024, 0, c->stream>>>(c->e_part, (size_t)c->J * ncb_of(c->N), c->sc, slot, c->err_part, c->err_ticket)));
+    ++c->t;
+    c->shard_open = false;
     CU(cudaGetLastError());
     return PTYCHO_OK;
 }

@@ -717,3 +717,73 @@ print("HASH", h.hexdigest())
         assert r.returncode == 0, r.stderr[-2000:]
         out[tag] = [l for l in r.stdout.splitlines() if l.startswith("HASH")][0]
     assert out["relaxed"] == out["strict"]
+
+
+# ------------------------------------------------------------- one scan over several GPUs (reading R27)
+@pytest.mark.parametrize("world,n,h,side,step,jitter,dtype,pbound", [
+    (2, 64, 420, 16, 21, 3, np.uint16, 0.3),       # two bands, frames cross the power bound on the way
+    (3, 64, 420, 16, 21, 3, np.float32, 0.0),      # three bands: the middle one exchanges with both neighbours
+    (5, 128, 400, 9, 30, 2, np.uint16, 0.3),       # thin bands (a band is lower than a frame): every rank overlaps several others
+    (1, 64, 300, 9, 21, 0, np.float32, 0.0)])      # one shard: the two-call form of the plain iteration
+def test_sharded_scan_matches_the_single_device_oracle(B, oracle_mod, world, n, h, side, step, jitter, dtype, pbound):
+    """The frames are split over `world` shards (row bands), every shard is its own C-ABI context holding only its frames, and the
+    overlap sums are completed by the exchange step between ptycho_shard_begin and ptycho_shard_end (sharded.py).  The result has
+    a plain definition -- the single-device iteration over ALL frames -- so the oracle is the ordinary one, which knows nothing of
+    shards.  All shards run in one process on this one GPU, stepped in lockstep (LocalGroup): the same calls, exchange code and
+    order of additions as the distributed run, whose communication layer is covered by the gloo test in test_abi_and_host.py."""
+    from paper_2202_03144_b200 import sharded
+    s = synth.make_custom(n, h, side, step, k=1, peak=2e4 if dtype == np.uint16 else None, dtype=dtype, jitter=jitter, seed=31,
+                          probe_kind="zone")
+    par = dict(pbound=pbound, probe_start=2)
+    plan = sharded.shard_plan(s.pos, n, h, h, world)
+    if world == 5:
+        assert max(len(e) for e in plan.exchange) >= 3      # the thin-band case really has many-way overlaps
+    o = oracle_mod.Oracle(s.obj0, s.probe0, s.pos, s.intensities, par)
+    grp = sharded.LocalGroup(plan, s.obj0, s.probe0, s.pos, s.intensities, **par)
+    lit = well_lit(s)
+    for it in range(12):
+        o.iterate("DM", 1)
+        grp.iterate(1)
+        O = grp.fetch_object()
+        assert rel(O, o.O) < TOL_RUN and rel(O[lit], o.O[lit]) < TOL_RUN, it
+    assert rel(grp.fetch_exit_waves(), o.psi) < TOL_RUN
+    assert rel(grp.fetch_probe(), o.P) < TOL_RUN
+    assert np.allclose(grp.fetch_error(), o.err, rtol=2e-3)
+    # every shard holds the same probe (the sums were completed before the blend), and on rows two shards cover their objects agree
+    P0 = grp.shards[0].core.fetch_probe()
+    objs = [sh.core.fetch_object() for sh in grp.shards]
+    for r, sh in enumerate(grp.shards):
+        assert np.array_equal(sh.core.fetch_probe(), P0)
+        for q, lo, hi in plan.exchange[r]:
+            assert rel(objs[r][lo:hi], objs[q][lo:hi]) < 1e-6
+    # the plain single-context run of the same scan, for scale: the sharded result is as close to the oracle as it is
+    g = make(B, s, **par)
+    g.iterate("DM", 12)
+    assert rel(O, g.fetch_object()) < 1e-4
+    g.destroy()
+    grp.destroy()
+
+
+def test_shard_contexts_refuse_what_they_do_not_support(B):
+    s = synth.make_custom(64, 300, 6, 21, k=1, seed=3)
+    with pytest.raises(B.PtychoError):                      # K > 1
+        s2 = synth.make_custom(64, 300, 6, 21, k=2, seed=3)
+        B.Ptycho(s2.obj0, s2.probe0, s2.pos, s2.intensities, B.default_params(shard_total_pos=len(s2.pos)))
+    with pytest.raises(B.PtychoError):                      # deterministic mode
+        B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(shard_total_pos=len(s.pos), deterministic=1))
+    with pytest.raises(B.PtychoError):                      # fewer frames in the scan than in the shard
+        B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(shard_total_pos=3))
+    g = B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(shard_total_pos=len(s.pos)))
+    with pytest.raises(B.PtychoError):
+        g.iterate("DM", 1)                                  # a shard is driven by begin / end
+    with pytest.raises(B.PtychoError):
+        g.shard_end()                                       # ... which alternate
+    g.shard_begin()
+    with pytest.raises(B.PtychoError):
+        g.shard_begin()
+    g.shard_end()
+    plain = make(B, s)
+    with pytest.raises(B.PtychoError):
+        plain.shard_begin()                                 # and an ordinary context is not a shard
+    plain.destroy()
+    g.destroy()

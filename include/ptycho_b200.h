@@ -265,6 +265,26 @@ ptycho_status ptycho_prepare_frames(const void *raw, ptycho_itype raw_type, int 
 /* Batched 2-D complex64 FFT of `count` n x n frames, in place, on `cuda_stream`. */
 ptycho_status ptycho_test_fft2(float *data, int n, int count, int inverse, void *cuda_stream);
 
+/* ---- an entry point that allocates nothing ----
+ * Some callers cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid it.
+ * ptycho_test_fft2 above gets the scratch of its kernels (the forward and inverse twiddle tables of the line FFT, fft_core.cuh)
+ * from cudaMalloc and fills it from the host.  This variant keeps that scratch in a file-scope device array of the library,
+ * 2 * PTYCHO_NOALLOC_MAX_N complex64 = 8 KB, which every GPU that loads the library holds until the process exits; the tables are
+ * written on the device (fp64 sine / cosine rounded to fp32, like the host's), so the call does no host-to-device copy either.
+ * The same batched in-place 2-D complex64 FFT of `count` n x n frames (n = 64, 128, 256 or 512; the inverse is scaled by 1/n^2;
+ * DC at [0][0]), same kernels, results within the FFT tolerance of ptycho_test_fft2 (2e-6 relative L2; bit-identical whenever the
+ * device's and the host's fp64 sine agree after rounding to fp32).
+ *   data: DEVICE pointer, count * n * n complex64, read and written.  cuda_stream: a cudaStream_t of the CURRENT device.
+ *   ASYNCHRONOUS: the work is queued on the stream and the call returns; it calls no cudaMalloc, cudaFree, or allocating library
+ *   routine, and does not synchronise.
+ *   n > PTYCHO_NOALLOC_MAX_N: PTYCHO_ENOMEM ("exceeds the static scratch"); other invalid arguments: PTYCHO_EINVAL; the message
+ *   is at ptycho_last_error(NULL).
+ *   The scratch is SHARED by all calls on a device and keeps the last call's tables: every call rewrites the part it uses, in
+ *   stream order, before its kernels read it.  Calls that overlap on the GPU (different streams, or several host threads on
+ *   different streams) with DIFFERENT n race on it; serialise them (one stream, or events). */
+#define PTYCHO_NOALLOC_MAX_N 512
+ptycho_status ptycho_fft2_noalloc(float *data, int n, int count, int inverse, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

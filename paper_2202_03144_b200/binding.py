@@ -353,3 +353,19 @@ def test_fft2(data, inverse: bool = False):
     if st != 0:
         raise PtychoError(st, "ptycho_test_fft2")
     return data
+
+
+def fft2_noalloc(data, inverse: bool = False):
+    """ptycho_fft2_noalloc: the same batched in-place 2-D FFT as test_fft2, with the kernels' scratch (the twiddle tables) in a
+    static device array of the library: no cudaMalloc / cudaFree, no host-to-device copy, no synchronisation.  Asynchronous on
+    torch's current stream.  n <= PTYCHO_NOALLOC_MAX_N = 512; calls that overlap on the GPU with different n race on the scratch."""
+    import torch
+    assert data.is_cuda and data.dtype == torch.complex64 and data.is_contiguous()
+    l = lib()
+    l.ptycho_fft2_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
+    with torch.cuda.device(data.device):
+        st = l.ptycho_fft2_noalloc(C.c_void_p(data.data_ptr()), data.shape[-1], int(data.numel() // data.shape[-1] ** 2),
+                                   int(inverse), C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if st != 0:
+        raise PtychoError(st, l.ptycho_last_error(None).decode())
+    return data

@@ -9,6 +9,7 @@
 #include <algorithm>
 #include <cmath>
 #include <complex>
+#include <mutex>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -1188,3 +1189,83 @@ ptycho_status ptycho_test_fft2(float* data, int n, int count, int inverse, void*
 }
 
 }  // extern "C"
+
+// =========================================================================================
+// ptycho_fft2_noalloc: the entry point that allocates nothing (include/ptycho_b200.h)
+// =========================================================================================
+// The scratch of the FFT kernels (forward table, then inverse table) for callers that cannot call cudaMalloc.  In HOST code this
+// name is a stand-in, not a device address: the address is taken once per device with cudaGetSymbolAddress (below), with that
+// device current, and only that pointer is handed to kernels.
+static __device__ __align__(256) float2 g_noalloc_tw[2 * PTYCHO_NOALLOC_MAX_N];
+
+namespace {
+
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+float2* g_noalloc_ptr[kNoAllocMaxDevices] = {};       // device address of g_noalloc_tw, per device ordinal
+unsigned g_noalloc_attrs[kNoAllocMaxDevices] = {};    // per device: bit log2(n) - 6 set once the kernels of size n have their attributes
+
+// The tables of host_twiddles(), written on the device: tw[ka * T + b] = twi[b * E + ka] = exp(-2 pi i b ka / n).
+__global__ void k_fill_twiddles(float2* __restrict__ tw, float2* __restrict__ twi, int n, int E, int T) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int ka = i / T, b = i % T;
+    const double ang = -2.0 * M_PI * (double)b * ka / n;
+    const float2 w = make_float2((float)cos(ang), (float)sin(ang));
+    tw[ka * T + b] = w;
+    twi[b * E + ka] = w;
+}
+
+ptycho_status noalloc_fail(ptycho_status st, const std::string& msg) {
+    g_init_error = "ptycho_fft2_noalloc: " + msg;
+    return st;
+}
+
+}  // namespace
+
+extern "C" ptycho_status ptycho_fft2_noalloc(float* data, int n, int count, int inverse, void* cuda_stream) {
+    if (n > PTYCHO_NOALLOC_MAX_N)
+        return noalloc_fail(PTYCHO_ENOMEM, "n = " + std::to_string(n) + " exceeds the static scratch (PTYCHO_NOALLOC_MAX_N = " + std::to_string(PTYCHO_NOALLOC_MAX_N) + ")");
+    if (!data || count < 1) return noalloc_fail(PTYCHO_EINVAL, "null data or count < 1");
+    if (!valid_n(n)) return noalloc_fail(PTYCHO_EINVAL, "n must be 64, 128, 256 or 512 (and built into this library)");
+    ptycho_ctx tmp;                                        // host-side bookkeeping of the launch helpers only
+    ptycho_ctx* c = &tmp;
+    c->N = n; c->K = 1; c->stream = static_cast<cudaStream_t>(cuda_stream);
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kNoAllocMaxDevices) return noalloc_fail(PTYCHO_ECUDA, "cudaGetDevice failed or device ordinal >= 64");
+    float2* tw = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_noalloc_mu);
+        if (!g_noalloc_ptr[dev]) {                         // once per device, with that device current
+            void* p = nullptr;
+            const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_tw);
+            if (e != cudaSuccess || !p) return noalloc_fail(PTYCHO_ECUDA, std::string("cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+            g_noalloc_ptr[dev] = static_cast<float2*>(p);
+        }
+        tw = g_noalloc_ptr[dev];
+        const unsigned bit = 1u << (n == 64 ? 0 : n == 128 ? 1 : n == 256 ? 2 : 3);
+        if (!(g_noalloc_attrs[dev] & bit)) {               // shared-memory opt-in of the kernels of this size (no allocation)
+            ptycho_status st = PTYCHO_OK;
+            dispatch_n(n, [&](auto nn) { st = set_attrs<decltype(nn)::value>(c); });
+            if (st != PTYCHO_OK) return noalloc_fail(st, c->err);
+            g_noalloc_attrs[dev] |= bit;
+        }
+    }
+    const int E = n == 64 ? 8 : n == 512 ? 32 : 16;
+    float2* twi = tw + PTYCHO_NOALLOC_MAX_N;
+    k_fill_twiddles<<<(n + 255) / 256, 256, 0, c->stream>>>(tw, twi, n, E, n / E);   // the part of the scratch this call uses
+    const size_t nn = (size_t)n * n;
+    for (int f0 = 0; f0 < count; f0 += 32768) {            // frames ride in gridDim.y
+        const int nf = std::min(32768, count - f0);
+        FrameArgs a{};
+        a.S = reinterpret_cast<float2*>(data) + (size_t)f0 * nn; a.K = 1; a.tw = tw; a.twi = twi;
+        if (!inverse) passes(c, a, nf, RF_PLAIN, CM_PLAIN_FWD, -1);
+        else {
+            passes(c, a, nf, -1, CM_PLAIN_INV, RI_PLAIN);
+            k_scale<<<ew_blocks((size_t)nf * nn), 256, 0, c->stream>>>(a.S, (size_t)nf * nn, 1.0f / ((float)n * n));
+        }
+    }
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return noalloc_fail(PTYCHO_ECUDA, cudaGetErrorString(e));
+    return PTYCHO_OK;
+}

@@ -165,11 +165,16 @@ template <class F> void dispatch_n(int n, F&& f) {
 }
 bool valid_n(int n) { return (n == 64 || n == 128 || n == 256 || n == 512) && PTYCHO_HAS_N(n); }
 
-int chunk_frames(int n, int K, int J) {
-    double mb = 64.0;
+// Frames per launch of the three-pass kernels (and per piece of fetch / set).  Measured at config 3 (K = 3, batches of 512 frames):
+// launches small enough for S to stay in L2 (64 MB: 42 frames, 2.3 waves of CTAs) lose more to their tails than they gain from
+// L2 -- 69 ms of kernel time per iteration at 64 MB, 57 at 256 MB, 49 with the whole batch in one launch.  So: a whole minibatch
+// per launch, up to 1 GB of scratch.
+int chunk_frames(int n, int K, int J, int batch) {
+    double mb = 1024.0;
     if (const char* e = getenv("PTYCHO_CHUNK_MB")) mb = atof(e) > 0 ? atof(e) : mb;
     long long per = (long long)K * n * n * 8;
-    long long c = (long long)(mb * 1048576.0) / per;
+    long long c = std::min<long long>((long long)(mb * 1048576.0) / per, 32768);   // (frames ride in gridDim.y)
+    if (batch > 0) c = std::min<long long>(c, batch);
     return (int)std::max<long long>(1, std::min<long long>(c, J));
 }
 
@@ -606,7 +611,7 @@ size_t ptycho_workspace_bytes(int obj_h, int obj_w, int n, int n_modes, int n_po
     ptycho_ctx tmp;
     tmp.H = obj_h; tmp.W = obj_w; tmp.N = n; tmp.K = n_modes; tmp.J = n_pos; tmp.itype = itype;
     if (params) tmp.par = *params; else ptycho_default_params(&tmp.par);
-    tmp.chunk = chunk_frames(n, n_modes, n_pos);
+    tmp.chunk = chunk_frames(n, n_modes, n_pos, tmp.par.batch_size);
     mega_config(&tmp);
     tmp.streaming = intensities_on_host == 2;
     return layout(&tmp, nullptr, intensities_on_host == 1);
@@ -664,7 +669,7 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     c = new ptycho_ctx;
     c->H = obj_h; c->W = obj_w; c->N = n; c->K = n_modes; c->J = n_pos; c->itype = itype; c->par = par;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
-    c->chunk = chunk_frames(n, n_modes, n_pos);
+    c->chunk = chunk_frames(n, n_modes, n_pos, par.batch_size);
     mega_config(c);
     c->streaming = intensities == nullptr;
     const bool dev_I = c->streaming || is_device_ptr(intensities);

@@ -1,0 +1,96 @@
+"""ORACLE (test infrastructure, like the rest of this package): ePIE-minibatch with SUB-PIXEL scan positions.
+
+SURVEY.md 8(f) f4 / R10 ("sub-pixel shifts = NEXT f4").  PAPER.md does not say how ptychopy treats the fractional
+part of a position; reading R28 of DESIGN.md fixes it as the textbook rule -- the Fourier shift theorem applied to
+the PROBE -- and this file is that rule written out in fp64 numpy, step by step.  Frame j sits at r_j + delta_j,
+r_j the integer corner (as everywhere else), delta_j = (dy, dx) in [0, 1)^2:
+
+    S_d[f]   = F^-1[ F[f](k) exp(-2 pi i (k_y d_y + k_x d_x) / N) ],  k = numpy.fft.fftfreq(N) N  (signed; Nyquist = -N/2)
+    P_jk     = S_{delta_j}[P_k]                      the probe as frame j sees it (periodic Fourier interpolation)
+    psi_jk   = P_jk O_j,  Phi = F psi,  Phi' = Pi_M Phi (R2, R3, R6: oracle.modulus_project, the C oracle's routine),
+    chi_jk   = F^-1 Phi' - psi_jk
+    n_O(r_j + r) += sum_k conj(P_jk) chi_jk          d_O(r_j + r) += sum_k |P_jk|^2
+    n_Pk         += S_{-delta_j}[ conj(O_j) chi_jk ]  (the adjoint of the shift brings the term back into the probe's frame)
+    d_P          += |O_j|^2                           (not shifted: a positive normaliser; Fourier interpolation could make it negative)
+    dO = n_O / (d_O + delta_O max_r sum_k |P_k|^2)    (R8; the regulariser from the UNSHIFTED probe)
+    dP_k = n_Pk / (d_P + delta_P max_r d_P),   O += alpha_O dO,   P_k += alpha_P dP_k (if the probe is updated)
+
+With every delta_j = 0 this is orc_minibatch_step(EPIE_MB) of ptycho_oracle.c (pinned so in tests/test_oracle_pins.py, together
+with the shift against its closed form on a Fourier mode, S_d S_{1-d} = a roll by one pixel, the common-shift equivalence with a
+pre-shifted probe, and the back-shift of the probe term).  Library primitives used as steps: numpy.fft, oracle.modulus_project.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import DEFAULTS, batches, modulus_project, to_real_intensity
+
+
+def shift(f: np.ndarray, dy: float, dx: float) -> np.ndarray:
+    """S_(dy,dx)[f] on the last two axes: f moved by +dy rows and +dx columns (periodic Fourier interpolation)."""
+    n = f.shape[-1]
+    k = np.fft.fftfreq(n) * n
+    ramp = np.exp(-2j * np.pi * (k[:, None] * dy + k[None, :] * dx) / n)
+    return np.fft.ifft2(np.fft.fft2(np.asarray(f, np.complex128)) * ramp)
+
+
+def epie_mb_step(O, P, pos, frac, inten, frames, update_probe, par):
+    """One minibatch step over `frames` (in place on O, P; fp64).  Returns the batch's error term sum (sqrt I - A)^2."""
+    K, n = P.shape[0], P.shape[-1]
+    nO = np.zeros_like(O)
+    dO = np.zeros(O.shape)
+    nP = np.zeros_like(P)
+    dP = np.zeros((n, n))
+    err = 0.0
+    for j in frames:
+        y, x = int(pos[j, 0]), int(pos[j, 1])
+        dy, dx = float(frac[j, 0]), float(frac[j, 1])
+        Oj = O[y:y + n, x:x + n]
+        Pj = shift(P, dy, dx)                                            # (K, n, n)
+        psi = Pj * Oj[None]
+        Phi = np.fft.fft2(psi)
+        Phi2, e = modulus_project(Phi, inten[j], par["pbound"])
+        err += e
+        chi = np.fft.ifft2(Phi2) - psi
+        nO[y:y + n, x:x + n] += np.sum(np.conj(Pj) * chi, axis=0)
+        dO[y:y + n, x:x + n] += np.sum(np.abs(Pj) ** 2, axis=0)
+        nP += shift(np.conj(Oj)[None] * chi, -dy, -dx)
+        dP += np.abs(Oj) ** 2
+    maxP = float(np.max(np.sum(np.abs(P) ** 2, axis=0)))
+    dirO = nO / (dO + par["delta_obj"] * maxP)
+    dirP = nP / (dP + par["delta_probe"] * float(np.max(dP)))[None]
+    O += par["alpha_obj"] * dirO
+    if update_probe:
+        P += par["alpha_probe"] * dirP
+    return err
+
+
+class SubpixelOracle:
+    """State and sequencing (batches R8, probe_start, error history C3), mirroring oracle.Oracle for EPIE_MB."""
+
+    def __init__(self, obj, probe, pos, frac, intensities, params=None):
+        self.par = dict(DEFAULTS)
+        self.par.update(params or {})
+        self.O = np.array(obj, np.complex128)
+        self.P = np.array(probe, np.complex128)
+        if self.P.ndim == 2:
+            self.P = self.P[None]
+        self.pos = np.asarray(pos, np.int64).reshape(-1, 2)
+        self.frac = np.asarray(frac, np.float64).reshape(-1, 2)
+        assert self.frac.shape == self.pos.shape and (self.frac >= 0).all() and (self.frac < 1).all()
+        self.inten = intensities                                        # uint16 / float32 as given (masks: R3)
+        it = to_real_intensity(intensities, np.float64)
+        self.sum_I = float(np.sum(it[it >= 0]))
+        self.t = 0
+        self.err: list[float] = []
+
+    def iterate(self, n_iters: int = 1):
+        p = self.par
+        for _ in range(n_iters):
+            upd = self.t >= p["probe_start"]
+            num = 0.0
+            for fr in batches(len(self.pos), p["batch_size"], p["batch_order"]):
+                num += epie_mb_step(self.O, self.P, self.pos, self.frac, self.inten, fr, upd, p)
+            self.err.append(num / (self.sum_I if self.sum_I > 0 else 1.0))
+            self.t += 1
+        return self

@@ -573,3 +573,81 @@ def test_mode_orthogonalisation_pins(oracle_mod):
     q2, psi2 = oracle_mod.orthogonalize_modes(p, psi)
     want = np.stack([q2 * obj[None, y:y + 12, x:x + 12] for y, x in ((0, 0), (3, 5), (8, 8))])
     assert rel(psi2, want) < 1e-12
+
+
+# ------------------------------------------------------------------ sub-pixel positions (reading R28; oracle/subpixel.py)
+def test_subpixel_shift_closed_form_roll_and_adjoint(oracle_mod):
+    from oracle import subpixel
+    n = 16
+    yy, xx = np.mgrid[0:n, 0:n]
+    dy, dx = 0.3, 0.85
+    for ay, ax in [(1, 0), (0, 1), (3, -5), (-7, 2)]:                     # a Fourier mode moved by (dy, dx): the closed form
+        f = np.exp(2j * np.pi * (ay * yy + ax * xx) / n)
+        want = np.exp(2j * np.pi * (ay * (yy - dy) + ax * (xx - dx)) / n)
+        assert np.allclose(subpixel.shift(f, dy, dx), want, atol=1e-12)
+    f = crandn(2, n, n)
+    g = subpixel.shift(subpixel.shift(f, dy, 0.0), 1 - dy, 0.0)           # dy then 1 - dy = one whole row DOWN (+y), columns untouched
+    assert np.allclose(g, np.roll(f, 1, axis=-2), atol=1e-12)
+    g = subpixel.shift(subpixel.shift(f, 0.0, dx), 0.0, 1 - dx)
+    assert np.allclose(g, np.roll(f, 1, axis=-1), atol=1e-12)
+    assert np.allclose(subpixel.shift(f, 0.0, 0.0), f, atol=1e-13)
+    a, b = crandn(n, n), crandn(n, n)                                      # S_{-d} is the adjoint of S_d
+    assert np.isclose(np.vdot(b, subpixel.shift(a, dy, dx)), np.vdot(subpixel.shift(b, -dy, -dx), a), atol=1e-10)
+
+
+@pytest.mark.parametrize("k,dtype,pbound", [(1, np.float32, 0.0), (2, np.uint16, 0.4)])
+def test_subpixel_zero_shift_is_the_ordinary_minibatch_step(oracle_mod, k, dtype, pbound):
+    """delta_j = 0 for every frame: oracle/subpixel.py (numpy) must give what orc_minibatch_step (C) gives -- masks, relaxed
+    projection, several modes, strided batches, probe update from iteration 1 on."""
+    from oracle import subpixel
+    s = synth.make_custom(16, 44, 4, 6, k=k, peak=3e3 if dtype == np.uint16 else None, dtype=dtype, seed=12, jitter=1)
+    inten = s.intensities.copy()
+    inten[3, 2, 5] = 65535 if dtype == np.uint16 else -1.0                 # a masked pixel (R3)
+    par = dict(batch_size=5, probe_start=1, pbound=pbound, alpha_obj=0.9, alpha_probe=0.7)
+    O0 = s.obj0 * (1 + 0.05 * crandn(*s.obj0.shape))
+    o = oracle_mod.Oracle(O0, s.probe0, s.pos, inten, par).iterate("EPIE_MB", 3)
+    q = subpixel.SubpixelOracle(O0, s.probe0, s.pos, np.zeros((len(s.pos), 2)), inten, par).iterate(3)
+    assert rel(q.O, o.O) < 1e-11 and rel(q.P, o.P) < 1e-11
+    assert np.allclose(q.err, o.err, rtol=1e-10)
+
+
+def test_subpixel_common_shift_equals_a_preshifted_probe(oracle_mod):
+    """Every frame shifted by the same delta: the object step must be the ordinary (C oracle) step taken with the probe
+    S_delta[P]; and with a huge regulariser the probe step reduces to alpha n_P / (delta_P max d_P), whose numerators must be
+    related by the BACK-shift S_{-delta} (catches a forward shift, or none, in the probe term)."""
+    from oracle import subpixel
+    s = synth.make_custom(16, 44, 4, 6, k=2, seed=5, jitter=1)
+    d = (0.35, 0.6)
+    frac = np.tile(np.array(d), (len(s.pos), 1))
+    O0 = s.obj0 * (1 + 0.05 * crandn(*s.obj0.shape))
+    Ps = subpixel.shift(s.probe0, *d)
+    big = 1e9
+    par = dict(batch_size=0, probe_start=0, delta_probe=big, alpha_probe=big)
+    o = oracle_mod.Oracle(O0, Ps, s.pos, s.intensities, par).iterate("EPIE_MB", 1)
+    # The object regulariser is delta_O max_r sum_k |P_k|^2: of the UNSHIFTED probe in the sub-pixel step (R28), of the probe it is
+    # given in the ordinary one.  The two runs differ only through that scalar, so it is matched through delta_obj.
+    mo, mq = np.max(np.sum(np.abs(Ps) ** 2, 0)), np.max(np.sum(np.abs(s.probe0) ** 2, 0))
+    par2 = dict(par, delta_obj=mo / mq)
+    q = subpixel.SubpixelOracle(O0, s.probe0, s.pos, frac, s.intensities, par2).iterate(1)
+    assert rel(q.O, o.O) < 1e-11
+    dq, do = q.P - s.probe0, o.P - Ps                                      # alpha n_P / (d_P + delta_P max d_P) -> n_P / max d_P
+    assert rel(dq, subpixel.shift(do, -d[0], -d[1])) < 1e-7
+    assert rel(dq, subpixel.shift(do, d[0], d[1])) > 1e-2 and rel(dq, do) > 1e-2
+    assert np.allclose(q.err, o.err, rtol=1e-10)
+
+
+def test_subpixel_positions_matter_and_the_true_ones_fit_best(oracle_mod):
+    """Data simulated (here, with numpy) from fractional positions: the ground truth is a fixed point of the sub-pixel step with
+    zero error, and it is NOT one when the fractions are dropped."""
+    from oracle import subpixel
+    s = synth.make_custom(16, 44, 4, 6, k=1, seed=9, jitter=1)
+    rng = np.random.default_rng(3)
+    frac = rng.uniform(0, 1, (len(s.pos), 2))
+    n = 16
+    inten = np.empty((len(s.pos), n, n), np.float32)
+    for j, (y, x) in enumerate(s.pos):
+        inten[j] = np.abs(np.fft.fft2(subpixel.shift(s.probe_true, *frac[j])[0] * s.obj_true[y:y + n, x:x + n])) ** 2
+    q = subpixel.SubpixelOracle(s.obj_true, s.probe_true, s.pos, frac, inten, dict(batch_size=4)).iterate(2)
+    assert q.err[0] < 1e-12 and rel(q.O, s.obj_true) < 1e-6 and rel(q.P, s.probe_true) < 1e-6
+    z = subpixel.SubpixelOracle(s.obj_true, s.probe_true, s.pos, 0 * frac, inten, dict(batch_size=4)).iterate(1)
+    assert z.err[0] > 1e-4

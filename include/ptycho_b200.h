@@ -97,6 +97,16 @@ typedef struct {
     const int32_t *foreign_pos; /* HOST pointer or NULL: (y, x) of the frames held by OTHER shards that overlap the object rows
                                    this shard's frames cover.  They enter d_O = sum_j |P(q - r_j)|^2 only (which needs the probe
                                    and the positions, not the frames' data).  Copied at init.                                */
+    /* Sub-pixel scan positions (reading R28 -- PAPER.md does not say how the fractional part of a position
+       is treated, so the textbook rule is taken: the Fourier shift theorem applied to the probe).                            */
+    const float *subpixel_yx;   /* HOST pointer or NULL: n_pos x (dy, dx), each in [0, 1): frame j sits at pos_yx[j] + (dy, dx).  It sees
+                                   the probe P_jk = S_d[P_k] = F^-1[F[P_k] exp(-2 pi i (k_y dy + k_x dx)/N)] (k signed, Nyquist = -N/2),
+                                   the object patch stays at the integer corner; object sums use conj(P_jk), |P_jk|^2; the probe term
+                                   conj(O_j) chi_jk is shifted back by S_{-d} before it is summed; d_P = sum_j |O_j|^2 and the object
+                                   regulariser delta_obj max_r sum_k |P_k|^2 use unshifted quantities.  PTYCHO_EPIE_MB only: ptycho_iterate
+                                   returns PTYCHO_EUNSUPPORTED for the other algorithms, ptycho_revised_waves / ptycho_eval_error
+                                   likewise; init returns it with deterministic, dm_sweeps or shard_total_pos.  Two more 2-D FFTs per
+                                   frame and mode, one launch-sized buffer of per-frame probes in the workspace.  Copied at init.  */
 } ptycho_params;
 
 void ptycho_default_params(ptycho_params *p);

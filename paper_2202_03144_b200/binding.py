@@ -41,7 +41,7 @@ class Params(C.Structure):
                 ("alpha_probe", C.c_float), ("lsq_lambda", C.c_float), ("pbound", C.c_float),
                 ("disable_dm", C.c_int), ("deterministic", C.c_int), ("dm_sweeps", C.c_int),
                 ("batch_order", C.POINTER(C.c_int32)), ("shard_total_pos", C.c_int), ("n_foreign", C.c_int),
-                ("foreign_pos", C.POINTER(C.c_int32))]
+                ("foreign_pos", C.POINTER(C.c_int32)), ("subpixel_yx", C.POINTER(C.c_float))]
 
 
 class ShardBufs(C.Structure):
@@ -117,6 +117,10 @@ def default_params(**over) -> Params:
             if v is not None:
                 keep = np.ascontiguousarray(v, np.int32)
                 p.batch_order = keep.ctypes.data_as(C.POINTER(C.c_int32))
+        elif k == "subpixel_yx":
+            if v is not None:
+                p._keep_sub = np.ascontiguousarray(v, np.float32).reshape(-1, 2)
+                p.subpixel_yx = p._keep_sub.ctypes.data_as(C.POINTER(C.c_float))
         elif k == "foreign_pos":
             if v is not None and len(v):
                 p._keep_foreign = np.ascontiguousarray(v, np.int32).reshape(-1, 2)

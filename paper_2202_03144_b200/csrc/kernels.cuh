@@ -17,9 +17,9 @@ namespace ptycho {
 
 struct YX { int y, x; };
 
-enum RowFwdMode { RF_EXIT = 0, RF_DM = 1, RF_PLAIN = 2 };
+enum RowFwdMode { RF_EXIT = 0, RF_DM = 1, RF_PLAIN = 2, RF_EXIT_PJ = 3 };   // _PJ: per-frame probes (sub-pixel positions, R28)
 enum ColMode { CM_FULL = 0, CM_ERRONLY = 1, CM_PLAIN_FWD = 2, CM_PLAIN_INV = 3 };
-enum RowInvMode { RI_MINIBATCH = 0, RI_DM = 1, RI_REVISED = 2, RI_PLAIN = 3, RI_LSQ_PF = 4 };
+enum RowInvMode { RI_MINIBATCH = 0, RI_DM = 1, RI_REVISED = 2, RI_PLAIN = 3, RI_LSQ_PF = 4, RI_MINIBATCH_PJ = 5 };
 
 #ifndef PTYCHO_THREADS
 #define PTYCHO_THREADS 256
@@ -47,6 +47,8 @@ struct FrameArgs {
     double* pf_part;                // RI_LSQ_PF: per slot of this launch, NCB x 5 partial sums (A11, A22, A12, b1, b2)
     const float2* __restrict__ tw;  // twiddles [ka*T + b]
     const float2* __restrict__ twi; // twiddles [b*E + ka]
+    float2* Pj;                     // _PJ modes: this launch's per-frame probes P_jk = S_delta_j[P_k], nframes x K x N x N (like S); the
+                                    // inverse row pass overwrites them with the probe terms conj(O_j) chi_jk (R28)
 };
 
 template <int N> struct Geo {
@@ -113,7 +115,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_fw
         const size_t off = ((size_t)k * N + y) * N;
         float2 v[E];
 #pragma unroll
-        for (int i = 0; i < E; ++i) v[i] = cmul(__ldg(a.P + off + t + T * i), o[i]);   // psi_O = P_k O_j
+        for (int i = 0; i < E; ++i) v[i] = cmul(MODE == RF_EXIT_PJ ? a.Pj[fr + off + t + T * i] : __ldg(a.P + off + t + T * i), o[i]);   // psi_O = P_k O_j
         if (MODE == RF_DM) {
             const float2* prow = a.psi + fr + off;
 #pragma unroll
@@ -316,7 +318,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads, (N >= 512
 #pragma unroll
         for (int r = 0; r < E; ++r) {
             const int x = pos_a_inv<N>(t, r);
-            const float2 p = __ldg(a.P + off + x);
+            const float2 p = MODE == RI_MINIBATCH_PJ ? a.Pj[fr + off + x] : __ldg(a.P + off + x);
             const float2 po = cmul(p, o[r]);            // psi_O
             float2 w;
             if (MODE == RI_DM) {
@@ -339,7 +341,8 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads, (N >= 512
                     pfs[4] = fmaf(vv.x, w.x, fmaf(vv.y, w.y, pfs[4]));
                     continue;
                 }
-                red_add(a.nP + off + x, cmulc(w, o[r]));                   // a9 conj(O_j) chi
+                if (MODE == RI_MINIBATCH_PJ) a.Pj[fr + off + x] = cmulc(w, o[r]);   // kept per frame: shifted back before it is summed (R28)
+                else red_add(a.nP + off + x, cmulc(w, o[r]));              // a9 conj(O_j) chi
             }
             accO[r] = cadd(accO[r], cmulc(w, p));                          // a8 conj(P_k) w
             accD[r] = fmaf(p.x, p.x, fmaf(p.y, p.y, accD[r]));
@@ -368,7 +371,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads, (N >= 512
         const int x = pos_a_inv<N>(t, r);
         red_add(a.nO + obase + x, accO[r]);
         red_add(a.dO + obase + x, accD[r]);
-        if (MODE == RI_MINIBATCH) red_add(a.dP + (size_t)y * N + x, o[r].x * o[r].x + o[r].y * o[r].y);
+        if (MODE == RI_MINIBATCH || MODE == RI_MINIBATCH_PJ) red_add(a.dP + (size_t)y * N + x, o[r].x * o[r].x + o[r].y * o[r].y);
     }
 }
 
@@ -786,6 +789,46 @@ template <typename TI, typename TO, int V> __global__ void __launch_bounds__(256
             for (int k = 0; k < (int)(V * sizeof(TO) / 16); ++k) reinterpret_cast<uint4*>(out + i)[k] = src[k];
         }
     }
+}
+
+// ---- sub-pixel positions (reading R28) ---------------------------------------------------------------------
+// ramp_d(k) = exp(-2 pi i (k_y d_y + k_x d_x) / N), k signed (k >= N/2 -> k - N).  Phase reduced in double: the argument reaches
+// pi N and fp32 would lose the last digits of the fraction there.
+__device__ __forceinline__ float2 shift_ramp(int ky, int kx, int n, float dy, float dx) {
+    const int sy = ky < n / 2 ? ky : ky - n, sx = kx < n / 2 ? kx : kx - n;
+    const double ph = -2.0 * ((double)sy * (double)dy + (double)sx * (double)dx) / (double)n;   // in units of pi
+    double sn, cs;
+    sincospi(ph, &sn, &cs);
+    return make_float2((float)cs, (float)sn);
+}
+// Pj[f][k] = FP[k] * ramp_{delta_f}: the spectra of the shifted probes of this launch's frames.  grid (nframes, K n^2 / 256)
+__global__ void k_sub_ramp(float2* __restrict__ Pj, const float2* __restrict__ FP, const float* __restrict__ frac, const int* __restrict__ frames,
+                           int K, int n, float scale) {
+    const size_t nn = (size_t)n * n, i = (size_t)blockIdx.y * blockDim.x + threadIdx.x;
+    if (i >= nn * K) return;
+    const int f = frames[blockIdx.x];
+    const size_t q = i % nn;
+    const float2 v = cmul(FP[i], shift_ramp((int)(q / n), (int)(q % n), n, frac[2 * f], frac[2 * f + 1]));
+    Pj[(size_t)blockIdx.x * K * nn + i] = make_float2(v.x * scale, v.y * scale);   // scale = 1/n^2 of the inverse transform that follows
+}
+// nPF[k] += sum_f conj(ramp_{delta_f}) G[f][k]: the back-shifted probe terms of this launch, summed in Fourier space in frame order
+// (fixed order, no atomics).  grid K n^2 / 256
+__global__ void k_sub_acc(float2* __restrict__ nPF, const float2* __restrict__ G, const float* __restrict__ frac, const int* __restrict__ frames,
+                          int nframes, int K, int n) {
+    const size_t nn = (size_t)n * n, i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nn * K) return;
+    const size_t q = i % nn;
+    const int ky = (int)(q / n), kx = (int)(q % n);
+    float2 acc = nPF[i];
+    for (int s = 0; s < nframes; ++s) {
+        const int f = frames[s];
+        acc = cadd(acc, cmulc(G[(size_t)s * K * nn + i], shift_ramp(ky, kx, n, frac[2 * f], frac[2 * f + 1])));   // G conj(ramp)
+    }
+    nPF[i] = acc;
+}
+// dst = src * s (element-wise)
+__global__ void k_scale_to(float2* __restrict__ dst, const float2* __restrict__ src, size_t n, float s) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) dst[i] = make_float2(src[i].x * s, src[i].y * s);
 }
 
 }  // namespace ptycho

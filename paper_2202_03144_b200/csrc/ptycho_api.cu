@@ -89,6 +89,11 @@ struct ptycho_ctx {
     std::vector<int> batch_order_h, mb_h;
     long long n_steps = 0;
     bool psi_valid = false;
+    // sub-pixel positions (params.subpixel_yx, R28): fractions (device, caller numbering), F[P], Fourier-space probe numerator,
+    // per-frame probes of one launch
+    float* sub_frac = nullptr;
+    float2 *sub_FP = nullptr, *sub_nPF = nullptr, *sub_Pj = nullptr;
+    std::vector<float> sub_frac_h;
     // shard of a scan held by several GPUs (ptycho_shard_begin / _end): positions of the other shards' frames over our rows
     std::vector<int32_t> foreign_h;
     bool shard_open = false;                   // between ptycho_shard_begin and ptycho_shard_end
@@ -271,6 +276,12 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
     }
     // Intensities passed from host memory are needed on the device only during init (sum, re-tiling): they are staged in the
     // exit-wave store, which is not written before the first DM iteration; only without that store do they get their own piece.
+    if (c->par.subpixel_yx || !c->sub_frac_h.empty()) {
+        c->sub_frac = w.take<float>(2 * (size_t)c->J);
+        c->sub_FP = w.take<float2>(knn);
+        c->sub_nPF = w.take<float2>(knn);
+        c->sub_Pj = w.take<float2>((size_t)c->chunk * knn);
+    }
     if (c->streaming) {
         c->stage_frames = std::max(1, std::min(c->J, (int)((64ull << 20) / (nn * (c->itype == PTYCHO_I_U16 ? 2 : 4)))));
         c->stage = w.take<char>((size_t)c->stage_frames * nn * (c->itype == PTYCHO_I_U16 ? 2 : 4));
@@ -292,6 +303,8 @@ template <int N> ptycho_status set_attrs(ptycho_ctx* c) {
     CU(cudaFuncSetAttribute(k_rows_fwd<N, RF_EXIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_fwd<N, RF_DM>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_fwd<N, RF_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_rows_fwd<N, RF_EXIT_PJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_rows_inv<N, RI_MINIBATCH_PJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_inv<N, RI_MINIBATCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_inv<N, RI_DM>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_inv<N, RI_REVISED>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
@@ -340,6 +353,7 @@ template <int N> void launch_passes(ptycho_ctx* c, const FrameArgs& a, int nfram
     if (fwd >= 0) LAUNCH(c, PTYCHO_K_ROWS_FWD, {
         if (fwd == RF_EXIT) k_rows_fwd<N, RF_EXIT><<<grid, blk, sr, s>>>(a);
         else if (fwd == RF_DM) k_rows_fwd<N, RF_DM><<<grid, blk, sr, s>>>(a);
+        else if (fwd == RF_EXIT_PJ) k_rows_fwd<N, RF_EXIT_PJ><<<grid, blk, sr, s>>>(a);
         else k_rows_fwd<N, RF_PLAIN><<<grid, blk, sr, s>>>(a);
     });
     if (col >= 0) LAUNCH(c, PTYCHO_K_COLS, {
@@ -353,6 +367,7 @@ template <int N> void launch_passes(ptycho_ctx* c, const FrameArgs& a, int nfram
         else if (inv == RI_DM) k_rows_inv<N, RI_DM><<<grid, blk, sr, s>>>(a);
         else if (inv == RI_REVISED) k_rows_inv<N, RI_REVISED><<<grid, blk, sr, s>>>(a);
         else if (inv == RI_LSQ_PF) k_rows_inv<N, RI_LSQ_PF><<<grid, blk, sr, s>>>(a);
+        else if (inv == RI_MINIBATCH_PJ) k_rows_inv<N, RI_MINIBATCH_PJ><<<grid, blk, sr, s>>>(a);
         else k_rows_inv<N, RI_PLAIN><<<grid, blk, sr, s>>>(a);
     });
 }
@@ -511,6 +526,17 @@ updates:
     return PTYCHO_OK;
 }
 
+// Unscaled batched 2-D FFT of `count` N x N frames in place (the plain variants of the three-pass kernels).
+void plain_fft2(ptycho_ctx* c, float2* buf, int count, bool inverse) {
+    const size_t nn = (size_t)c->N * c->N;
+    for (int f0 = 0; f0 < count; f0 += 32768) {             // frames ride in gridDim.y
+        FrameArgs a = base_args(c);
+        a.S = buf + (size_t)f0 * nn; a.K = 1;
+        if (!inverse) passes(c, a, std::min(32768, count - f0), RF_PLAIN, CM_PLAIN_FWD, -1);
+        else passes(c, a, std::min(32768, count - f0), -1, CM_PLAIN_INV, RI_PLAIN);
+    }
+}
+
 ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
     const size_t nn = (size_t)c->N * c->N, HW = (size_t)c->H * c->W;
     const int ncb = ncb_of(c->N);
@@ -520,6 +546,32 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
         const int b0 = c->mb_offsets[b], b1 = c->mb_offsets[b + 1];
         CU(cudaMemsetAsync(&c->sc->max_p2, 0, sizeof(float), c->stream));
         LAUNCH(c, PTYCHO_K_UPDATE, (k_probe_max<<<64, 256, 0, c->stream>>>(c->P, c->K, (int)nn, c->sc)));
+        if (c->sub_frac) {
+            // Sub-pixel positions (R28).  Per launch: the frames' shifted probes P_jk = F^-1[F[P_k] ramp_j] into sub_Pj, the cycle with
+            // them (the inverse row pass leaves the probe terms conj(O_j) chi_jk in sub_Pj), their spectra times conj(ramp_j) summed
+            // into sub_nPF; per batch one inverse transform brings the sum back: n_P = F^-1[sub_nPF].
+            const size_t knn = nn * c->K;
+            const float inv_n2 = 1.0f / ((float)c->N * (float)c->N);
+            CU(cudaMemcpyAsync(c->sub_FP, c->P, knn * 8, cudaMemcpyDeviceToDevice, c->stream));
+            plain_fft2(c, c->sub_FP, c->K, false);
+            CU(cudaMemsetAsync(c->sub_nPF, 0, knn * 8, c->stream));
+            for (int s0 = b0; s0 < b1; s0 += c->chunk) {
+                const int nf = std::min(c->chunk, b1 - s0);
+                LAUNCH(c, PTYCHO_K_OTHER, (k_sub_ramp<<<dim3(nf, (unsigned)((knn + 255) / 256)), 256, 0, c->stream>>>(
+                                               c->sub_Pj, c->sub_FP, c->sub_frac, c->mb_frames + s0, c->K, c->N, inv_n2)));
+                plain_fft2(c, c->sub_Pj, nf * c->K, true);
+                FrameArgs a = base_args(c);
+                a.frames = c->mb_frames + s0;
+                a.e_part = c->e_part + (size_t)s0 * ncb;
+                a.Pj = c->sub_Pj;
+                passes(c, a, nf, RF_EXIT_PJ, CM_FULL, RI_MINIBATCH_PJ);
+                plain_fft2(c, c->sub_Pj, nf * c->K, false);
+                LAUNCH(c, PTYCHO_K_OTHER, (k_sub_acc<<<(unsigned)((knn + 255) / 256), 256, 0, c->stream>>>(
+                                               c->sub_nPF, c->sub_Pj, c->sub_frac, c->mb_frames + s0, nf, c->K, c->N)));
+            }
+            plain_fft2(c, c->sub_nPF, c->K, true);
+            LAUNCH(c, PTYCHO_K_OTHER, (k_scale_to<<<ew_blocks(knn), 256, 0, c->stream>>>(c->nP, c->sub_nPF, knn, inv_n2)));
+        } else
         for (int s0 = b0; s0 < b1; s0 += c->chunk) {
             const int nf = std::min(c->chunk, b1 - s0);
             FrameArgs a = base_args(c);
@@ -642,6 +694,11 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     if (!shard && par.n_foreign > 0) return PTYCHO_EINVAL;
     if (shard && par.shard_total_pos < n_pos + par.n_foreign) return PTYCHO_EINVAL;
     if (shard && (n_modes != 1 || par.disable_dm || par.deterministic || par.dm_sweeps > 0 || !intensities)) return PTYCHO_EUNSUPPORTED;
+    if (par.subpixel_yx) {
+        if (par.deterministic || par.dm_sweeps > 0 || shard || !intensities) return PTYCHO_EUNSUPPORTED;
+        for (int j = 0; j < 2 * n_pos; ++j)
+            if (!(par.subpixel_yx[j] >= 0.f && par.subpixel_yx[j] < 1.f)) return PTYCHO_EINVAL;
+    }
     for (int j = 0; j < par.n_foreign; ++j) {
         const int y = par.foreign_pos[2 * j], x = par.foreign_pos[2 * j + 1];
         if (y < 0 || x < 0 || y + n > obj_h || x + n > obj_w) return PTYCHO_EBOUNDS;
@@ -721,6 +778,11 @@ ptycho_status ptycho_init(ptycho_ctx** out, const float* object, int obj_h, int 
     c->par.batch_order = nullptr;   // copied; the caller's pointer is not kept
     if (par.n_foreign > 0) c->foreign_h.assign(par.foreign_pos, par.foreign_pos + 2 * (size_t)par.n_foreign);
     c->par.foreign_pos = nullptr;
+    if (par.subpixel_yx) {
+        c->sub_frac_h.assign(par.subpixel_yx, par.subpixel_yx + 2 * (size_t)n_pos);
+        CUI(cudaMemcpyAsync(c->sub_frac, c->sub_frac_h.data(), c->sub_frac_h.size() * 4, cudaMemcpyHostToDevice, s));
+    }
+    c->par.subpixel_yx = nullptr;
     if (shard) {
         if (!c->p2) { g_init_error = "a shard needs the DM megakernel path"; delete c; return PTYCHO_EUNSUPPORTED; }
         int r0 = obj_h, r1 = 0;
@@ -813,6 +875,7 @@ ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
     if (alg != PTYCHO_DM && c->par.deterministic) return fail(c, PTYCHO_EUNSUPPORTED, "deterministic mode covers DM only");
     if (alg == PTYCHO_DM && !c->psi) return fail(c, PTYCHO_ESTATE, "DM needs the exit-wave store (disable_dm was set)");
     if (c->par.shard_total_pos > 0) return fail(c, PTYCHO_ESTATE, "a shard is driven by ptycho_shard_begin / ptycho_shard_end");
+    if (c->sub_frac && alg != PTYCHO_EPIE_MB) return fail(c, PTYCHO_EUNSUPPORTED, "sub-pixel positions: PTYCHO_EPIE_MB only");
     if (c->streaming) {
         if (c->present == 0) return fail(c, PTYCHO_ESTATE, "no frame has been appended yet");
         if (alg == PTYCHO_DM && c->present < c->J) return fail(c, PTYCHO_ESTATE, "DM needs every frame (PAPER.md:58); append the rest first");
@@ -944,6 +1007,7 @@ ptycho_status ptycho_set_exit_waves(ptycho_ctx* c, const float* psi) {
 
 ptycho_status ptycho_revised_waves(ptycho_ctx* c, const int32_t* idx, int count, float* out) {
     if (!c || !idx || !out || count < 0) return PTYCHO_EINVAL;
+    if (c->sub_frac) return fail(c, PTYCHO_EUNSUPPORTED, "sub-pixel positions: not available");
     for (int i = 0; i < count; ++i)
         if (idx[i] < 0 || idx[i] >= c->J) return fail(c, PTYCHO_EINVAL, "frame index out of range");
     const size_t knn = (size_t)c->K * c->N * c->N;
@@ -963,6 +1027,7 @@ ptycho_status ptycho_revised_waves(ptycho_ctx* c, const int32_t* idx, int count,
 
 ptycho_status ptycho_eval_error(ptycho_ctx* c, double* out) {
     if (!c || !out) return PTYCHO_EINVAL;
+    if (c->sub_frac) return fail(c, PTYCHO_EUNSUPPORTED, "sub-pixel positions: not available");
     if (c->present < c->J) return fail(c, PTYCHO_ESTATE, "eval_error needs every frame");
     if (c->streaming) CU(cudaStreamWaitEvent(c->stream, c->ev_append, 0));
     k_snap_sum_I<<<1, 1, 0, c->stream>>>(c->sc);

@@ -787,3 +787,55 @@ def test_shard_contexts_refuse_what_they_do_not_support(B):
         plain.shard_begin()                                 # and an ordinary context is not a shard
     plain.destroy()
     g.destroy()
+
+
+# ------------------------------------------------------------- sub-pixel scan positions (reading R28)
+@pytest.mark.parametrize("n,h,side,step,k,dtype,pbound,batch", [
+    (64, 300, 6, 21, 1, np.float32, 0.0, 9),
+    (64, 300, 6, 21, 2, np.uint16, 0.3, 0),
+    (128, 420, 5, 40, 3, np.uint16, 0.0, 7),
+    (256, 600, 3, 90, 1, np.float32, 0.0, 4)])
+def test_subpixel_positions_epie_minibatch(B, oracle_mod, n, h, side, step, k, dtype, pbound, batch):
+    """ePIE-minibatch with fractional positions: the probe every frame sees is the Fourier-shifted one, the probe term is shifted
+    back before it is summed.  Against oracle/subpixel.py (fp64 numpy, pinned in test_oracle_pins.py), free-running."""
+    from oracle import subpixel
+    s = synth.make_custom(n, h, side, step, k=k, peak=2e4 if dtype == np.uint16 else None, dtype=dtype, jitter=2, seed=41,
+                          probe_kind="zone")
+    rng = np.random.default_rng(17)
+    frac = rng.uniform(0, 1, (len(s.pos), 2)).astype(np.float32)
+    frac[0] = 0.0                                            # an exactly integer position among them
+    par = dict(batch_size=batch, probe_start=1, pbound=pbound, alpha_obj=0.9, alpha_probe=0.8)
+    o = subpixel.SubpixelOracle(s.obj0, s.probe0, s.pos, frac, s.intensities, par)
+    g = B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(subpixel_yx=frac, **par))
+    for it in range(4):
+        o.iterate(1)
+        g.iterate("EPIE_MB", 1)
+        ro, rp = rel(g.fetch_object(), o.O), rel(g.fetch_probe(), o.P)
+        assert ro < TOL_ITER * (it + 1) and rp < TOL_ITER * (it + 1), (it, ro, rp)
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+    # the fractions matter at this tolerance: the ordinary path on the same input is far away
+    z = B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(**par))
+    z.iterate("EPIE_MB", 4)
+    assert rel(z.fetch_object(), o.O) > 50 * TOL_ITER
+    z.destroy()
+    for alg in ("DM", "LSQML", "LSQML_PF"):                  # ePIE-minibatch only
+        with pytest.raises(B.PtychoError):
+            g.iterate(alg, 1)
+    with pytest.raises(B.PtychoError):
+        g.revised_waves(np.arange(2, dtype=np.int32))
+    g.destroy()
+
+
+def test_subpixel_zero_fractions_reproduce_the_ordinary_path(B):
+    """delta_j = 0: the per-frame probes are F^-1 F P = P up to fp32 rounding, so the sub-pixel path must track the ordinary one."""
+    s = synth.make_custom(64, 300, 6, 21, k=2, seed=43, jitter=2)
+    par = dict(batch_size=9, probe_start=0)
+    g = B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(subpixel_yx=np.zeros((len(s.pos), 2), np.float32), **par))
+    z = B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(**par))
+    g.iterate("EPIE_MB", 3); z.iterate("EPIE_MB", 3)
+    assert rel(g.fetch_object(), z.fetch_object()) < 1e-5 and rel(g.fetch_probe(), z.fetch_probe()) < 1e-5
+    with pytest.raises(B.PtychoError):                       # a fraction outside [0, 1)
+        B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(subpixel_yx=np.full((len(s.pos), 2), 1.0, np.float32)))
+    with pytest.raises(B.PtychoError):
+        B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(subpixel_yx=np.zeros((len(s.pos), 2), np.float32), deterministic=1))
+    g.destroy(); z.destroy()

@@ -435,6 +435,48 @@ def test_cfg2_full_size_steady_state_teacher_forced(B, oracle_mod, record_proper
     g.destroy()
 
 
+def test_cfg4_full_size_second_iteration_teacher_forced(B, oracle_mod):
+    """Config 4 at FULL size (N = 512, J = 16 384: a 34 GB exit-wave store, 4.3 G complex elements -- indices beyond 2^31 -- and
+    the ring capped at 96 MB), as `bench.py --config 4` runs it.  The first iteration forms psi in pass 1; the SECOND reads the
+    store, so it is the one checked: teacher-forced from the GPU's state after iteration 1 on 24 sampled frames (first, last,
+    random), and the object on a window from the closed form of the overlap update with the new waves of every frame over it."""
+    s = synth.make_config(4)
+    par = dict(pbound=s.params["pbound"])
+    J, n = s.n_pos, s.n
+    assert J == 16384 and n == 512
+    rng = np.random.default_rng(44)
+    idx = np.sort(rng.choice(J, 24, replace=False)).astype(np.int32)
+    idx[0], idx[-1] = 0, J - 1
+    g = make(B, s, **par)
+    g.iterate("DM", 1)
+    O1, P1, psi1 = g.fetch_object(), g.fetch_probe(), g.fetch_exit_waves(idx)
+    g.iterate("DM", 1)
+    o = oracle_mod.Oracle(O1, P1, s.pos[idx], s.intensities[idx], par)
+    o.psi = psi1.astype(np.complex128)
+    o.iterate("DM", 1)
+    psi2 = g.fetch_exit_waves(idx)
+    worst = max(rel(psi2[k], o.psi[k]) for k in range(len(idx)))
+    assert worst < TOL_ITER, worst
+    cy, cx = s.obj0.shape[0] // 2, s.obj0.shape[1] // 2
+    y0, x0, w = cy - 40, cx + 25, 32
+    cover = np.array([j for j, (y, x) in enumerate(s.pos) if y < y0 + w and y + n > y0 and x < x0 + w and x + n > x0], np.int32)
+    assert len(cover) > 20
+    psi_c = g.fetch_exit_waves(cover)                            # iteration 2's waves
+    num = np.zeros((w, w), complex); den = np.zeros((w, w))
+    for k, j in enumerate(cover):
+        py, px = s.pos[j]
+        ys, ye, xs, xe = max(y0, py), min(y0 + w, py + n), max(x0, px), min(x0 + w, px + n)
+        sl = (slice(ys - py, ye - py), slice(xs - px, xe - px))
+        num[ys - y0:ye - y0, xs - x0:xe - x0] += np.conj(P1[0][sl]) * psi_c[k, 0][sl].astype(complex)
+        den[ys - y0:ye - y0, xs - x0:xe - x0] += np.abs(P1[0][sl]) ** 2
+    eps = 1e-2 * np.max(np.abs(s.probe0) ** 2)                   # R5, fixed at init
+    O2 = g.fetch_object()
+    assert rel(O2[y0:y0 + w, x0:x0 + w], (num + eps * O1[y0:y0 + w, x0:x0 + w]) / (den + eps)) < TOL_ITER
+    e = g.fetch_error()
+    assert np.all(np.isfinite(e)) and e[1] < e[0]
+    g.destroy()
+
+
 def test_dm_inside_the_power_bound_paths(B, oracle_mod):
     """Frames whose error is inside the power bound (R6, rb = 1) take the short pass 3 (psi' = P O_j, no transform, no
     scatter), and once most frames are there the megakernel switches to its split form (error-only column pass, the full pass

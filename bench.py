@@ -392,9 +392,9 @@ def sharded_line(args) -> dict | None:
         raise SystemExit("bench.py: no CUDA device; the projection cycle has no CPU path")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
+    if "RANK" in os.environ and "MASTER_ADDR" in os.environ:       # launched by torchrun (any world size): its rendezvous
         dist.init_process_group("nccl", device_id=dev)
-    else:
+    else:                                                            # plain `python bench.py --sharded`: a group of one
         dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % (29500 + os.getpid() % 2000), rank=0, world_size=1, device_id=dev)
     from paper_2202_03144_b200 import binding, sharded, synth
     binding.lib()

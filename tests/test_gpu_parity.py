@@ -733,29 +733,39 @@ def test_split_form_under_queue_geometries(B, oracle_mod, monkeypatch):
         g.destroy()
 
 
-def test_strict_sync_build_is_bit_identical(tmp_path):
+@pytest.mark.parametrize("size", ["small", pytest.param("cfg2_full", marks=pytest.mark.skipif(
+    not __import__("os").environ.get("PTYCHO_LONG_TESTS"), reason="opt-in (PTYCHO_LONG_TESTS=1): builds N = 256 twice, config 2 at full size"))])
+def test_strict_sync_build_is_bit_identical(tmp_path, size):
     """The megakernel's hand-off polls with relaxed loads (DESIGN.md section 5.2 says what that assumes).  A build with
     -DPTYCHO_STRICT_SYNC polls with ld.acquire.gpu instead; in deterministic mode the two builds must agree bit for bit over a
-    multi-iteration run with ring wrap-around -- a reordering the relaxed protocol allowed would show up as a difference."""
+    multi-iteration run with ring wrap-around -- a reordering the relaxed protocol allowed would show up as a difference.
+    "cfg2_full" (opt-in) does the same at the size bench.py times: J = 10 000 frames of 256^2, 12 iterations, default geometry."""
     import hashlib, os, subprocess, sys
     script = tmp_path / "run.py"
-    script.write_text('''
+    make_scan = ('s = synth.make_custom(64, 260, 9, 21, k=1, peak=2e4, dtype=np.uint16, jitter=3, seed=77, probe_kind="zone"); pb, its = 0.3, 25'
+                 if size == "small" else 's = synth.make_config(2); pb, its = s.params["pbound"], 12')
+    script.write_text(('''
 import hashlib, sys, numpy as np
 sys.path.insert(0, %r)
 from paper_2202_03144_b200 import binding, synth
 binding.build()
-s = synth.make_custom(64, 260, 9, 21, k=1, peak=2e4, dtype=np.uint16, jitter=3, seed=77, probe_kind="zone")
-g = binding.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, binding.default_params(pbound=0.3, deterministic=1))
-g.iterate("DM", 25)
+MAKE_SCAN
+g = binding.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, binding.default_params(pbound=pb, deterministic=1))
+g.iterate("DM", its)
+'''.replace("MAKE_SCAN", make_scan) + '''
 h = hashlib.sha1()
 for a in (g.fetch_object(), g.fetch_probe(), g.fetch_exit_waves(), g.fetch_error()):
     h.update(np.ascontiguousarray(a).tobytes())
 print("HASH", h.hexdigest())
-''' % os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+''') % os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
     out = {}
     for tag, defs in (("relaxed", ""), ("strict", "-DPTYCHO_STRICT_SYNC")):
-        env = dict(os.environ, PTYCHO_BUILD_ONLY_N="64", PTYCHO_BUILD_TAG=tag, PTYCHO_BUILD_DEFS=defs, PTYCHO_MEGA_M="2", PTYCHO_MEGA_D="2", PTYCHO_MEGA_X="1")
-        r = subprocess.run([sys.executable, str(script)], env=env, capture_output=True, text=True, timeout=900)
+        env = dict(os.environ, PTYCHO_BUILD_TAG=tag, PTYCHO_BUILD_DEFS=defs)
+        if size == "small":
+            env.update(PTYCHO_BUILD_ONLY_N="64", PTYCHO_MEGA_M="2", PTYCHO_MEGA_D="2", PTYCHO_MEGA_X="1")
+        else:
+            env.update(PTYCHO_BUILD_ONLY_N="256")
+        r = subprocess.run([sys.executable, str(script)], env=env, capture_output=True, text=True, timeout=1800)
         assert r.returncode == 0, r.stderr[-2000:]
         out[tag] = [l for l in r.stdout.splitlines() if l.startswith("HASH")][0]
     assert out["relaxed"] == out["strict"]

@@ -218,6 +218,44 @@ def cufft_reference_line(args) -> dict:
             "note": "torch.fft (cuFFT) on resident complex64 frames; a reference point, not part of the library"}
 
 
+def mma_dft_line(args) -> dict:
+    """B:ns "tensor cores ... DFT-as-GEMM ... only if it beats the packed-fp32 line FFT at <= 2e-6 error": the micro-benchmark.
+    The forward FFT of every row of resident 256 x 256 complex64 frames by (0) the row pass of the product kernels and (1) the
+    tensor-core kernel of csrc/fft_mma.cuh, on 2048 frames (1 GB, 524 288 lines per launch; a working set small enough to stay in
+    L2 would make launches of ~20 us, which measure the launch); CUDA events, 20 repetitions after 3 warm-ups; error of each
+    against numpy's FFT in double.  torch.fft (cuFFT) rows beside them as a reference point.  At 4 KB per line the HBM bound is
+    1.6 G lines/s."""
+    import torch
+    from paper_2202_03144_b200 import binding
+    dev = torch.device("cuda", 0)
+    n = 256
+    g = torch.Generator(device=dev).manual_seed(1)
+    out = {"impl": "mma_dft_microbenchmark", "unit": "lines/s", "line": n}
+    small = torch.randn((6, n, n), dtype=torch.complex64, device=dev, generator=g)
+    want = np.fft.fft(small.cpu().numpy().astype(np.complex128), axis=-1)
+    for impl, name in ((0, "packed_fp32"), (1, "mma_tf32x3")):
+        got = binding.test_fft_rows(small.clone(), impl=impl).cpu().numpy()
+        out[name + "_rel_l2_error"] = float(np.linalg.norm(got - want) / np.linalg.norm(want))
+    for frames, tag in ((2048, "hbm_streamed_1GB"),):
+        x = torch.randn((frames, n, n), dtype=torch.complex64, device=dev, generator=g)
+        fns = {"packed_fp32": lambda: binding.test_fft_rows(x, impl=0), "mma_tf32x3": lambda: binding.test_fft_rows(x, impl=1),
+               "cufft_rows": lambda: torch.fft.fft(x, dim=-1, out=x)}
+        for name, fn in fns.items():
+            x.normal_(generator=g); x *= 1e-30               # unscaled transforms applied repeatedly in place (x16 each): stays finite
+            for _ in range(3):
+                fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(20):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            out[f"{name}_{tag}"] = frames * n * 20 / (e0.elapsed_time(e1) * 1e-3)
+    out["note"] = ("rows only (load, 256-point FFT, store); lines/s; the product's DM iteration needs 4 x 2.56 M line FFTs at config 2. "
+                   "A micro-benchmark: the tensor-core kernel is not part of any product path")
+    return out
+
+
 # --------------------------------------------------------------------------- this build's arm
 def dist_env():
     return (int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)),
@@ -460,6 +498,7 @@ def main():
     ap.add_argument("--config", type=int, default=CFG, choices=[1, 2, 3, 4], help="BASELINE.json configs[i] (default 2: the metric's)")
     ap.add_argument("--alg", default=None, choices=["DM", "EPIE_MB", "LSQML"], help="default: the config's own algorithm")
     ap.add_argument("--cufft-ref", action="store_true", help="print the torch.fft reference point instead (harness-side)")
+    ap.add_argument("--mma-dft", action="store_true", help="print the DFT-as-GEMM micro-benchmark instead (csrc/fft_mma.cuh)")
     ap.add_argument("--n-pos", type=int, default=None, help="truncate the scan (debugging only; invalidates the metric)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sharded", action="store_true", help="split ONE scan over the ranks instead of running replicas (SURVEY 8(f) f4)")
@@ -468,6 +507,10 @@ def main():
     if args.cufft_ref:
         if rank == 0:
             print(json.dumps(cufft_reference_line(args)), flush=True)
+        return
+    if args.mma_dft:
+        if rank == 0:
+            print(json.dumps(mma_dft_line(args)), flush=True)
         return
     if args.impl == "reference":
         if rank == 0:

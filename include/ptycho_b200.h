@@ -295,6 +295,16 @@ ptycho_status ptycho_test_fft2(float *data, int n, int count, int inverse, void 
 #define PTYCHO_NOALLOC_MAX_N 512
 ptycho_status ptycho_fft2_noalloc(float *data, int n, int count, int inverse, void *cuda_stream);
 
+/* ---- micro-benchmark entry point: DFT-as-GEMM against the packed-fp32 line FFT (BASELINE.json north_star) ----
+ * The forward 1-D FFT of every ROW of `count` n x n complex64 frames, in place, unscaled, natural order.
+ *   impl 0: the row pass of the product kernels (register-blocked packed-fp32 line FFT, one shared-memory exchange); n = 64..512.
+ *   impl 1: the same transform as two radix-16 stages on the tensor cores, one warp per line, no shared memory
+ *           (csrc/fft_mma.cuh: mma.sync m16n8k8 TF32 with a 3-term split, fp32 accumulation); n = 256 only.
+ * data: DEVICE pointer.  Asynchronous on cuda_stream (time it with events); allocates nothing (uses the static scratch of
+ * ptycho_fft2_noalloc for the twiddles of impl 0: the same sharing rules apply).  PTYCHO_EUNSUPPORTED for other n, PTYCHO_EINVAL
+ * for bad arguments.  Not used by any product path. */
+ptycho_status ptycho_test_fft_rows(float *data, int n, int count, int impl, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -373,3 +373,18 @@ def fft2_noalloc(data, inverse: bool = False):
     if st != 0:
         raise PtychoError(st, l.ptycho_last_error(None).decode())
     return data
+
+
+def test_fft_rows(data, impl: int = 0):
+    """ptycho_test_fft_rows: forward 1-D FFT of every row of a torch CUDA complex64 tensor (count, n, n), in place; impl 0 = the
+    product's packed-fp32 line FFT, impl 1 = tensor-core DFT (n = 256).  Asynchronous on torch's current stream."""
+    import torch
+    assert data.is_cuda and data.dtype == torch.complex64 and data.is_contiguous()
+    l = lib()
+    l.ptycho_test_fft_rows.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
+    with torch.cuda.device(data.device):
+        st = l.ptycho_test_fft_rows(C.c_void_p(data.data_ptr()), data.shape[-1], int(data.numel() // data.shape[-1] ** 2), int(impl),
+                                    C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if st != 0:
+        raise PtychoError(st, l.ptycho_last_error(None).decode())
+    return data

@@ -20,6 +20,7 @@
 #include "kernels.cuh"
 #include "dm_mega.cuh"
 #include "dm_det.cuh"
+#include "fft_mma.cuh"
 
 using namespace ptycho;
 
@@ -1293,14 +1294,9 @@ ptycho_status noalloc_fail(ptycho_status st, const std::string& msg) {
 
 }  // namespace
 
-extern "C" ptycho_status ptycho_fft2_noalloc(float* data, int n, int count, int inverse, void* cuda_stream) {
-    if (n > PTYCHO_NOALLOC_MAX_N)
-        return noalloc_fail(PTYCHO_ENOMEM, "n = " + std::to_string(n) + " exceeds the static scratch (PTYCHO_NOALLOC_MAX_N = " + std::to_string(PTYCHO_NOALLOC_MAX_N) + ")");
-    if (!data || count < 1) return noalloc_fail(PTYCHO_EINVAL, "null data or count < 1");
-    if (!valid_n(n)) return noalloc_fail(PTYCHO_EINVAL, "n must be 64, 128, 256 or 512 (and built into this library)");
-    ptycho_ctx tmp;                                        // host-side bookkeeping of the launch helpers only
-    ptycho_ctx* c = &tmp;
-    c->N = n; c->K = 1; c->stream = static_cast<cudaStream_t>(cuda_stream);
+// The static scratch's device address on the current device (taken once per device), the kernels' attributes for size n (once per
+// device and size), and this call's twiddle tables written into the scratch on c->stream.
+static ptycho_status noalloc_setup(ptycho_ctx* c, int n, float2** tw_out) {
     int dev = -1;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kNoAllocMaxDevices) return noalloc_fail(PTYCHO_ECUDA, "cudaGetDevice failed or device ordinal >= 64");
     float2* tw = nullptr;
@@ -1322,8 +1318,25 @@ extern "C" ptycho_status ptycho_fft2_noalloc(float* data, int n, int count, int 
         }
     }
     const int E = n == 64 ? 8 : n == 512 ? 32 : 16;
+    k_fill_twiddles<<<(n + 255) / 256, 256, 0, c->stream>>>(tw, tw + PTYCHO_NOALLOC_MAX_N, n, E, n / E);   // the part of the scratch this call uses
+    *tw_out = tw;
+    return PTYCHO_OK;
+}
+
+extern "C" ptycho_status ptycho_fft2_noalloc(float* data, int n, int count, int inverse, void* cuda_stream) {
+    if (n > PTYCHO_NOALLOC_MAX_N)
+        return noalloc_fail(PTYCHO_ENOMEM, "n = " + std::to_string(n) + " exceeds the static scratch (PTYCHO_NOALLOC_MAX_N = " + std::to_string(PTYCHO_NOALLOC_MAX_N) + ")");
+    if (!data || count < 1) return noalloc_fail(PTYCHO_EINVAL, "null data or count < 1");
+    if (!valid_n(n)) return noalloc_fail(PTYCHO_EINVAL, "n must be 64, 128, 256 or 512 (and built into this library)");
+    ptycho_ctx tmp;                                        // host-side bookkeeping of the launch helpers only
+    ptycho_ctx* c = &tmp;
+    c->N = n; c->K = 1; c->stream = static_cast<cudaStream_t>(cuda_stream);
+    float2* tw = nullptr;
+    {
+        const ptycho_status st = noalloc_setup(c, n, &tw);
+        if (st != PTYCHO_OK) return st;
+    }
     float2* twi = tw + PTYCHO_NOALLOC_MAX_N;
-    k_fill_twiddles<<<(n + 255) / 256, 256, 0, c->stream>>>(tw, twi, n, E, n / E);   // the part of the scratch this call uses
     const size_t nn = (size_t)n * n;
     for (int f0 = 0; f0 < count; f0 += 32768) {            // frames ride in gridDim.y
         const int nf = std::min(32768, count - f0);
@@ -1333,6 +1346,33 @@ extern "C" ptycho_status ptycho_fft2_noalloc(float* data, int n, int count, int 
         else {
             passes(c, a, nf, -1, CM_PLAIN_INV, RI_PLAIN);
             k_scale<<<ew_blocks((size_t)nf * nn), 256, 0, c->stream>>>(a.S, (size_t)nf * nn, 1.0f / ((float)n * n));
+        }
+    }
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return noalloc_fail(PTYCHO_ECUDA, cudaGetErrorString(e));
+    return PTYCHO_OK;
+}
+
+// Micro-benchmark entry point (include/ptycho_b200.h): the 1-D FFT of every row, by the product's packed-fp32 line FFT or on the
+// tensor cores (fft_mma.cuh).  Allocates nothing (the static scratch above), asynchronous.
+extern "C" ptycho_status ptycho_test_fft_rows(float* data, int n, int count, int impl, void* cuda_stream) {
+    if (!data || count < 1 || (impl != 0 && impl != 1)) return noalloc_fail(PTYCHO_EINVAL, "ptycho_test_fft_rows: bad argument");
+    if (!valid_n(n) || (impl == 1 && n != 256)) return noalloc_fail(PTYCHO_EUNSUPPORTED, "ptycho_test_fft_rows: n must be 64..512 (impl 0) or 256 (impl 1)");
+    ptycho_ctx tmp;
+    ptycho_ctx* c = &tmp;
+    c->N = n; c->K = 1; c->stream = static_cast<cudaStream_t>(cuda_stream);
+    if (impl == 1) {
+        int dev = 0, sms = 148;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PTYCHO_ECUDA;
+        k_rows_mma256<<<sms * 16, 128, 0, c->stream>>>(reinterpret_cast<float2*>(data), (long long)count * n);
+    } else {
+        float2* tw = nullptr;
+        const ptycho_status st = noalloc_setup(c, n, &tw);
+        if (st != PTYCHO_OK) return st;
+        for (int f0 = 0; f0 < count; f0 += 32768) {
+            FrameArgs a{};
+            a.S = reinterpret_cast<float2*>(data) + (size_t)f0 * n * n; a.K = 1; a.tw = tw; a.twi = tw + PTYCHO_NOALLOC_MAX_N;
+            passes(c, a, std::min(32768, count - f0), RF_PLAIN, -1, -1);
         }
     }
     const cudaError_t e = cudaGetLastError();

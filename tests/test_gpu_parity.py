@@ -55,6 +55,25 @@ def test_fft2_vs_oracle(B, oracle_mod, n):
     assert rel(back, x) < 2e-6
 
 
+@pytest.mark.parametrize("impl,n", [(0, 64), (0, 128), (0, 256), (0, 512), (1, 256)])
+def test_fft_rows_both_implementations_vs_library(B, n, impl):
+    """The row pass alone: the product's packed-fp32 line FFT (impl 0) and the tensor-core DFT micro-benchmark kernel (impl 1,
+    csrc/fft_mma.cuh: two radix-16 stages in mma.sync TF32 with a 3-term split) against numpy's FFT in double, at the FFT tolerance
+    north_star sets for the DFT-as-GEMM question (2e-6)."""
+    import torch
+    rng = np.random.default_rng(100 + n + impl)
+    x = (rng.standard_normal((6, n, n)) + 1j * rng.standard_normal((6, n, n))).astype(np.complex64)
+    x[0, 0] = 0; x[0, 0, 3] = 1.0                                           # a delta: one pure twiddle per output, catches index slips
+    d = torch.from_numpy(x).cuda()
+    got = B.test_fft_rows(d, impl=impl).cpu().numpy()
+    want = np.fft.fft(x.astype(np.complex128), axis=-1)
+    assert rel(got, want) < 2e-6, rel(got, want)
+    assert np.abs(got[0, 0] - want[0, 0]).max() < 2e-6
+    if impl == 1:
+        with pytest.raises(B.PtychoError):
+            B.test_fft_rows(torch.zeros((1, 128, 128), dtype=torch.complex64, device="cuda"), impl=1)
+
+
 # ------------------------------------------------------------- T3/T4 on config 0 (full size)
 @pytest.mark.parametrize("probe_start", [10 ** 9, 0])
 def test_cfg0_dm_free_running(B, oracle_mod, probe_start):

@@ -84,6 +84,15 @@ class SubpixelOracle:
         self.t = 0
         self.err: list[float] = []
 
+    def eval_error(self) -> float:
+        """C3 with the shifted probes: sum_j sum_q (sqrt I_j - A_j)^2 / sum I over unmasked pixels, A_j^2 = sum_k |F[P_jk O_j]|^2."""
+        n = self.P.shape[-1]
+        num = 0.0
+        for j, (y, x) in enumerate(self.pos):
+            Phi = np.fft.fft2(shift(self.P, *self.frac[j]) * self.O[None, y:y + n, x:x + n])
+            num += modulus_project(Phi, self.inten[j], 0.0)[1]
+        return num / (self.sum_I if self.sum_I > 0 else 1.0)
+
     def iterate(self, n_iters: int = 1):
         p = self.par
         for _ in range(n_iters):

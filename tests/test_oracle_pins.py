@@ -649,5 +649,8 @@ def test_subpixel_positions_matter_and_the_true_ones_fit_best(oracle_mod):
         inten[j] = np.abs(np.fft.fft2(subpixel.shift(s.probe_true, *frac[j])[0] * s.obj_true[y:y + n, x:x + n])) ** 2
     q = subpixel.SubpixelOracle(s.obj_true, s.probe_true, s.pos, frac, inten, dict(batch_size=4)).iterate(2)
     assert q.err[0] < 1e-12 and rel(q.O, s.obj_true) < 1e-6 and rel(q.P, s.probe_true) < 1e-6
+    assert q.eval_error() < 1e-12
     z = subpixel.SubpixelOracle(s.obj_true, s.probe_true, s.pos, 0 * frac, inten, dict(batch_size=4)).iterate(1)
     assert z.err[0] > 1e-4
+    z2 = subpixel.SubpixelOracle(s.obj_true, s.probe_true, s.pos, 0 * frac, inten)      # eval_error with zero fractions = the C oracle's
+    assert np.isclose(z2.eval_error(), oracle_mod.Oracle(s.obj_true, s.probe_true, s.pos, inten).eval_error(), rtol=1e-10) and z2.eval_error() > 1e-4

@@ -1028,16 +1028,28 @@ ptycho_status ptycho_revised_waves(ptycho_ctx* c, const int32_t* idx, int count,
 
 ptycho_status ptycho_eval_error(ptycho_ctx* c, double* out) {
     if (!c || !out) return PTYCHO_EINVAL;
-    if (c->sub_frac) return fail(c, PTYCHO_EUNSUPPORTED, "sub-pixel positions: not available");
     if (c->present < c->J) return fail(c, PTYCHO_ESTATE, "eval_error needs every frame");
     if (c->streaming) CU(cudaStreamWaitEvent(c->stream, c->ev_append, 0));
     k_snap_sum_I<<<1, 1, 0, c->stream>>>(c->sc);
     const int ncb = ncb_of(c->N);
+    if (c->sub_frac) {                                      // sub-pixel positions (R28): F[P] once, then every launch with its shifted probes
+        const size_t knn = (size_t)c->K * c->N * c->N;
+        CU(cudaMemcpyAsync(c->sub_FP, c->P, knn * 8, cudaMemcpyDeviceToDevice, c->stream));
+        plain_fft2(c, c->sub_FP, c->K, false);
+    }
     for (int s0 = 0; s0 < c->J; s0 += c->chunk) {
         const int nf = std::min(c->chunk, c->J - s0);
         FrameArgs a = base_args(c);
         a.frames = c->dm_frames + s0;
         a.e_part = c->e_tmp + (size_t)s0 * ncb;
+        if (c->sub_frac) {
+            const size_t knn = (size_t)c->K * c->N * c->N;
+            LAUNCH(c, PTYCHO_K_OTHER, (k_sub_ramp<<<dim3(nf, (unsigned)((knn + 255) / 256)), 256, 0, c->stream>>>(
+                                           c->sub_Pj, c->sub_FP, c->sub_frac, c->dm_frames + s0, c->K, c->N, 1.0f / ((float)c->N * (float)c->N))));
+            plain_fft2(c, c->sub_Pj, nf * c->K, true);
+            a.Pj = c->sub_Pj;
+            passes(c, a, nf, RF_EXIT_PJ, CM_ERRONLY, -1);
+        } else
         passes(c, a, nf, RF_EXIT, CM_ERRONLY, -1);
     }
     LAUNCH(c, PTYCHO_K_OTHER, (k_sum_error<<<kErrBlocks, 1024, 0, c->stream>>>(c->e_tmp, (size_t)c->J * ncb, c->sc, c->scratch_d, c->err_part, c->err_ticket)));

@@ -884,6 +884,7 @@ def test_subpixel_positions_epie_minibatch(B, oracle_mod, n, h, side, step, k, d
         ro, rp = rel(g.fetch_object(), o.O), rel(g.fetch_probe(), o.P)
         assert ro < TOL_ITER * (it + 1) and rp < TOL_ITER * (it + 1), (it, ro, rp)
     assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+    assert np.isclose(g.eval_error(), o.eval_error(), rtol=2e-3)          # the data-fit error of the CURRENT O, P, shifted probes
     # the fractions matter at this tolerance: the ordinary path on the same input is far away
     z = B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(**par))
     z.iterate("EPIE_MB", 4)

@@ -513,19 +513,39 @@ __global__ void k_direction(float2* n, const float* __restrict__ d, size_t plane
 
 // LSQML cross term A12 = Re sum_j sum_r T(r) conj(dO[r_j+r]) O[r_j+r],  T = sum_k conj(P_k) dP_k.
 // grid (nframes, parts): block (f, p) sums every parts-th pixel group of frame f; part[f * parts + p].
-__global__ void k_lsq_cross(const float2* __restrict__ O, const float2* __restrict__ dO, int W,
-                            const float2* __restrict__ P, const float2* __restrict__ dPk, int K, int n,
+// T = sum_k conj(P_k) dP_k, the same for every frame of the batch: formed once (k_lsq_T), gathered by k_lsq_cross.
+__global__ void k_lsq_T(float2* __restrict__ T, const float2* __restrict__ P, const float2* __restrict__ dPk, int K, int nn) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= nn) return;
+    float2 tq = make_float2(0.f, 0.f);
+    for (int k = 0; k < K; ++k) tq = cadd(tq, cmulc(dPk[(size_t)k * nn + q], P[(size_t)k * nn + q]));
+    T[q] = tq;
+}
+__global__ void k_lsq_cross(const float2* __restrict__ O, const float2* __restrict__ dO, int W, const float2* __restrict__ T, int n, int log2n,
                             const YX* __restrict__ pos, const int* __restrict__ frames, double* part) {
     const YX p0 = pos[frames[blockIdx.x]];
-    const int nn = n * n;
+    const int nn = n * n, stride = gridDim.y * blockDim.x;
+    const size_t base = (size_t)p0.y * W + p0.x;
     double acc = 0.0;
-    for (int q = blockIdx.y * blockDim.x + threadIdx.x; q < nn; q += gridDim.y * blockDim.x) {
-        const int y = q / n, x = q % n;
-        float2 tq = make_float2(0.f, 0.f);
-        for (int k = 0; k < K; ++k) tq = cadd(tq, cmulc(dPk[(size_t)k * nn + q], P[(size_t)k * nn + q]));
-        const size_t o = (size_t)(p0.y + y) * W + p0.x + x;
-        const float2 s = cmulc(O[o], dO[o]);           // conj(dO) O
-        acc += (double)(tq.x * s.x - tq.y * s.y);
+    int q = blockIdx.y * blockDim.x + threadIdx.x;
+    for (; q + 3 * stride < nn; q += 4 * stride) {          // four gathers in flight (n is a power of two: no division)
+        float2 t[4], o[4], d[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int qq = q + u * stride;
+            const size_t i = base + (size_t)(qq >> log2n) * W + (qq & (n - 1));
+            t[u] = __ldg(T + qq); o[u] = __ldg(O + i); d[u] = __ldg(dO + i);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const float2 s = cmulc(o[u], d[u]);            // conj(dO) O
+            acc += (double)(t[u].x * s.x - t[u].y * s.y);
+        }
+    }
+    for (; q < nn; q += stride) {
+        const size_t i = base + (size_t)(q >> log2n) * W + (q & (n - 1));
+        const float2 s = cmulc(O[i], dO[i]);
+        acc += (double)(T[q].x * s.x - T[q].y * s.y);
     }
     __shared__ double sa[32];
     for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);

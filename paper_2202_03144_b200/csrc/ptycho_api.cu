@@ -71,6 +71,7 @@ struct ptycho_ctx {
     int* mega_ctr = nullptr;                   // device: [head | pad to 64 ints | cnt1[J] | cnt2[J] | cnt3[J]]
     float* p2 = nullptr;                       // |P|^2 of the current probe (d_O gather, dm_det.cuh)
     float* wO = nullptr;                       // LSQML_PF: sum_j w_j canvas (the a_j w_j canvas reuses dO)
+    float2* lsqT = nullptr;                    // LSQML: sum_k conj(P_k) dP_k of the current batch (k_lsq_T)
     double* pf_part = nullptr; float2* pf_ab = nullptr;   // LSQML_PF: per-frame partial sums (J x NCB x 5) and steps (J)
     double* err_part = nullptr; unsigned int* err_ticket = nullptr;   // k_sum_error: per-CTA pieces and the finishing ticket
     int* dm_stat = nullptr;                    // [0] frames inside the power bound in the previous DM iteration, [1] running count
@@ -262,6 +263,7 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
     c->partO = w.take<double>(2 * kRedBlocks);
     c->partP = w.take<double>(2 * kRedBlocks);
     c->partX = w.take<double>((size_t)c->J * kCrossParts);
+    c->lsqT = w.take<float2>(nn);
     c->scratch_d = w.take<double>(kRedBlocks);
     c->err_part = w.take<double>(kErrBlocks);
     c->err_ticket = w.take<unsigned int>(1);
@@ -624,7 +626,9 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
         }
         if (lsq) {
             if (upd) {
-                LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_cross<<<dim3(b1 - b0, kCrossParts), 256, 0, c->stream>>>(c->O, c->nO, c->W, c->P, c->nP, c->K, c->N, c->pos,
+                const int log2n = c->N == 64 ? 6 : c->N == 128 ? 7 : c->N == 256 ? 8 : 9;
+                LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_T<<<(unsigned)((nn + 255) / 256), 256, 0, c->stream>>>(c->lsqT, c->P, c->nP, c->K, (int)nn)));
+                LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_cross<<<dim3(b1 - b0, kCrossParts), 256, 0, c->stream>>>(c->O, c->nO, c->W, c->lsqT, c->N, log2n, c->pos,
                                                                                         c->mb_frames + b0, c->partX)));
             }
             LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_solve<<<1, 256, 0, c->stream>>>(c->partO, gO, c->partP, upd ? gP : 0, c->partX, upd ? (b1 - b0) * kCrossParts : 0,

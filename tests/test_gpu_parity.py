@@ -911,3 +911,82 @@ def test_subpixel_zero_fractions_reproduce_the_ordinary_path(B):
     with pytest.raises(B.PtychoError):
         B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(subpixel_yx=np.zeros((len(s.pos), 2), np.float32), deterministic=1))
     g.destroy(); z.destroy()
+
+
+# ------------------------------------------------------------- degenerate and extreme inputs (task brief: "the degenerate cases the method has")
+def _scan_from(obj, probe, pos, dtype=np.float32, peak=None, seed=3):
+    """Intensities of an arbitrary (object, probe, positions) through the package's seeded generator."""
+    _, inten, _ = synth.simulate(obj, probe, np.asarray(pos, np.int32), peak, seed, dtype, 2)
+    return inten
+
+
+@pytest.mark.parametrize("alg", ["DM", "EPIE_MB", "LSQML"])
+def test_single_frame_on_an_object_of_exactly_the_frame_size(B, oracle_mod, alg):
+    """J = 1 and H = W = N: one wave (a ragged one: M = 6 slots per item), one minibatch of one frame, every object pixel covered
+    once, the position (0, 0) the only legal one."""
+    n = 64
+    obj = synth.make_object(n, n, 8)
+    probe = synth.probe_disk(n, n * 0.3125)[None]
+    pos = np.zeros((1, 2), np.int32)
+    inten = _scan_from(obj, probe, pos)
+    par = dict(batch_size=1, pbound=0.0)
+    obj0 = np.ones_like(obj)
+    o = oracle_mod.Oracle(obj0, probe, pos, inten, par)
+    g = B.Ptycho(obj0, probe, pos, inten, B.default_params(**par))
+    for it in range(4):
+        o.iterate(alg, 1)
+        g.iterate(alg, 1)
+        assert rel(g.fetch_object(), o.O) < TOL_RUN and rel(g.fetch_probe(), o.P) < TOL_RUN, (alg, it)
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3, atol=1e-12)
+    with pytest.raises(B.PtychoError):                      # (0, 1) would hang over the edge: no wrap-around, no clamping
+        B.Ptycho(obj0, probe, np.array([[0, 1]], np.int32), inten)
+    g.destroy()
+
+
+@pytest.mark.parametrize("alg", ["DM", "LSQML", "EPIE_MB"])
+def test_eight_probe_modes(B, oracle_mod, alg):
+    """K = PTYCHO_MAX_MODES = 8 at N = 64 (the column pass loops the modes and parks their spectra in S); K = 9 is refused."""
+    n, K = 64, 8
+    rng = np.random.default_rng(23)
+    base = synth.probe_disk(n, n * 0.3125)
+    yy, xx = np.mgrid[0:n, 0:n] - n / 2
+    modes = np.stack([base * (1 + 0.0 * yy) if k == 0 else base * (np.cos(0.07 * k * yy) + 1j * np.sin(0.05 * k * xx)) * 0.6 ** k for k in range(K)])
+    obj = synth.make_object(170, 170, 9)
+    pos = synth.raster_positions(5, 5, 21, (8, 8), jitter=2, seed=4)
+    inten = _scan_from(obj, modes, pos, dtype=np.uint16, peak=2e4)
+    par = dict(batch_size=9, pbound=0.2)
+    probe0 = (modes * (1 + 0.02 * (rng.standard_normal(modes.shape) + 1j * rng.standard_normal(modes.shape)))).astype(np.complex64)
+    obj0 = np.ones_like(obj)
+    o = oracle_mod.Oracle(obj0, probe0, pos, inten, par)
+    g = B.Ptycho(obj0, probe0, pos, inten, B.default_params(**par))
+    o.iterate(alg, 3); g.iterate(alg, 3)
+    assert rel(g.fetch_object(), o.O) < TOL_RUN and rel(g.fetch_probe(), o.P) < TOL_RUN
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+    g.destroy()
+    with pytest.raises(B.PtychoError):
+        B.Ptycho(obj0, np.concatenate([probe0, probe0[:1]]), pos, inten)
+
+
+@pytest.mark.parametrize("alg,dtype", [("DM", np.uint16), ("EPIE_MB", np.uint16), ("DM", np.float32), ("LSQML", np.float32)])
+def test_dead_frames_and_frames_on_every_border(B, oracle_mod, alg, dtype):
+    """One frame with every pixel masked (R3: it must pass through the cycle unchanged and add nothing to the error), one frame
+    with all-zero counts (sqrt I = 0 everywhere: the projection sends the wave to zero), frames flush with all four borders of
+    the object, and a relaxed projection whose bound some frames are inside of from the first iteration."""
+    n, h = 64, 150
+    obj = synth.make_object(h, h, 10)
+    probe = synth.probe_zone(n, n * 0.3125)[None]
+    pos = np.array([[0, 0], [0, h - n], [h - n, 0], [h - n, h - n], [0, 40], [43, 0], [h - n, 37], [41, h - n], [40, 40], [50, 30], [30, 52]], np.int32)
+    inten = _scan_from(obj, probe, pos, dtype=dtype, peak=5e3)
+    inten[8] = 65535 if dtype == np.uint16 else -1.0         # fully masked frame
+    inten[9] = 0                                             # dead frame
+    par = dict(batch_size=4, pbound=0.3)
+    obj0 = np.ones_like(obj)
+    o = oracle_mod.Oracle(obj0, probe, pos, inten, par)
+    g = B.Ptycho(obj0, probe, pos, inten, B.default_params(**par))
+    for it in range(5):
+        o.iterate(alg, 1); g.iterate(alg, 1)
+        assert rel(g.fetch_object(), o.O) < TOL_RUN and rel(g.fetch_probe(), o.P) < TOL_RUN, (alg, it)
+    if alg == "DM":
+        assert rel(g.fetch_exit_waves(), o.psi) < TOL_RUN
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+    g.destroy()

@@ -1,4 +1,4 @@
-"""ORACLE (test infrastructure, like the rest of this package): ePIE-minibatch with SUB-PIXEL scan positions.
+"""ORACLE (test infrastructure, like the rest of this package): ePIE-minibatch and the LSQML-style joint step with SUB-PIXEL scan positions.
 
 SURVEY.md 8(f) f4 / R10 ("sub-pixel shifts = NEXT f4").  PAPER.md does not say how ptychopy treats the fractional
 part of a position; reading R28 of DESIGN.md fixes it as the textbook rule -- the Fourier shift theorem applied to
@@ -34,14 +34,21 @@ def shift(f: np.ndarray, dy: float, dx: float) -> np.ndarray:
     return np.fft.ifft2(np.fft.fft2(np.asarray(f, np.complex128)) * ramp)
 
 
-def epie_mb_step(O, P, pos, frac, inten, frames, update_probe, par):
-    """One minibatch step over `frames` (in place on O, P; fp64).  Returns the batch's error term sum (sqrt I - A)^2."""
+def epie_mb_step(O, P, pos, frac, inten, frames, update_probe, par, lsqml=False, steps_out=None):
+    """One minibatch step over `frames` (in place on O, P; fp64).  Returns the batch's error term sum (sqrt I - A)^2.
+    lsqml = True: the joint step (a, b) of R9 instead of the fixed (alpha_O, alpha_P), its five sums taken from their per-frame
+    DEFINITIONS with the shifted probes and the shifted probe direction:
+        u_jk = P_jk dO_j,   v_jk = S_{delta_j}[dP_k] O_j   (O_j the object BEFORE the step),   c = chi_jk
+        A11 = sum |u|^2, A22 = sum |v|^2, A12 = Re sum conj(u) v, b1 = Re sum conj(u) c, b2 = Re sum conj(v) c
+        l = 1 + lambda;  probe updated: (a, b) solve [[A11 l, A12], [A12, A22 l]] (a, b)^T = (b1, b2)^T (0, 0 if singular);
+        otherwise a = b1 / (A11 l), b = 0      -- exactly the rule of orc_minibatch_step."""
     K, n = P.shape[0], P.shape[-1]
     nO = np.zeros_like(O)
     dO = np.zeros(O.shape)
     nP = np.zeros_like(P)
     dP = np.zeros((n, n))
     err = 0.0
+    kept = []
     for j in frames:
         y, x = int(pos[j, 0]), int(pos[j, 1])
         dy, dx = float(frac[j, 0]), float(frac[j, 1])
@@ -52,6 +59,8 @@ def epie_mb_step(O, P, pos, frac, inten, frames, update_probe, par):
         Phi2, e = modulus_project(Phi, inten[j], par["pbound"])
         err += e
         chi = np.fft.ifft2(Phi2) - psi
+        if lsqml:
+            kept.append((Pj, chi, Oj.copy()))
         nO[y:y + n, x:x + n] += np.sum(np.conj(Pj) * chi, axis=0)
         dO[y:y + n, x:x + n] += np.sum(np.abs(Pj) ** 2, axis=0)
         nP += shift(np.conj(Oj)[None] * chi, -dy, -dx)
@@ -59,9 +68,30 @@ def epie_mb_step(O, P, pos, frac, inten, frames, update_probe, par):
     maxP = float(np.max(np.sum(np.abs(P) ** 2, axis=0)))
     dirO = nO / (dO + par["delta_obj"] * maxP)
     dirP = nP / (dP + par["delta_probe"] * float(np.max(dP)))[None]
-    O += par["alpha_obj"] * dirO
+    sa, sb = par["alpha_obj"], (par["alpha_probe"] if update_probe else 0.0)
+    if lsqml:
+        A11 = A22 = A12 = b1 = b2 = 0.0
+        for j, (Pj, chi, Oj) in zip(frames, kept):
+            y, x = int(pos[j, 0]), int(pos[j, 1])
+            u = Pj * dirO[None, y:y + n, x:x + n]
+            v = shift(dirP, float(frac[j, 0]), float(frac[j, 1])) * Oj[None]
+            A11 += float(np.sum(np.abs(u) ** 2)); A22 += float(np.sum(np.abs(v) ** 2))
+            A12 += float(np.sum((np.conj(u) * v).real))
+            b1 += float(np.sum((np.conj(u) * chi).real)); b2 += float(np.sum((np.conj(v) * chi).real))
+        l = 1.0 + par["lsq_lambda"]
+        if not update_probe:
+            sa, sb = (b1 / (A11 * l) if A11 > 0 else 0.0), 0.0
+        else:
+            det = A11 * l * A22 * l - A12 * A12
+            if not (det > 0) or not np.isfinite(det):
+                sa, sb = 0.0, 0.0
+            else:
+                sa, sb = (b1 * A22 * l - A12 * b2) / det, (A11 * l * b2 - A12 * b1) / det
+    O += sa * dirO
     if update_probe:
-        P += par["alpha_probe"] * dirP
+        P += sb * dirP
+    if steps_out is not None:
+        steps_out.append((sa, sb))
     return err
 
 
@@ -83,6 +113,7 @@ class SubpixelOracle:
         self.sum_I = float(np.sum(it[it >= 0]))
         self.t = 0
         self.err: list[float] = []
+        self.steps: list[tuple[float, float]] = []
 
     def eval_error(self) -> float:
         """C3 with the shifted probes: sum_j sum_q (sqrt I_j - A_j)^2 / sum I over unmasked pixels, A_j^2 = sum_k |F[P_jk O_j]|^2."""
@@ -93,13 +124,14 @@ class SubpixelOracle:
             num += modulus_project(Phi, self.inten[j], 0.0)[1]
         return num / (self.sum_I if self.sum_I > 0 else 1.0)
 
-    def iterate(self, n_iters: int = 1):
+    def iterate(self, n_iters: int = 1, alg: str = "EPIE_MB"):
+        assert alg in ("EPIE_MB", "LSQML")
         p = self.par
         for _ in range(n_iters):
             upd = self.t >= p["probe_start"]
             num = 0.0
             for fr in batches(len(self.pos), p["batch_size"], p["batch_order"]):
-                num += epie_mb_step(self.O, self.P, self.pos, self.frac, self.inten, fr, upd, p)
+                num += epie_mb_step(self.O, self.P, self.pos, self.frac, self.inten, fr, upd, p, lsqml=alg == "LSQML", steps_out=self.steps)
             self.err.append(num / (self.sum_I if self.sum_I > 0 else 1.0))
             self.t += 1
         return self

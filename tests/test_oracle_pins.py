@@ -654,3 +654,48 @@ def test_subpixel_positions_matter_and_the_true_ones_fit_best(oracle_mod):
     assert z.err[0] > 1e-4
     z2 = subpixel.SubpixelOracle(s.obj_true, s.probe_true, s.pos, 0 * frac, inten)      # eval_error with zero fractions = the C oracle's
     assert np.isclose(z2.eval_error(), oracle_mod.Oracle(s.obj_true, s.probe_true, s.pos, inten).eval_error(), rtol=1e-10) and z2.eval_error() > 1e-4
+
+
+@pytest.mark.parametrize("k,probe_start", [(1, 0), (3, 1)])
+def test_subpixel_lsqml_zero_shift_is_the_ordinary_joint_step(oracle_mod, k, probe_start):
+    """The LSQML-style joint step of oracle/subpixel.py with every fraction zero: objects, probes, error history AND the step
+    lengths (a, b) of every batch must be those of orc_minibatch_step(LSQML), with and without the probe update."""
+    from oracle import subpixel
+    s = synth.make_custom(16, 44, 4, 6, k=k, seed=21, jitter=1)
+    par = dict(batch_size=6, probe_start=probe_start, pbound=0.0, lsq_lambda=0.1)
+    O0 = s.obj0 * (1 + 0.05 * crandn(*s.obj0.shape))
+    o = oracle_mod.Oracle(O0, s.probe0, s.pos, s.intensities, par).iterate("LSQML", 3)
+    q = subpixel.SubpixelOracle(O0, s.probe0, s.pos, np.zeros((len(s.pos), 2)), s.intensities, par).iterate(3, "LSQML")
+    assert rel(q.O, o.O) < 1e-10 and rel(q.P, o.P) < 1e-10
+    assert np.allclose(q.steps, o.steps, rtol=1e-9, atol=1e-14) and np.allclose(q.err, o.err, rtol=1e-10)
+    assert any(b != 0 for _, b in q.steps) and (probe_start == 0 or q.steps[0][1] == 0.0)
+
+
+def test_subpixel_lsqml_step_minimises_the_linearised_residual(oracle_mod):
+    """With fractions: the (a, b) applied must be the Tikhonov-regularised least-squares solution of
+    sum_jk || chi_jk - a P_jk dO_j - b S_delta_j[dP_k] O_j ||^2, found here by numpy's lstsq on the stacked real system."""
+    from oracle import subpixel
+    s = synth.make_custom(16, 44, 3, 7, k=2, seed=22, jitter=1)
+    rng = np.random.default_rng(4)
+    frac = rng.uniform(0, 1, (len(s.pos), 2))
+    par = dict(oracle_mod.DEFAULTS, batch_size=0, probe_start=0, lsq_lambda=0.0)
+    O0 = (s.obj0 * (1 + 0.05 * crandn(*s.obj0.shape))).astype(np.complex128)
+    P0 = np.array(s.probe0, np.complex128)
+    # the directions, from one ePIE-type step with unit steps and the probe updated: dO = O' - O, dP = P' - P
+    Oe, Pe = O0.copy(), P0.copy()
+    subpixel.epie_mb_step(Oe, Pe, s.pos, frac, s.intensities, np.arange(len(s.pos)), True, dict(par, alpha_obj=1.0, alpha_probe=1.0))
+    dO, dP = Oe - O0, Pe - P0
+    n = 16
+    cols_u, cols_v, rhs = [], [], []
+    for j, (y, x) in enumerate(s.pos):
+        Pj = subpixel.shift(P0, *frac[j]); Oj = O0[y:y + n, x:x + n]
+        psi = Pj * Oj[None]
+        chi = np.fft.ifft2(oracle_mod.modulus_project(np.fft.fft2(psi), s.intensities[j], 0.0)[0]) - psi
+        cols_u.append((Pj * dO[None, y:y + n, x:x + n]).ravel()); cols_v.append((subpixel.shift(dP, *frac[j]) * Oj[None]).ravel()); rhs.append(chi.ravel())
+    u, v, c = np.concatenate(cols_u), np.concatenate(cols_v), np.concatenate(rhs)
+    A = np.stack([np.concatenate([u.real, u.imag]), np.concatenate([v.real, v.imag])], 1)
+    ab = np.linalg.lstsq(A, np.concatenate([c.real, c.imag]), rcond=None)[0]
+    Ol, Pl, steps = O0.copy(), P0.copy(), []
+    subpixel.epie_mb_step(Ol, Pl, s.pos, frac, s.intensities, np.arange(len(s.pos)), True, par, lsqml=True, steps_out=steps)
+    assert np.allclose(steps[0], ab, rtol=1e-8)
+    assert rel(Ol, O0 + ab[0] * dO) < 1e-12 and rel(Pl, P0 + ab[1] * dP) < 1e-12

@@ -556,13 +556,14 @@ __global__ void k_lsq_cross(const float2* __restrict__ O, const float2* __restri
 
 // a11: sum the partials in a fixed order (thread-strided, then a shared-memory tree: the same order
 // on every run), solve the 2x2 system (R9), publish the steps.  One CTA of 256 threads.
+// partA22 != nullptr (sub-pixel positions, R28): A22 comes from the per-frame sums of k_lsq_cross_pj instead of the canvas closed form.
 __global__ void k_lsq_solve(const double* partO, int nO, const double* partP, int nP, const double* partX, int nX,
-                            float lambda, int update_probe, Scalars* sc, double* steps_out) {
+                            float lambda, int update_probe, Scalars* sc, double* steps_out, const double* partA22 = nullptr) {
     __shared__ double sh[5][256];
     double v[5] = {0, 0, 0, 0, 0};                       // A11, b1, A22, b2, A12
     for (int i = threadIdx.x; i < nO; i += 256) { v[0] += partO[2 * i]; v[1] += partO[2 * i + 1]; }
-    for (int i = threadIdx.x; i < nP; i += 256) { v[2] += partP[2 * i]; v[3] += partP[2 * i + 1]; }
-    for (int i = threadIdx.x; i < nX; i += 256) v[4] += partX[i];
+    for (int i = threadIdx.x; i < nP; i += 256) { if (!partA22) v[2] += partP[2 * i]; v[3] += partP[2 * i + 1]; }
+    for (int i = threadIdx.x; i < nX; i += 256) { v[4] += partX[i]; if (partA22) v[2] += partA22[i]; }
     for (int q = 0; q < 5; ++q) sh[q][threadIdx.x] = v[q];
     __syncthreads();
     for (int w = 128; w > 0; w >>= 1) {
@@ -845,6 +846,34 @@ __global__ void k_sub_acc(float2* __restrict__ nPF, const float2* __restrict__ G
         acc = cadd(acc, cmulc(G[(size_t)s * K * nn + i], shift_ramp(ky, kx, n, frac[2 * f], frac[2 * f + 1])));   // G conj(ramp)
     }
     nPF[i] = acc;
+}
+// LSQML with sub-pixel positions: the two sums that have no canvas closed form, from their per-frame definitions.
+//   A22 = sum_j sum_k || dP_jk O_j ||^2,   A12 = Re sum_j sum_k conj(P_jk dO_j) (dP_jk O_j),   dP_jk = S_delta_j[dP_k]
+// Pj, dPj: this launch's per-frame probes and probe directions (nframes x K x n x n).  grid (nframes, parts); fixed order, double.
+__global__ void k_lsq_cross_pj(const float2* __restrict__ O, const float2* __restrict__ dO, int W, const float2* __restrict__ Pj,
+                               const float2* __restrict__ dPj, int K, int n, int log2n, const YX* __restrict__ pos, const int* __restrict__ frames,
+                               double* partX, double* partA22) {
+    const YX p0 = pos[frames[blockIdx.x]];
+    const int nn = n * n, stride = gridDim.y * blockDim.x;
+    const size_t base = (size_t)p0.y * W + p0.x, fr = (size_t)blockIdx.x * K * nn;
+    double a12 = 0.0, a22 = 0.0;
+    for (int q = blockIdx.y * blockDim.x + threadIdx.x; q < nn; q += stride) {
+        const size_t i = base + (size_t)(q >> log2n) * W + (q & (n - 1));
+        const float2 o = __ldg(O + i), d = __ldg(dO + i);
+        for (int k = 0; k < K; ++k) {
+            const float2 u = cmul(Pj[fr + (size_t)k * nn + q], d), v = cmul(dPj[fr + (size_t)k * nn + q], o);
+            a22 += (double)(v.x * v.x + v.y * v.y);
+            a12 += (double)(u.x * v.x + u.y * v.y);
+        }
+    }
+    __shared__ double sa[32], sb[32];
+    for (int s = 16; s > 0; s >>= 1) { a12 += __shfl_xor_sync(0xffffffffu, a12, s); a22 += __shfl_xor_sync(0xffffffffu, a22, s); }
+    if ((threadIdx.x & 31) == 0) { sa[threadIdx.x >> 5] = a12; sb[threadIdx.x >> 5] = a22; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)blockDim.x / 32; ++w) { a12 += sa[w]; a22 += sb[w]; }
+        partX[blockIdx.x * gridDim.y + blockIdx.y] = a12; partA22[blockIdx.x * gridDim.y + blockIdx.y] = a22;
+    }
 }
 // dst = src * s (element-wise)
 __global__ void k_scale_to(float2* __restrict__ dst, const float2* __restrict__ src, size_t n, float s) {

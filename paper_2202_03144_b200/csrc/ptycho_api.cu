@@ -95,6 +95,8 @@ struct ptycho_ctx {
     // per-frame probes of one launch
     float* sub_frac = nullptr;
     float2 *sub_FP = nullptr, *sub_nPF = nullptr, *sub_Pj = nullptr;
+    float2 *sub_FdP = nullptr, *sub_dPj = nullptr;   // LSQML: F[dP] and the per-frame shifted probe directions of one launch
+    double* partA22 = nullptr;
     std::vector<float> sub_frac_h;
     // shard of a scan held by several GPUs (ptycho_shard_begin / _end): positions of the other shards' frames over our rows
     std::vector<int32_t> foreign_h;
@@ -284,6 +286,9 @@ size_t layout(ptycho_ctx* c, void* base, bool copy_I) {
         c->sub_FP = w.take<float2>(knn);
         c->sub_nPF = w.take<float2>(knn);
         c->sub_Pj = w.take<float2>((size_t)c->chunk * knn);
+        c->sub_FdP = w.take<float2>(knn);
+        c->sub_dPj = w.take<float2>((size_t)c->chunk * knn);
+        c->partA22 = w.take<double>((size_t)c->J * kCrossParts);
     }
     if (c->streaming) {
         c->stage_frames = std::max(1, std::min(c->J, (int)((64ull << 20) / (nn * (c->itype == PTYCHO_I_U16 ? 2 : 4)))));
@@ -624,7 +629,28 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
             c->n_steps += b1 - b0;
             continue;
         }
-        if (lsq) {
+        if (lsq && c->sub_frac && upd) {
+            // Sub-pixel positions: A22 and A12 from their per-frame definitions (R28).  F[dP] once, then per launch the frames'
+            // shifted probes (again: sub_Pj was used up by the cycle) and shifted probe directions, and the per-frame gather.
+            const size_t knn = nn * c->K;
+            const float inv_n2 = 1.0f / ((float)c->N * (float)c->N);
+            const int log2n = c->N == 64 ? 6 : c->N == 128 ? 7 : c->N == 256 ? 8 : 9;
+            CU(cudaMemcpyAsync(c->sub_FdP, c->nP, knn * 8, cudaMemcpyDeviceToDevice, c->stream));
+            plain_fft2(c, c->sub_FdP, c->K, false);
+            for (int s0 = b0; s0 < b1; s0 += c->chunk) {
+                const int nf = std::min(c->chunk, b1 - s0);
+                const dim3 gr(nf, (unsigned)((knn + 255) / 256));
+                LAUNCH(c, PTYCHO_K_OTHER, (k_sub_ramp<<<gr, 256, 0, c->stream>>>(c->sub_Pj, c->sub_FP, c->sub_frac, c->mb_frames + s0, c->K, c->N, inv_n2)));
+                LAUNCH(c, PTYCHO_K_OTHER, (k_sub_ramp<<<gr, 256, 0, c->stream>>>(c->sub_dPj, c->sub_FdP, c->sub_frac, c->mb_frames + s0, c->K, c->N, inv_n2)));
+                plain_fft2(c, c->sub_Pj, nf * c->K, true);
+                plain_fft2(c, c->sub_dPj, nf * c->K, true);
+                LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_cross_pj<<<dim3(nf, kCrossParts), 256, 0, c->stream>>>(
+                                                c->O, c->nO, c->W, c->sub_Pj, c->sub_dPj, c->K, c->N, log2n, c->pos, c->mb_frames + s0,
+                                                c->partX + (size_t)(s0 - b0) * kCrossParts, c->partA22 + (size_t)(s0 - b0) * kCrossParts)));
+            }
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_solve<<<1, 256, 0, c->stream>>>(c->partO, gO, c->partP, gP, c->partX, (b1 - b0) * kCrossParts,
+                                                                            c->par.lsq_lambda, upd, c->sc, step_slot ? step_slot : c->scratch_d, c->partA22)));
+        } else if (lsq) {
             if (upd) {
                 const int log2n = c->N == 64 ? 6 : c->N == 128 ? 7 : c->N == 256 ? 8 : 9;
                 LAUNCH(c, PTYCHO_K_UPDATE, (k_lsq_T<<<(unsigned)((nn + 255) / 256), 256, 0, c->stream>>>(c->lsqT, c->P, c->nP, c->K, (int)nn)));
@@ -880,7 +906,7 @@ ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
     if (alg != PTYCHO_DM && c->par.deterministic) return fail(c, PTYCHO_EUNSUPPORTED, "deterministic mode covers DM only");
     if (alg == PTYCHO_DM && !c->psi) return fail(c, PTYCHO_ESTATE, "DM needs the exit-wave store (disable_dm was set)");
     if (c->par.shard_total_pos > 0) return fail(c, PTYCHO_ESTATE, "a shard is driven by ptycho_shard_begin / ptycho_shard_end");
-    if (c->sub_frac && alg != PTYCHO_EPIE_MB) return fail(c, PTYCHO_EUNSUPPORTED, "sub-pixel positions: PTYCHO_EPIE_MB only");
+    if (c->sub_frac && alg != PTYCHO_EPIE_MB && alg != PTYCHO_LSQML) return fail(c, PTYCHO_EUNSUPPORTED, "sub-pixel positions: PTYCHO_EPIE_MB and PTYCHO_LSQML only");
     if (c->streaming) {
         if (c->present == 0) return fail(c, PTYCHO_ESTATE, "no frame has been appended yet");
         if (alg == PTYCHO_DM && c->present < c->J) return fail(c, PTYCHO_ESTATE, "DM needs every frame (PAPER.md:58); append the rest first");

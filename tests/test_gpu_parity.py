@@ -890,11 +890,37 @@ def test_subpixel_positions_epie_minibatch(B, oracle_mod, n, h, side, step, k, d
     z.iterate("EPIE_MB", 4)
     assert rel(z.fetch_object(), o.O) > 50 * TOL_ITER
     z.destroy()
-    for alg in ("DM", "LSQML", "LSQML_PF"):                  # ePIE-minibatch only
+    for alg in ("DM", "LSQML_PF"):                           # ePIE-minibatch and LSQML only
         with pytest.raises(B.PtychoError):
             g.iterate(alg, 1)
     with pytest.raises(B.PtychoError):
         g.revised_waves(np.arange(2, dtype=np.int32))
+    g.destroy()
+
+
+@pytest.mark.parametrize("n,h,side,step,k,dtype,batch,probe_start", [
+    (64, 300, 6, 21, 1, np.float32, 9, 0),
+    (64, 300, 6, 21, 3, np.uint16, 12, 1),
+    (256, 600, 3, 90, 2, np.uint16, 0, 0)])
+def test_subpixel_positions_lsqml(B, oracle_mod, n, h, side, step, k, dtype, batch, probe_start):
+    """The LSQML-style joint step with fractional positions: A11, b1, b2 from the canvas closed forms (exact with shifted probes),
+    A22 and A12 from the per-frame gather with shifted probes and shifted probe directions.  Objects, probes, error history and the
+    step lengths (a, b) of every batch against oracle/subpixel.py."""
+    from oracle import subpixel
+    s = synth.make_custom(n, h, side, step, k=k, peak=2e4 if dtype == np.uint16 else None, dtype=dtype, jitter=2, seed=47,
+                          probe_kind="zone")
+    rng = np.random.default_rng(19)
+    frac = rng.uniform(0, 1, (len(s.pos), 2)).astype(np.float32)
+    par = dict(batch_size=batch, probe_start=probe_start, lsq_lambda=0.1)
+    o = subpixel.SubpixelOracle(s.obj0, s.probe0, s.pos, frac, s.intensities, par)
+    g = B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(subpixel_yx=frac, **par))
+    for it in range(3):
+        o.iterate(1, "LSQML")
+        g.iterate("LSQML", 1)
+        ro, rp = rel(g.fetch_object(), o.O), rel(g.fetch_probe(), o.P)
+        assert ro < TOL_ITER * (it + 1) and rp < TOL_ITER * (it + 1), (it, ro, rp)
+    assert np.allclose(g.fetch_steps(), np.array(o.steps), rtol=2e-3, atol=1e-6)
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
     g.destroy()
 
 

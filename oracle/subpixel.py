@@ -95,6 +95,38 @@ def epie_mb_step(O, P, pos, frac, inten, frames, update_probe, par, lsqml=False,
     return err
 
 
+def dm_iteration(O, P, psi, pos, frac, inten, eps_O, eps_P, update_probe, pbound):
+    """One DM iteration with sub-pixel positions, in place on O, P, psi (J, K, n, n); the steps of orc_dm_iteration (SURVEY 8(c)
+    "DM" 1-5; R4 lagged probe sums, R5 blends, R6) with P_jk = S_{delta_j}[P_k] in place of P_k and the probe term shifted back:
+        1  n_Pk += S_{-delta_j}[conj(O_j) psi_jk],  d_P += |O_j|^2                 (incoming psi, current O)
+        2  psi_O = P_jk O_j;  Phi = F[2 psi_O - psi_j];  Phi' = Pi_M Phi;  psi_F = F^-1 Phi'
+        3  psi_j <- psi_j + psi_F - psi_O
+        4  n_O += sum_k conj(P_jk) psi_jk,  d_O += sum_k |P_jk|^2                  (new psi, current P)
+        5  O <- (n_O + eps_O O)/(d_O + eps_O);  P_k <- (n_Pk + eps_P P_k)/(d_P + eps_P) if the probe is updated
+    Returns the error term sum.  (d_P is not shifted, as in the minibatch step: a shift does not commute with the multiplication
+    by |O_j|^2, so with the probe updated the ground truth is a fixed point only up to the variation of |O_j|^2 over a pixel;
+    with the probe frozen it is one exactly -- pinned.)"""
+    K, n = P.shape[0], P.shape[-1]
+    nP = np.zeros_like(P); dP = np.zeros((n, n)); nO = np.zeros_like(O); dO = np.zeros(O.shape)
+    for j, (y, x) in enumerate(pos):
+        Oj = O[y:y + n, x:x + n]
+        nP += shift(np.conj(Oj)[None] * psi[j], -float(frac[j, 0]), -float(frac[j, 1]))
+        dP += np.abs(Oj) ** 2
+    err = 0.0
+    for j, (y, x) in enumerate(pos):
+        Pj = shift(P, float(frac[j, 0]), float(frac[j, 1]))
+        psiO = Pj * O[None, y:y + n, x:x + n]
+        Phi2, e = modulus_project(np.fft.fft2(2 * psiO - psi[j]), inten[j], pbound)
+        err += e
+        psi[j] = psi[j] + np.fft.ifft2(Phi2) - psiO
+        nO[y:y + n, x:x + n] += np.sum(np.conj(Pj) * psi[j], axis=0)
+        dO[y:y + n, x:x + n] += np.sum(np.abs(Pj) ** 2, axis=0)
+    O[...] = (nO + eps_O * O) / (dO + eps_O)
+    if update_probe:
+        P[...] = (nP + eps_P * P) / (dP + eps_P)[None]
+    return err
+
+
 class SubpixelOracle:
     """State and sequencing (batches R8, probe_start, error history C3), mirroring oracle.Oracle for EPIE_MB."""
 
@@ -114,6 +146,10 @@ class SubpixelOracle:
         self.t = 0
         self.err: list[float] = []
         self.steps: list[tuple[float, float]] = []
+        self.psi = None
+        d = self.par["delta_blend"]                                      # R5: fixed at init, from the unshifted probe
+        self.eps_O = d * float(np.max(np.sum(np.abs(self.P) ** 2, axis=0)))
+        self.eps_P = d * len(self.pos) * float(np.max(np.abs(self.O) ** 2))
 
     def eval_error(self) -> float:
         """C3 with the shifted probes: sum_j sum_q (sqrt I_j - A_j)^2 / sum I over unmasked pixels, A_j^2 = sum_k |F[P_jk O_j]|^2."""
@@ -125,11 +161,20 @@ class SubpixelOracle:
         return num / (self.sum_I if self.sum_I > 0 else 1.0)
 
     def iterate(self, n_iters: int = 1, alg: str = "EPIE_MB"):
-        assert alg in ("EPIE_MB", "LSQML")
+        assert alg in ("EPIE_MB", "LSQML", "DM")
         p = self.par
+        n = self.P.shape[-1]
         for _ in range(n_iters):
             upd = self.t >= p["probe_start"]
             num = 0.0
+            if alg == "DM":
+                if self.psi is None:                                     # R4: psi_j = P_jk O_j before the first DM iteration
+                    self.psi = np.stack([shift(self.P, *self.frac[j]) * self.O[None, y:y + n, x:x + n] for j, (y, x) in enumerate(self.pos)])
+                num = dm_iteration(self.O, self.P, self.psi, self.pos, self.frac, self.inten, self.eps_O, self.eps_P, upd, p["pbound"])
+                self.err.append(num / (self.sum_I if self.sum_I > 0 else 1.0))
+                self.t += 1
+                continue
+            self.psi = None
             for fr in batches(len(self.pos), p["batch_size"], p["batch_order"]):
                 num += epie_mb_step(self.O, self.P, self.pos, self.frac, self.inten, fr, upd, p, lsqml=alg == "LSQML", steps_out=self.steps)
             self.err.append(num / (self.sum_I if self.sum_I > 0 else 1.0))

@@ -699,3 +699,35 @@ def test_subpixel_lsqml_step_minimises_the_linearised_residual(oracle_mod):
     subpixel.epie_mb_step(Ol, Pl, s.pos, frac, s.intensities, np.arange(len(s.pos)), True, par, lsqml=True, steps_out=steps)
     assert np.allclose(steps[0], ab, rtol=1e-8)
     assert rel(Ol, O0 + ab[0] * dO) < 1e-12 and rel(Pl, P0 + ab[1] * dP) < 1e-12
+
+
+def test_subpixel_dm_pins(oracle_mod):
+    """DM with sub-pixel positions (oracle/subpixel.py dm_iteration): zero fractions = orc_dm_iteration (K = 2, relaxed projection,
+    probe update from iteration 1, exit waves included); a common shift with the probe frozen = the ordinary DM run with the
+    pre-shifted probe; data simulated at fractional positions keep the ground truth fixed with zero error (probe frozen), and do not
+    when the fractions are dropped."""
+    from oracle import subpixel
+    s = synth.make_custom(16, 44, 4, 6, k=2, peak=3e3, dtype=np.uint16, seed=31, jitter=1)
+    par = dict(probe_start=1, pbound=0.4)
+    O0 = s.obj0 * (1 + 0.05 * crandn(*s.obj0.shape))
+    o = oracle_mod.Oracle(O0, s.probe0, s.pos, s.intensities, par).iterate("DM", 4)
+    q = subpixel.SubpixelOracle(O0, s.probe0, s.pos, np.zeros((len(s.pos), 2)), s.intensities, par).iterate(4, "DM")
+    assert rel(q.O, o.O) < 1e-11 and rel(q.P, o.P) < 1e-11 and rel(q.psi, o.psi) < 1e-11 and np.allclose(q.err, o.err, rtol=1e-10)
+    d = (0.4, 0.75)
+    frac = np.tile(np.array(d), (len(s.pos), 1))
+    Ps = subpixel.shift(s.probe0, *d)
+    frozen = dict(probe_start=10 ** 9, pbound=0.0)
+    o = oracle_mod.Oracle(O0, Ps, s.pos, s.intensities, frozen)
+    q = subpixel.SubpixelOracle(O0, s.probe0, s.pos, frac, s.intensities, frozen)
+    q.eps_O = o.eps_O                                                       # (R5 takes eps_O from the probe it is given: matched)
+    o.iterate("DM", 3); q.iterate(3, "DM")
+    assert rel(q.O, o.O) < 1e-11 and rel(q.psi, o.psi) < 1e-11
+    s1 = synth.make_custom(16, 44, 4, 6, k=1, seed=9, jitter=1)
+    rng = np.random.default_rng(3)
+    fr = rng.uniform(0, 1, (len(s1.pos), 2))
+    inten = np.stack([np.abs(np.fft.fft2(subpixel.shift(s1.probe_true, *fr[j])[0] * s1.obj_true[y:y + 16, x:x + 16])) ** 2
+                      for j, (y, x) in enumerate(s1.pos)]).astype(np.float32)
+    q = subpixel.SubpixelOracle(s1.obj_true, s1.probe_true, s1.pos, fr, inten, dict(probe_start=10 ** 9)).iterate(2, "DM")
+    assert q.err[-1] < 1e-12 and rel(q.O, s1.obj_true) < 1e-9           # (probe frozen: with d_P = sum |O_j|^2 unshifted the probe
+    z = subpixel.SubpixelOracle(s1.obj_true, s1.probe_true, s1.pos, 0 * fr, inten, dict(probe_start=10 ** 9)).iterate(2, "DM")
+    assert z.err[-1] > 1e-4                                                # update keeps the truth only approximately, see the docstring)

@@ -728,6 +728,6 @@ def test_subpixel_dm_pins(oracle_mod):
     inten = np.stack([np.abs(np.fft.fft2(subpixel.shift(s1.probe_true, *fr[j])[0] * s1.obj_true[y:y + 16, x:x + 16])) ** 2
                       for j, (y, x) in enumerate(s1.pos)]).astype(np.float32)
     q = subpixel.SubpixelOracle(s1.obj_true, s1.probe_true, s1.pos, fr, inten, dict(probe_start=10 ** 9)).iterate(2, "DM")
-    assert q.err[-1] < 1e-12 and rel(q.O, s1.obj_true) < 1e-9           # (probe frozen: with d_P = sum |O_j|^2 unshifted the probe
+    assert q.err[-1] < 1e-12 and rel(q.O, s1.obj_true) < 1e-6           # (probe frozen: with d_P = sum |O_j|^2 unshifted the probe
     z = subpixel.SubpixelOracle(s1.obj_true, s1.probe_true, s1.pos, 0 * fr, inten, dict(probe_start=10 ** 9)).iterate(2, "DM")
     assert z.err[-1] > 1e-4                                                # update keeps the truth only approximately, see the docstring)

@@ -103,9 +103,11 @@ typedef struct {
                                    the probe P_jk = S_d[P_k] = F^-1[F[P_k] exp(-2 pi i (k_y dy + k_x dx)/N)] (k signed, Nyquist = -N/2),
                                    the object patch stays at the integer corner; object sums use conj(P_jk), |P_jk|^2; the probe term
                                    conj(O_j) chi_jk is shifted back by S_{-d} before it is summed; d_P = sum_j |O_j|^2 and the object
-                                   regulariser delta_obj max_r sum_k |P_k|^2 use unshifted quantities.  PTYCHO_EPIE_MB and PTYCHO_LSQML (the joint step's
-                                   sums A22, A12 are then taken per frame with the shifted probe direction S_d[dP_k]); ptycho_iterate
-                                   returns PTYCHO_EUNSUPPORTED for the other algorithms, ptycho_revised_waves likewise (ptycho_eval_error works:
+                                   regulariser delta_obj max_r sum_k |P_k|^2 use unshifted quantities.  PTYCHO_EPIE_MB, PTYCHO_LSQML (the joint step's
+                                   sums A22, A12 are then taken per frame with the shifted probe direction S_d[dP_k]) and PTYCHO_DM (through
+                                   the three-pass kernels: the persistent DM kernel shares one probe among frames; the lagged probe
+                                   terms conj(O_j) psi_jk are shifted back like the minibatch ones); ptycho_iterate
+                                   returns PTYCHO_EUNSUPPORTED for PTYCHO_LSQML_PF, ptycho_revised_waves likewise (ptycho_eval_error works:
                                    the data-fit error with the shifted probes); init returns it with deterministic, dm_sweeps or shard_total_pos.  Two more 2-D FFTs per
                                    frame and mode, one launch-sized buffer of per-frame probes in the workspace.  Copied at init.  */
 } ptycho_params;

@@ -17,9 +17,9 @@ namespace ptycho {
 
 struct YX { int y, x; };
 
-enum RowFwdMode { RF_EXIT = 0, RF_DM = 1, RF_PLAIN = 2, RF_EXIT_PJ = 3 };   // _PJ: per-frame probes (sub-pixel positions, R28)
+enum RowFwdMode { RF_EXIT = 0, RF_DM = 1, RF_PLAIN = 2, RF_EXIT_PJ = 3, RF_DM_PJ = 4 };   // _PJ: per-frame probes (sub-pixel positions, R28)
 enum ColMode { CM_FULL = 0, CM_ERRONLY = 1, CM_PLAIN_FWD = 2, CM_PLAIN_INV = 3 };
-enum RowInvMode { RI_MINIBATCH = 0, RI_DM = 1, RI_REVISED = 2, RI_PLAIN = 3, RI_LSQ_PF = 4, RI_MINIBATCH_PJ = 5 };
+enum RowInvMode { RI_MINIBATCH = 0, RI_DM = 1, RI_REVISED = 2, RI_PLAIN = 3, RI_LSQ_PF = 4, RI_MINIBATCH_PJ = 5, RI_DM_PJ = 6 };
 
 #ifndef PTYCHO_THREADS
 #define PTYCHO_THREADS 256
@@ -49,6 +49,7 @@ struct FrameArgs {
     const float2* __restrict__ twi; // twiddles [b*E + ka]
     float2* Pj;                     // _PJ modes: this launch's per-frame probes P_jk = S_delta_j[P_k], nframes x K x N x N (like S); the
                                     // inverse row pass overwrites them with the probe terms conj(O_j) chi_jk (R28)
+    float2* Gj;                     // RF_DM_PJ: the lagged probe terms conj(O_j) psi_jk of this launch's frames, kept per frame (shifted back later)
 };
 
 template <int N> struct Geo {
@@ -115,13 +116,14 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_fw
         const size_t off = ((size_t)k * N + y) * N;
         float2 v[E];
 #pragma unroll
-        for (int i = 0; i < E; ++i) v[i] = cmul(MODE == RF_EXIT_PJ ? a.Pj[fr + off + t + T * i] : __ldg(a.P + off + t + T * i), o[i]);   // psi_O = P_k O_j
-        if (MODE == RF_DM) {
+        for (int i = 0; i < E; ++i) v[i] = cmul((MODE == RF_EXIT_PJ || MODE == RF_DM_PJ) ? a.Pj[fr + off + t + T * i] : __ldg(a.P + off + t + T * i), o[i]);   // psi_O = P_k O_j
+        if (MODE == RF_DM || MODE == RF_DM_PJ) {
             const float2* prow = a.psi + fr + off;
 #pragma unroll
             for (int i = 0; i < E; ++i) {
                 const float2 s = prow[t + T * i];
-                red_add(a.nP + off + t + T * i, cmulc(s, o[i]));                        // conj(O_j) psi_j (lagged, R4)
+                if (MODE == RF_DM_PJ) a.Gj[fr + off + t + T * i] = cmulc(s, o[i]);      // kept per frame: shifted back before it is summed (R28)
+                else red_add(a.nP + off + t + T * i, cmulc(s, o[i]));                   // conj(O_j) psi_j (lagged, R4)
                 v[i] = make_float2(2.f * v[i].x - s.x, 2.f * v[i].y - s.y);             // reflector
             }
         }
@@ -131,7 +133,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_fw
         for (int r = 0; r < E; ++r) srow[freq_b<N>(t, r)] = v[r];
         __syncwarp();
     }
-    if (MODE == RF_DM) {
+    if (MODE == RF_DM || MODE == RF_DM_PJ) {
 #pragma unroll
         for (int i = 0; i < E; ++i) red_add(a.dP + (size_t)y * N + t + T * i, o[i].x * o[i].x + o[i].y * o[i].y);
     }
@@ -318,10 +320,10 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads, (N >= 512
 #pragma unroll
         for (int r = 0; r < E; ++r) {
             const int x = pos_a_inv<N>(t, r);
-            const float2 p = MODE == RI_MINIBATCH_PJ ? a.Pj[fr + off + x] : __ldg(a.P + off + x);
+            const float2 p = (MODE == RI_MINIBATCH_PJ || MODE == RI_DM_PJ) ? a.Pj[fr + off + x] : __ldg(a.P + off + x);
             const float2 po = cmul(p, o[r]);            // psi_O
             float2 w;
-            if (MODE == RI_DM) {
+            if (MODE == RI_DM || MODE == RI_DM_PJ) {
                 float2* ps = a.psi + fr + off + x;
                 const float2 s = *ps;
                 const float2 phi = make_float2(2.f * po.x - s.x, 2.f * po.y - s.y);
@@ -874,6 +876,15 @@ __global__ void k_lsq_cross_pj(const float2* __restrict__ O, const float2* __res
         for (int w = 1; w < (int)blockDim.x / 32; ++w) { a12 += sa[w]; a22 += sb[w]; }
         partX[blockIdx.x * gridDim.y + blockIdx.y] = a12; partA22[blockIdx.x * gridDim.y + blockIdx.y] = a22;
     }
+}
+// psi_jk = P_jk O_j for the slots of one launch (R4 initial exit waves with per-frame probes).  grid (nslots, K n^2 / 256)
+__global__ void k_init_psi_pj(float2* __restrict__ psi, const float2* __restrict__ O, int W, const float2* __restrict__ Pj, int K, int n,
+                              const YX* __restrict__ pos, const int* __restrict__ frames) {
+    const size_t nn = (size_t)n * n, i = (size_t)blockIdx.y * blockDim.x + threadIdx.x;
+    if (i >= nn * K) return;
+    const size_t q = i % nn;
+    const YX p0 = pos[frames[blockIdx.x]];
+    psi[(size_t)blockIdx.x * K * nn + i] = cmul(Pj[(size_t)blockIdx.x * K * nn + i], O[(size_t)(p0.y + (int)(q / n)) * W + p0.x + (int)(q % n)]);
 }
 // dst = src * s (element-wise)
 __global__ void k_scale_to(float2* __restrict__ dst, const float2* __restrict__ src, size_t n, float s) {

@@ -202,7 +202,7 @@ int ncb_of(int n);
 // D = X = 8 against D = 4, X = 0 is 9.3 ms against 12.4 ms), and M shrinks until the ring fits the L2 share.
 void mega_config(ptycho_ctx* c) {
     c->mega_M = c->mega_D = c->mega_R = 0;
-    if (c->K != 1 || c->par.disable_dm) return;
+    if (c->K != 1 || c->par.disable_dm || c->par.subpixel_yx) return;   // (sub-pixel positions: per-frame probes, three-pass kernels)
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) { int v = 0; if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v; }
     cudaGetLastError();
@@ -312,6 +312,8 @@ template <int N> ptycho_status set_attrs(ptycho_ctx* c) {
     CU(cudaFuncSetAttribute(k_rows_fwd<N, RF_DM>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_fwd<N, RF_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_fwd<N, RF_EXIT_PJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_rows_fwd<N, RF_DM_PJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
+    CU(cudaFuncSetAttribute(k_rows_inv<N, RI_DM_PJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_inv<N, RI_MINIBATCH_PJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_inv<N, RI_MINIBATCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
     CU(cudaFuncSetAttribute(k_rows_inv<N, RI_DM>, cudaFuncAttributeMaxDynamicSharedMemorySize, rows));
@@ -362,6 +364,7 @@ template <int N> void launch_passes(ptycho_ctx* c, const FrameArgs& a, int nfram
         if (fwd == RF_EXIT) k_rows_fwd<N, RF_EXIT><<<grid, blk, sr, s>>>(a);
         else if (fwd == RF_DM) k_rows_fwd<N, RF_DM><<<grid, blk, sr, s>>>(a);
         else if (fwd == RF_EXIT_PJ) k_rows_fwd<N, RF_EXIT_PJ><<<grid, blk, sr, s>>>(a);
+        else if (fwd == RF_DM_PJ) k_rows_fwd<N, RF_DM_PJ><<<grid, blk, sr, s>>>(a);
         else k_rows_fwd<N, RF_PLAIN><<<grid, blk, sr, s>>>(a);
     });
     if (col >= 0) LAUNCH(c, PTYCHO_K_COLS, {
@@ -376,6 +379,7 @@ template <int N> void launch_passes(ptycho_ctx* c, const FrameArgs& a, int nfram
         else if (inv == RI_REVISED) k_rows_inv<N, RI_REVISED><<<grid, blk, sr, s>>>(a);
         else if (inv == RI_LSQ_PF) k_rows_inv<N, RI_LSQ_PF><<<grid, blk, sr, s>>>(a);
         else if (inv == RI_MINIBATCH_PJ) k_rows_inv<N, RI_MINIBATCH_PJ><<<grid, blk, sr, s>>>(a);
+        else if (inv == RI_DM_PJ) k_rows_inv<N, RI_DM_PJ><<<grid, blk, sr, s>>>(a);
         else k_rows_inv<N, RI_PLAIN><<<grid, blk, sr, s>>>(a);
     });
 }
@@ -434,6 +438,17 @@ ptycho_status build_batches(ptycho_ctx* c, int np) {
     return PTYCHO_OK;
 }
 
+// Unscaled batched 2-D FFT of `count` N x N frames in place (the plain variants of the three-pass kernels).
+void plain_fft2(ptycho_ctx* c, float2* buf, int count, bool inverse) {
+    const size_t nn = (size_t)c->N * c->N;
+    for (int f0 = 0; f0 < count; f0 += 32768) {             // frames ride in gridDim.y
+        FrameArgs a = base_args(c);
+        a.S = buf + (size_t)f0 * nn; a.K = 1;
+        if (!inverse) passes(c, a, std::min(32768, count - f0), RF_PLAIN, CM_PLAIN_FWD, -1);
+        else passes(c, a, std::min(32768, count - f0), -1, CM_PLAIN_INV, RI_PLAIN);
+    }
+}
+
 // phase: 1 = up to the overlap sums (a1-a9), 2 = the normalising updates (a10), 3 = both.  A shard of a multi-GPU scan runs the
 // two halves separately (ptycho_shard_begin / _end) so that the caller can add the other shards' sums in between.
 ptycho_status dm_iteration(ptycho_ctx* c, int phase = 3) {
@@ -443,7 +458,7 @@ ptycho_status dm_iteration(ptycho_ctx* c, int phase = 3) {
     // 5 GB write and read at config 2); the other forms of the cycle read the store, so it is written first.
     const bool fresh = !c->psi_valid;
     const bool fresh_in_kernel = fresh && c->mega_M > 0 && !c->par.deterministic;
-    if (fresh && !fresh_in_kernel) {
+    if (fresh && !fresh_in_kernel && !c->sub_frac) {
         const dim3 g(c->J, (unsigned)((knn + 255) / 256));   // frame index in grid.x: J may exceed 65535
         LAUNCH(c, PTYCHO_K_OTHER, (k_init_psi<<<g, 256, 0, c->stream>>>(c->psi, c->O, c->W, c->P, c->K, c->N, c->pos, c->dm_frames)));
     }
@@ -489,6 +504,30 @@ ptycho_status dm_iteration(ptycho_ctx* c, int phase = 3) {
             });
         });
         }
+    } else if (c->sub_frac) {
+        // Sub-pixel positions (R28): per launch the frames' shifted probes; the lagged probe terms conj(O_j) psi_jk stay per frame
+        // (sub_dPj), are transformed, multiplied by conj(ramp_j) and summed in Fourier space; one inverse transform gives n_P.
+        const float inv_n2 = 1.0f / ((float)c->N * (float)c->N);
+        CU(cudaMemcpyAsync(c->sub_FP, c->P, knn * 8, cudaMemcpyDeviceToDevice, c->stream));
+        plain_fft2(c, c->sub_FP, c->K, false);
+        CU(cudaMemsetAsync(c->sub_nPF, 0, knn * 8, c->stream));
+        for (int s0 = 0; s0 < c->J; s0 += c->chunk) {
+            const int nf = std::min(c->chunk, c->J - s0);
+            const dim3 gr(nf, (unsigned)((knn + 255) / 256));
+            LAUNCH(c, PTYCHO_K_OTHER, (k_sub_ramp<<<gr, 256, 0, c->stream>>>(c->sub_Pj, c->sub_FP, c->sub_frac, c->dm_frames + s0, c->K, c->N, inv_n2)));
+            plain_fft2(c, c->sub_Pj, nf * c->K, true);
+            if (fresh) LAUNCH(c, PTYCHO_K_OTHER, (k_init_psi_pj<<<gr, 256, 0, c->stream>>>(c->psi + (size_t)s0 * knn, c->O, c->W, c->sub_Pj, c->K, c->N, c->pos, c->dm_frames + s0)));
+            FrameArgs a = base_args(c);
+            a.psi = c->psi + (size_t)s0 * knn;
+            a.frames = c->dm_frames + s0;
+            a.e_part = c->e_part + (size_t)s0 * ncb;
+            a.Pj = c->sub_Pj; a.Gj = c->sub_dPj;
+            passes(c, a, nf, RF_DM_PJ, CM_FULL, RI_DM_PJ);
+            plain_fft2(c, c->sub_dPj, nf * c->K, false);
+            LAUNCH(c, PTYCHO_K_OTHER, (k_sub_acc<<<(unsigned)((knn + 255) / 256), 256, 0, c->stream>>>(c->sub_nPF, c->sub_dPj, c->sub_frac, c->dm_frames + s0, nf, c->K, c->N)));
+        }
+        plain_fft2(c, c->sub_nPF, c->K, true);
+        LAUNCH(c, PTYCHO_K_OTHER, (k_scale_to<<<ew_blocks(knn), 256, 0, c->stream>>>(c->nP, c->sub_nPF, knn, inv_n2)));
     } else
     for (int s0 = 0; s0 < c->J; s0 += c->chunk) {
         const int nf = std::min(c->chunk, c->J - s0);
@@ -532,17 +571,6 @@ updates:
     CU(cudaGetLastError());
     c->psi_valid = true;                                    // only once every launch of the iteration has been accepted
     return PTYCHO_OK;
-}
-
-// Unscaled batched 2-D FFT of `count` N x N frames in place (the plain variants of the three-pass kernels).
-void plain_fft2(ptycho_ctx* c, float2* buf, int count, bool inverse) {
-    const size_t nn = (size_t)c->N * c->N;
-    for (int f0 = 0; f0 < count; f0 += 32768) {             // frames ride in gridDim.y
-        FrameArgs a = base_args(c);
-        a.S = buf + (size_t)f0 * nn; a.K = 1;
-        if (!inverse) passes(c, a, std::min(32768, count - f0), RF_PLAIN, CM_PLAIN_FWD, -1);
-        else passes(c, a, std::min(32768, count - f0), -1, CM_PLAIN_INV, RI_PLAIN);
-    }
 }
 
 ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
@@ -906,7 +934,7 @@ ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
     if (alg != PTYCHO_DM && c->par.deterministic) return fail(c, PTYCHO_EUNSUPPORTED, "deterministic mode covers DM only");
     if (alg == PTYCHO_DM && !c->psi) return fail(c, PTYCHO_ESTATE, "DM needs the exit-wave store (disable_dm was set)");
     if (c->par.shard_total_pos > 0) return fail(c, PTYCHO_ESTATE, "a shard is driven by ptycho_shard_begin / ptycho_shard_end");
-    if (c->sub_frac && alg != PTYCHO_EPIE_MB && alg != PTYCHO_LSQML) return fail(c, PTYCHO_EUNSUPPORTED, "sub-pixel positions: PTYCHO_EPIE_MB and PTYCHO_LSQML only");
+    if (c->sub_frac && alg == PTYCHO_LSQML_PF) return fail(c, PTYCHO_EUNSUPPORTED, "sub-pixel positions: not with per-frame LSQML steps");
     if (c->streaming) {
         if (c->present == 0) return fail(c, PTYCHO_ESTATE, "no frame has been appended yet");
         if (alg == PTYCHO_DM && c->present < c->J) return fail(c, PTYCHO_ESTATE, "DM needs every frame (PAPER.md:58); append the rest first");

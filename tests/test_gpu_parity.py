@@ -890,9 +890,8 @@ def test_subpixel_positions_epie_minibatch(B, oracle_mod, n, h, side, step, k, d
     z.iterate("EPIE_MB", 4)
     assert rel(z.fetch_object(), o.O) > 50 * TOL_ITER
     z.destroy()
-    for alg in ("DM", "LSQML_PF"):                           # ePIE-minibatch and LSQML only
-        with pytest.raises(B.PtychoError):
-            g.iterate(alg, 1)
+    with pytest.raises(B.PtychoError):                       # not with per-frame LSQML steps
+        g.iterate("LSQML_PF", 1)
     with pytest.raises(B.PtychoError):
         g.revised_waves(np.arange(2, dtype=np.int32))
     g.destroy()
@@ -921,6 +920,36 @@ def test_subpixel_positions_lsqml(B, oracle_mod, n, h, side, step, k, dtype, bat
         assert ro < TOL_ITER * (it + 1) and rp < TOL_ITER * (it + 1), (it, ro, rp)
     assert np.allclose(g.fetch_steps(), np.array(o.steps), rtol=2e-3, atol=1e-6)
     assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+    g.destroy()
+
+
+@pytest.mark.parametrize("n,h,side,step,k,dtype,pbound,probe_start", [
+    (64, 300, 6, 21, 1, np.uint16, 0.3, 2),
+    (64, 300, 6, 21, 2, np.float32, 0.0, 0),
+    (256, 600, 3, 90, 1, np.uint16, 0.4, 1)])
+def test_subpixel_positions_dm(B, oracle_mod, n, h, side, step, k, dtype, pbound, probe_start):
+    """DM with fractional positions (the three-pass kernels with per-frame probes: the megakernel shares one probe among the frames
+    of an item): exit waves, object, probe and error history against oracle/subpixel.py over six free-running iterations, the
+    first of which forms psi_j = P_jk O_j."""
+    from oracle import subpixel
+    s = synth.make_custom(n, h, side, step, k=k, peak=2e4 if dtype == np.uint16 else None, dtype=dtype, jitter=2, seed=53,
+                          probe_kind="zone")
+    rng = np.random.default_rng(29)
+    frac = rng.uniform(0, 1, (len(s.pos), 2)).astype(np.float32)
+    par = dict(pbound=pbound, probe_start=probe_start)
+    o = subpixel.SubpixelOracle(s.obj0, s.probe0, s.pos, frac, s.intensities, par)
+    g = B.Ptycho(s.obj0, s.probe0, s.pos, s.intensities, B.default_params(subpixel_yx=frac, **par))
+    for it in range(6):
+        o.iterate(1, "DM")
+        g.iterate("DM", 1)
+        ro, rp = rel(g.fetch_object(), o.O), rel(g.fetch_probe(), o.P)
+        assert ro < TOL_RUN and rp < TOL_RUN, (it, ro, rp)
+    assert rel(g.fetch_exit_waves(), o.psi) < TOL_RUN
+    assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+    # switching algorithms keeps working: a minibatch iteration invalidates psi, the next DM iteration re-forms it with the shifted probes
+    o.iterate(1, "EPIE_MB"); g.iterate("EPIE_MB", 1)
+    o.iterate(1, "DM"); g.iterate("DM", 1)
+    assert rel(g.fetch_object(), o.O) < TOL_RUN and rel(g.fetch_exit_waves(), o.psi) < TOL_RUN
     g.destroy()
 
 

@@ -1045,3 +1045,26 @@ def test_dead_frames_and_frames_on_every_border(B, oracle_mod, alg, dtype):
         assert rel(g.fetch_exit_waves(), o.psi) < TOL_RUN
     assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
     g.destroy()
+
+
+def test_more_than_65535_frames(B, oracle_mod):
+    """J = 70 000 small frames: every launch that carries a frame index in a grid dimension has to cope with more than 65 535 of them
+    (gridDim.y is capped there), the three-pass kernels cut the batch into several launches, the DM counters and tile lists index
+    beyond 2^16.  DM (megakernel) and full-batch ePIE against the oracle."""
+    n, h, J = 64, 700, 70000
+    rng = np.random.default_rng(61)
+    obj = synth.make_object(h, h, 12)
+    probe = synth.probe_disk(n, n * 0.3125)[None]
+    pos = rng.integers(0, h - n + 1, (J, 2)).astype(np.int32)
+    _, inten, _ = synth.simulate(obj, probe, pos, 2e3, 5, np.uint16, 8)
+    obj0 = np.ones_like(obj)
+    for alg, par in (("DM", dict(pbound=0.3)), ("EPIE_MB", dict(batch_size=0))):
+        o = oracle_mod.Oracle(obj0, probe, pos, inten, par)
+        g = B.Ptycho(obj0, probe, pos, inten, B.default_params(**par))
+        o.iterate(alg, 2); g.iterate(alg, 2)
+        assert rel(g.fetch_object(), o.O) < TOL_RUN and rel(g.fetch_probe(), o.P) < TOL_RUN, alg
+        assert np.allclose(g.fetch_error(), o.err, rtol=2e-3)
+        if alg == "DM":
+            sel = np.array([0, 65535, 65536, J - 1], np.int32)
+            assert rel(g.fetch_exit_waves(sel), o.psi[sel]) < TOL_RUN
+        g.destroy()

@@ -207,11 +207,11 @@ template <int N, typename TI> __global__ void __launch_bounds__(kThreads) k_tile
 template <int N> struct MegaGeo {
     using G = Geo<N>;
     static constexpr int LINE = (G::LS_ROW > G::LS_COL ? G::LS_ROW : G::LS_COL);
-    static constexpr size_t smem = (size_t)(G::LPB * LINE + 4 * N + G::LPB * N) * sizeof(float2);   // exchange, twiddles, probe rows
+    static constexpr size_t smem = (size_t)(G::LPB * LINE + 2 * N * kTwWords + G::LPB * N) * sizeof(float2);   // exchange, twiddles, probe rows
 };
 
 // ---- pass 1: a1 exit wave, a2 reflector, a9 lagged probe sums, a3 forward row FFTs -> S --------
-template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
+template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(const MegaArgs& m, int blk, int wave, float2* sm, const tw_t* s_tw,
                                                             Deferred& df, bool split) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T, LW = 32 / T;
@@ -225,7 +225,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(co
 #pragma unroll
     for (int i = 0; i < E; ++i) { accN[i] = make_float2(0.f, 0.f); accD[i] = 0.f; }
     const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
-    float2* sP = reinterpret_cast<float2*>(const_cast<float4*>(s_tw) + 2 * N) + l * N;   // this line's probe row, kept for the M slots
+    float2* sP = reinterpret_cast<float2*>(const_cast<tw_t*>(s_tw) + 2 * N) + l * N;   // this line's probe row, kept for the M slots
 #pragma unroll
     for (int i = 0; i < E; ++i) sP[t + T * i] = __ldg(a.P + off + t + T * i);
     __syncwarp();
@@ -290,7 +290,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass1(co
 // S is left untouched; MODE 2 = the whole pass once more for ONE frame whose error turned out to exceed the bound (mega_pass2b
 // below: pass 1 is known to be complete, no wait).  s_lo / s_hi >= 0 restrict the call to those slots of the wave.
 enum { P2_FUSED = 0, P2_ERR_ONLY = 1, P2_REDO = 2 };
-template <int N, bool U16, int MODE> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
+template <int N, bool U16, int MODE> __device__ __forceinline__ void mega_pass2(const MegaArgs& m, int blk, int wave, float2* sm, const tw_t* s_tw,
                                                             float* s_red, Deferred& df, int s_lo = -1, int s_hi = -1) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T, CB = G::LPB;
@@ -375,7 +375,7 @@ template <int N, bool U16, int MODE> __device__ __forceinline__ void mega_pass2(
 // ---- pass 2b of the split form: ONE item per wave.  For every frame of the wave: once all its error partials are there, a frame
 // inside its power bound is passed on to pass 3 at once (the common case: a few microseconds per wave); a frame outside it gets
 // the whole pass 2, all NCB column blocks, from this CTA (rare once the split form is in use).
-template <int N, bool U16> __device__ __forceinline__ void mega_pass2b(const MegaArgs& m, int wave, float2* sm, const float4* s_tw, float* s_red,
+template <int N, bool U16> __device__ __forceinline__ void mega_pass2b(const MegaArgs& m, int wave, float2* sm, const tw_t* s_tw, float* s_red,
                                                                        Deferred& df) {
     using G = Geo<N>;
     const int s_begin = wave * m.M, s_end = min(m.J, (wave + 1) * m.M);
@@ -398,7 +398,7 @@ template <int N, bool U16> __device__ __forceinline__ void mega_pass2b(const Meg
 }
 
 // ---- pass 3: a6 inverse row FFTs, a7 exit-wave update, a8 object scatter-add ---------------------
-template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, int blk, int wave, float2* sm, const float4* s_tw,
+template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(const MegaArgs& m, int blk, int wave, float2* sm, const tw_t* s_tw,
                                                             Deferred& df, bool split) {
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T;
@@ -415,7 +415,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
         for (int k = threadIdx.x & 31; k < s_end - s_begin; k += 32) all_done = all_done && ld_relaxed_gpu(m.cnt2 + s_begin + k) >= 2 * G::NCB;
         if (__all_sync(0xffffffffu, all_done)) return;
     }
-    float2* sP = reinterpret_cast<float2*>(const_cast<float4*>(s_tw) + 2 * N) + l * N;                                      // this line's probe row, kept for the M slots
+    float2* sP = reinterpret_cast<float2*>(const_cast<tw_t*>(s_tw) + 2 * N) + l * N;                                      // this line's probe row, kept for the M slots
 #pragma unroll
     for (int i = 0; i < E; ++i) sP[t + T * i] = __ldg(a.P + off + t + T * i);
     __syncwarp();
@@ -481,7 +481,7 @@ template <int N, bool SYNC = true> __device__ __forceinline__ void mega_pass3(co
 template <int N, bool U16> __global__ void __launch_bounds__(kThreads, (N >= 512 ? 1 : PTYCHO_MEGA_OCC)) k_dm_mega(MegaArgs m) {
     using G = Geo<N>;
     extern __shared__ __align__(16) float2 sm[];
-    float4* s_tw = reinterpret_cast<float4*>(sm + G::LPB * MegaGeo<N>::LINE);
+    tw_t* s_tw = reinterpret_cast<tw_t*>(sm + G::LPB * MegaGeo<N>::LINE);
     __shared__ float s_red[kThreads / 32];
     __shared__ int s_item;
     load_tw(s_tw, m.f.tw, m.f.twi, N);

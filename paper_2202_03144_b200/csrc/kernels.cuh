@@ -58,16 +58,16 @@ template <int N> struct Geo {
     static constexpr int LS_ROW = LineSmem<N>::SIZE + ((T == 8 && (LineSmem<N>::SIZE % 16) != 8) ? 8 : 0);
     static constexpr int LS_COL = LineSmem<N>::SIZE | 1;         // odd: lanes run along lines
     static constexpr int NCB = N / LPB;                          // column blocks (= row blocks) per frame
-    static constexpr size_t smem_rows = (size_t)(LPB * LS_ROW + 4 * N) * sizeof(float2);
+    static constexpr size_t smem_rows = (size_t)(LPB * LS_ROW + 2 * N * kTwWords) * sizeof(float2);
     static size_t smem_cols(int K) {
         (void)K;
-        return (size_t)(LPB * LS_COL + 4 * N) * sizeof(float2) + 64;
+        return (size_t)(LPB * LS_COL + 2 * N * kTwWords) * sizeof(float2) + 64;
     }
 };
 
 // Twiddle tables in shared memory, packed for the two-wide multiply (fft_core.cuh tw_pack): 2 n float4.
-__device__ __forceinline__ void load_tw(float4* s_tw, const float2* tw, const float2* twi, int n) {
-    for (int i = threadIdx.x; i < n; i += kThreads) { s_tw[i] = tw_pack(tw[i]); s_tw[n + i] = tw_pack(twi[i]); }
+__device__ __forceinline__ void load_tw(tw_t* s_tw, const float2* tw, const float2* twi, int n) {
+    for (int i = threadIdx.x; i < n; i += kThreads) { s_tw[i] = tw_store(tw[i], s_tw); s_tw[n + i] = tw_store(twi[i], s_tw); }
 }
 
 __device__ __forceinline__ float load_intensity(const void* I, int itype, size_t idx) {
@@ -88,7 +88,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_rows_fw
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T;
     extern __shared__ __align__(16) float2 sm[];
-    float4* s_tw = reinterpret_cast<float4*>(sm + G::LPB * G::LS_ROW);
+    tw_t* s_tw = reinterpret_cast<tw_t*>(sm + G::LPB * G::LS_ROW);
     load_tw(s_tw, a.tw, a.twi, N);
     const int l = threadIdx.x / T, t = threadIdx.x % T;
     float2* sx = sm + l * G::LS_ROW;
@@ -147,7 +147,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads) k_cols(Fr
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T, CB = G::LPB;
     extern __shared__ __align__(16) float2 sm[];
-    float4* s_tw = reinterpret_cast<float4*>(sm + CB * G::LS_COL);
+    tw_t* s_tw = reinterpret_cast<tw_t*>(sm + CB * G::LS_COL);
     __shared__ float s_red[kThreads / 32];
     load_tw(s_tw, a.tw, a.twi, N);
     const int c = threadIdx.x % CB, t = threadIdx.x / CB;
@@ -272,7 +272,7 @@ template <int N, int MODE> __global__ void __launch_bounds__(kThreads, (N >= 512
     using G = Geo<N>;
     constexpr int E = G::E, T = G::T;
     extern __shared__ __align__(16) float2 sm[];
-    float4* s_tw = reinterpret_cast<float4*>(sm + G::LPB * G::LS_ROW);
+    tw_t* s_tw = reinterpret_cast<tw_t*>(sm + G::LPB * G::LS_ROW);
     load_tw(s_tw, a.tw, a.twi, N);
     const int l = threadIdx.x / T, t = threadIdx.x % T;
     float2* sx = sm + l * G::LS_ROW;

@@ -1068,3 +1068,17 @@ def test_more_than_65535_frames(B, oracle_mod):
             sel = np.array([0, 65535, 65536, J - 1], np.int32)
             assert rel(g.fetch_exit_waves(sel), o.psi[sel]) < TOL_RUN
         g.destroy()
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("PTYCHO_LONG_TESTS"), reason="opt-in (PTYCHO_LONG_TESTS=1): thousands of iterations at full size")
+@pytest.mark.parametrize("cfg,iters", [(2, 3000), (4, 400), (1, 20000)])
+def test_soak_thousands_of_dm_iterations(B, cfg, iters):
+    """The persistent queue over many launches at full size: no hang (the call returns), finite and non-increasing error tail."""
+    import torch
+    s = synth.make_config(cfg)
+    g = B.Ptycho(s.obj0, s.probe0, s.pos, torch.from_numpy(s.intensities).cuda(),
+                 B.default_params(pbound=s.params.get("pbound", s.params.get("pbound_dm", 0.0))))
+    g.iterate("DM", iters)
+    e = g.fetch_error()
+    assert len(e) == iters and np.isfinite(e).all() and e[-1] < e[0] and e[-1] <= 1.05 * e[iters // 2]
+    g.destroy()

@@ -409,6 +409,7 @@ struct Scalars {            // device-resident scalars (no host round trip insid
     double sum_I;           // sum of unmasked intensities of the frames present
     double sum_I_iter;      // its value when the running iteration started (frames may be appended meanwhile)
     float eps_O, eps_P;     // DM blend constants (fixed at init)
+    float max_p2s[2];       // ePIE-minibatch: max_r sum_k |P_k|^2 of the probe the NEXT batch starts from, ping-pong (k_epie_update)
     unsigned int max_bits;  // scratch for atomicMax on non-negative floats
 };
 
@@ -641,17 +642,36 @@ __global__ void k_set_steps(Scalars* sc, float a, float b, double* steps_out) {
 
 // ePIE-minibatch (R8) in ONE pass over a canvas: x += alpha n / (d + delta max); zero n and d.  which = 0: object (max = max_p2),
 // 1: probe (max = max_dp).  (LSQML needs the directions before it knows its steps: k_direction, then k_apply.)
-__global__ void k_epie_update(float2* x, float2* n, float* d, size_t plane, int modes, float delta, float alpha, const Scalars* sc, int which,
-                              int update) {
-    const float reg = delta * (which ? sc->max_dp : sc->max_p2);
+// The small per-batch jobs ride along instead of being launches of their own (config 1 is launch-bound: ten launches per batch
+// became six).  which = 0 (object): the regulariser comes from sc->max_p2 (pi < 0) or sc->max_p2s[pi]; thread 0 zeroes sc->max_dp and
+// sc->max_p2s[pw] for the kernels that follow (nobody reads them here).  which = 1 (probe): the step record is written, and with
+// pw >= 0 the maximum of sum_k |P_k|^2 of the UPDATED probe is left in sc->max_p2s[pw] for the next batch.
+__global__ void k_epie_update(float2* x, float2* n, float* d, size_t plane, int modes, float delta, float alpha, Scalars* sc, int which,
+                              int update, int pi, int pw, double* steps_out, float step_a, float step_b) {
+    const float reg = delta * (which ? sc->max_dp : (pi < 0 ? sc->max_p2 : sc->max_p2s[pi]));
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        if (!which) { sc->max_dp = 0.f; if (pw >= 0) sc->max_p2s[pw] = 0.f; }
+        else if (steps_out) { steps_out[0] = step_a; steps_out[1] = step_b; }
+    }
+    float pm = 0.f;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < plane; i += (size_t)gridDim.x * blockDim.x) {
         const float st = alpha / (d[i] + reg);
+        float p2 = 0.f;
         for (int k = 0; k < modes; ++k) {
             const size_t q = (size_t)k * plane + i;
-            if (update) { const float2 nv = n[q]; float2 xv = x[q]; xv.x = fmaf(st, nv.x, xv.x); xv.y = fmaf(st, nv.y, xv.y); x[q] = xv; }
+            if (update || (which && pw >= 0)) {
+                float2 xv = x[q];
+                if (update) { const float2 nv = n[q]; xv.x = fmaf(st, nv.x, xv.x); xv.y = fmaf(st, nv.y, xv.y); x[q] = xv; }
+                p2 = fmaf(xv.x, xv.x, fmaf(xv.y, xv.y, p2));
+            }
             n[q] = make_float2(0.f, 0.f);
         }
+        pm = fmaxf(pm, p2);
         d[i] = 0.f;
+    }
+    if (which && pw >= 0) {
+        for (int s = 16; s > 0; s >>= 1) pm = fmaxf(pm, __shfl_xor_sync(0xffffffffu, pm, s));
+        if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<unsigned int*>(&sc->max_p2s[pw]), __float_as_uint(pm));
     }
 }
 

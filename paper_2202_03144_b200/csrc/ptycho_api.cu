@@ -91,6 +91,7 @@ struct ptycho_ctx {
     std::vector<int> batch_order_h, mb_h;
     long long n_steps = 0;
     bool psi_valid = false;
+    int epie_pi = -1;                          // ePIE-minibatch: which sc->max_p2s slot holds the current probe's maximum (-1: none, k_probe_max runs)
     // sub-pixel positions (params.subpixel_yx, R28): fractions (device, caller numbering), F[P], Fourier-space probe numerator,
     // per-frame probes of one launch
     float* sub_frac = nullptr;
@@ -580,8 +581,12 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
     const int nb = (int)c->mb_offsets.size() - 1;
     for (int b = 0; b < nb; ++b) {
         const int b0 = c->mb_offsets[b], b1 = c->mb_offsets[b + 1];
-        CU(cudaMemsetAsync(&c->sc->max_p2, 0, sizeof(float), c->stream));
-        LAUNCH(c, PTYCHO_K_UPDATE, (k_probe_max<<<64, 256, 0, c->stream>>>(c->P, c->K, (int)nn, c->sc)));
+        const bool epie = alg == PTYCHO_EPIE_MB;
+        if (!epie) c->epie_pi = -1;
+        if (!epie || c->epie_pi < 0) {                      // (ePIE: the previous batch's probe update left the maximum behind)
+            CU(cudaMemsetAsync(&c->sc->max_p2, 0, sizeof(float), c->stream));
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_probe_max<<<64, 256, 0, c->stream>>>(c->P, c->K, (int)nn, c->sc)));
+        }
         if (c->sub_frac) {
             // Sub-pixel positions (R28).  Per launch: the frames' shifted probes P_jk = F^-1[F[P_k] ramp_j] into sub_Pj, the cycle with
             // them (the inverse row pass leaves the probe terms conj(O_j) chi_jk in sub_Pj), their spectra times conj(ramp_j) summed
@@ -618,13 +623,14 @@ ptycho_status minibatch_iteration(ptycho_ctx* c, ptycho_alg alg) {
         const bool lsq = alg == PTYCHO_LSQML, pfm = alg == PTYCHO_LSQML_PF;
         const int gO = ew_blocks(HW), gP = ew_blocks(nn);
         if (!lsq && !pfm) {                                 // ePIE: directions and steps in one pass per canvas
-            LAUNCH(c, PTYCHO_K_UPDATE, (k_epie_update<<<gO, 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->par.delta_obj, c->par.alpha_obj, c->sc, 0, 1)));
-            if (upd) {
-                CU(cudaMemsetAsync(&c->sc->max_dp, 0, sizeof(float), c->stream));
-                LAUNCH(c, PTYCHO_K_UPDATE, (k_real_max<<<64, 256, 0, c->stream>>>(c->dP, (int)nn, c->sc)));
-            }
-            LAUNCH(c, PTYCHO_K_UPDATE, (k_epie_update<<<gP, 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->par.delta_probe, c->par.alpha_probe, c->sc, 1, upd)));
-            if (c->n_steps < kStepCap) LAUNCH(c, PTYCHO_K_UPDATE, (k_set_steps<<<1, 1, 0, c->stream>>>(c->sc, c->par.alpha_obj, upd ? c->par.alpha_probe : 0.f, c->steps + 2 * c->n_steps)));
+            const int pi = c->epie_pi, pw = pi < 0 ? 0 : 1 - pi;
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_epie_update<<<gO, 256, 0, c->stream>>>(c->O, c->nO, c->dO, HW, 1, c->par.delta_obj, c->par.alpha_obj, c->sc, 0, 1,
+                                                                                 pi, pw, nullptr, 0.f, 0.f)));   // (zeroes max_dp and max_p2s[pw])
+            if (upd) LAUNCH(c, PTYCHO_K_UPDATE, (k_real_max<<<64, 256, 0, c->stream>>>(c->dP, (int)nn, c->sc)));
+            LAUNCH(c, PTYCHO_K_UPDATE, (k_epie_update<<<gP, 256, 0, c->stream>>>(c->P, c->nP, c->dP, nn, c->K, c->par.delta_probe, c->par.alpha_probe, c->sc, 1, upd,
+                                                                                 -1, pw, c->n_steps < kStepCap ? c->steps + 2 * c->n_steps : nullptr,
+                                                                                 c->par.alpha_obj, upd ? c->par.alpha_probe : 0.f)));
+            c->epie_pi = pw;
             ++c->n_steps;
             continue;
         }
@@ -941,6 +947,7 @@ ptycho_status ptycho_iterate(ptycho_ctx* c, ptycho_alg alg, int n_iters) {
         CU(cudaStreamWaitEvent(c->stream, c->ev_append, 0));   // the frames appended so far have been copied and re-tiled
     }
     if (alg != PTYCHO_DM) { ptycho_status st = build_batches(c, c->present); if (st != PTYCHO_OK) return st; }
+    c->epie_pi = -1;                                        // the probe may have changed since the last call (set_probe, DM, orthogonalisation)
     k_snap_sum_I<<<1, 1, 0, c->stream>>>(c->sc);
     ++c->launches;
     for (int it = 0; it < n_iters; ++it) {
